@@ -1,0 +1,197 @@
+/*
+ * lsd.h -- C ABI of liblsd_b200.so: the window-verification hot path of Langevin Speculative
+ * Dynamics (LSD, arxiv/paper_2606_02455) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are /root/reference/PAPER.md:<line> plus section / equation / algorithm; readings of
+ * points where the paper is silent are numbered R1..R16 / M1..M9 in DESIGN.md.
+ *
+ * The problem statement fixes the arguments (PAPER.md:41 positions q, momenta p, diagonal mass
+ * matrix M; :45-50, :66 temperature T, friction gamma, time step dt; :76 a draft and a target
+ * force field; :572 initial state x_0).  "BAOAB" in the task metadata is implemented as the paper's
+ * ABOBA splitting (Eq. 2; Alg. 2 :568); R1.
+ *
+ * Conventions
+ *   - plain C, no exceptions; every call returns an lsd_status (0 = LSD_OK, negative = error) and
+ *     leaves a message retrievable with lsd_last_error().
+ *   - units: Angstrom, fs, eV, K; masses in amu at the boundary (1 amu A^2/fs^2 = 103.642696 eV).
+ *   - vectors over atoms are component-major ("SoA"): q[c * n_atoms + i], c = 0,1,2.  Batches of
+ *     states are state-major: q[(k * 3 + c) * n_atoms + i].
+ *   - pointers inside lsd_system / lsd_potential and q0/p0 of lsd_init are HOST pointers; they are
+ *     copied during lsd_init and need not outlive it.
+ *   - `where` arguments say whether a bulk pointer is host (LSD_HOST) or device (LSD_DEVICE)
+ *     memory.  Device buffers are owned by the caller (e.g. torch tensors).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work on it
+ *     and return immediately, except where a host-visible result is produced (stated below).
+ *   - the context owns all internal device memory; one context must not be used from two host
+ *     threads at once.
+ *   - there is no CPU fallback: without a CUDA device lsd_init fails with LSD_ERR_CUDA.
+ */
+#ifndef LSD_H
+#define LSD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t lsd_status;
+#define LSD_OK                  0
+#define LSD_ERR_INVALID_ARG    (-1)
+#define LSD_ERR_CUDA           (-2)
+#define LSD_ERR_OOM            (-3)
+#define LSD_ERR_STATE          (-4)   /* call order violated                                        */
+#define LSD_ERR_UNSUPPORTED    (-5)
+#define LSD_ERR_NBR_OVERFLOW   (-6)   /* a neighbour row exceeded its capacity                      */
+#define LSD_ERR_SKIN_VIOLATED  (-7)   /* an atom moved > skin/2 from the list's reference state     */
+#define LSD_ERR_NONFINITE      (-8)
+
+#define LSD_HOST    0
+#define LSD_DEVICE  1
+
+#define LSD_SCHEME_ABOBA 0            /* A(1/2) B(1/2) O B(1/2) A(1/2), Eq. 2        */
+
+/* arithmetic of the MLIP (state, priors, transport reductions are always fp64)                     */
+#define LSD_FP32     1                /* fp32 FMA pipes                                              */
+#define LSD_BF16_TC  2                /* bf16 tcgen05 filter contractions, fp32 accumulation         */
+
+/* which potential */
+#define LSD_DRAFT   0
+#define LSD_TARGET  1
+
+/* pair-parameter table columns, per ordered species pair (zero = term off) */
+#define LSD_PAIR_COLS 8               /* lj_eps, lj_sigma, lj_rc, morse_D, morse_a, morse_r0, morse_rc, tether_k */
+
+typedef struct lsd_ctx lsd_ctx;
+
+typedef struct {
+    int32_t n_atoms, n_species;
+    int32_t periodic;                 /* 1: orthorhombic periodic box (box >= 2 (r_c + skin) required); 0: vacuum */
+    double  box[3];
+    const int32_t* species;           /* [n_atoms], 0 <= s < n_species                               */
+    const double*  mass_amu;          /* [n_atoms] diagonal of M                       */
+    int32_t n_bonds;  const int32_t* bonds;  /* [n_bonds][2]                                        */
+    const double*  bond_k;  const double* bond_r0;          /* U = k/2 (r - r0)^2                   */
+    int32_t n_angles; const int32_t* angles; /* [n_angles][3] (end, apex, end)                      */
+    const double*  angle_k; const double* angle_theta0;     /* U = k/2 (theta - theta0)^2, radians  */
+} lsd_system;
+
+/* SchNet-style network, M1-M8.  weights: flat fp64, emb[ns][F]; per block W_in[F][F],
+ * W_f1[F][R], W_f2[F][F], W_o1[F][F], W_o2[F][F] (row-major [out][in]); W_r1[F/2][F]; w_r2[F/2]. */
+typedef struct {
+    int32_t width;                    /* F in {32, 64, 128}; 0 = no network                          */
+    int32_t n_blocks;                 /* T >= 1                                                      */
+    int32_t n_rbf;                    /* R = 32                                                      */
+    int32_t n_species;
+    double  cutoff;                   /* r_c (A)                                                     */
+    double  energy_scale;             /* alpha                                                       */
+    const double* weights;
+} lsd_mlip;
+
+typedef struct {
+    int32_t n_species;
+    int32_t use_bonded;               /* include the system's bonds and angles                        */
+    const double* pair;               /* [n_species][n_species][LSD_PAIR_COLS]                       */
+    lsd_mlip mlip;
+} lsd_potential;
+
+typedef struct {
+    double   temperature_K, friction_per_fs, dt_fs;
+    uint64_t seed;                    /* Philox4x32-10 key (R5)                                      */
+    int32_t  scheme;                  /* LSD_SCHEME_ABOBA                                            */
+    int32_t  precision;               /* LSD_FP32 | LSD_BF16_TC                                      */
+    int32_t  k_max;                   /* largest window length K that will be requested (<= 64)      */
+    double   skin;                    /* Verlet skin (A) of the window-shared neighbour lists        */
+} lsd_config;
+
+typedef struct {
+    int64_t windows, committed_steps, rejections;
+    double  beta_sum;                 /* sum over committed steps of erf(sqrt(S2)/sqrt 8), Eq. 9     */
+    int64_t step;                     /* committed step index n of the base state                    */
+} lsd_stats;
+
+/* Create a context.  q0: [3][n_atoms].  p0: [3][n_atoms] or NULL -> Maxwell-Boltzmann momenta
+ * p_i = sqrt(m_i k_B T) xi from Philox stream tag 2 (R12).  Builds the first neighbour lists to size
+ * the rows (synchronises).  Errors: INVALID_ARG (sizes, widths, box < 2 (r_c + skin)), CUDA, OOM. */
+lsd_status lsd_init(const lsd_config* cfg, const lsd_system* sys, const lsd_potential* draft,
+                    const lsd_potential* target, const double* q0, const double* p0, lsd_ctx** out);
+void        lsd_destroy(lsd_ctx* ctx);
+const char* lsd_last_error(const lsd_ctx* ctx);   /* ctx may be NULL: error of the last failed lsd_init */
+
+/* a0 (PAPER.md:584-593 DRAFT_STEP; Eq. 2, Eq. 7): draft K ABOBA steps from the current draft head
+ * (the base state, or y_K of the previous, still unverified window), storing per step q_half_j,
+ * draft forces F~_j and y_j in the next window slot.  Builds the window-shared Verlet lists from the
+ * head state first.  Noise xi_j = Philox(seed; step index n + j, atom) (R5).  Asynchronous.
+ * Errors: INVALID_ARG (K < 1 or > k_max), STATE (two unverified windows already drafted). */
+lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream);
+
+/* a1 + a2 (PAPER.md:598-599 VERIFY_STEP): one batched target force evaluation F_j = F(q_half_j) for
+ * all K draft states of the oldest unverified window (waits on the rollout's event).  Asynchronous. */
+lsd_status lsd_verify_window(lsd_ctx* ctx, int32_t K, void* stream);
+
+/* a3 + a4 + a5 (PAPER.md:108-111 Eq. 8 REFLECTIONVERIFY; :424 l = min{j : x_j != y_j}; :602 map g):
+ * per step d = (b/sigma)(F~ - F), S1 = xi.d, S2 = d.d, ell = -S1 - S2/2, u_j ~ U(0,1);
+ * reject_j = S2 > 0 and ln u_j > min(0, ell).  The first rejected step l is overridden with
+ * p* = c1 p_{l-1} + b F_l + sigma (xi_l - 2 (S1/S2) d_l), q* = q_half_l + (dt/2) p* / m and becomes the
+ * new base state; with no rejection y_K does.  SYNCHRONISES on `stream` and returns
+ * *first_reject (0 = none, else 1..K) and *n_commit (l, or K).  Errors: STATE, SKIN_VIOLATED /
+ * NBR_OVERFLOW (nothing is committed; enlarge with lsd_set_skin and redo the window), NONFINITE. */
+lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* first_reject, int32_t* n_commit);
+
+/* a6 (PAPER.md:78 "flush them and restart drafting from the just overridden state"; :612 y <- x'):
+ * book-keeping after lsd_transport_accept.  first_reject == 0: the K drafted states are committed,
+ * a speculative next window (if drafted) stays valid.  first_reject == l > 0: l states are committed,
+ * any speculative window is discarded and the draft head returns to the base state (also for l == K). */
+lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject);
+
+/* Convenience driver: repeat {rollout, verify (+ speculative rollout of the next window on a second
+ * internal stream when overlap != 0), transport, rollback} until n_steps more steps are committed
+ * (the last window is shortened).  Synchronous. */
+lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream);
+
+/* Base state x_n: q, p [3][n_atoms] (either may be NULL), *step = n.  Synchronises. */
+lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int32_t where);
+lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t step, int32_t where);
+lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out);
+
+/* Committed state j (1..n_commit) of the window most recently passed to lsd_transport_accept. */
+lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where);
+
+/* Debug rows of that window (parity tests).  `what`: */
+#define LSD_DBG_QHALF    0   /* double [K][3][n]   positions after the first A half-step                */
+#define LSD_DBG_FDRAFT   1   /* double [K][3][n]   F~_j                                                */
+#define LSD_DBG_FTARGET  2   /* double [K][3][n]   F_j                                                 */
+#define LSD_DBG_S1       3   /* double [K]                                                             */
+#define LSD_DBG_S2       4   /* double [K]                                                             */
+#define LSD_DBG_ELL      5   /* double [K]         log-ratio                                           */
+#define LSD_DBG_LNU      6   /* double [K]         ln u_j                                              */
+#define LSD_DBG_REJECT   7   /* int32  [K]                                                             */
+#define LSD_DBG_XI       8   /* double [K][3][n]   the regenerated normals                             */
+#define LSD_DBG_YP       9   /* double [K][3][n]   draft momenta p~_j                                  */
+#define LSD_DBG_YQ      10   /* double [K][3][n]   draft positions q~_j                                */
+lsd_status lsd_get_window_debug(lsd_ctx* ctx, int32_t what, void* out, int32_t where);
+
+/* One batched force evaluation outside the LSD loop (parity, benchmarks): F[b] = F_which(q[b]) for
+ * n_states states, q and F [n_states][3][n_atoms].  All states must lie within skin/2 of state 0
+ * (they share one Verlet list) else SKIN_VIOLATED.  energy_nn (may be NULL): [n_states][n_atoms]
+ * per-atom network energies alpha e_i (M6).  Synchronises. */
+lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const double* q, double* F,
+                           double* energy_nn, int32_t where, void* stream);
+
+/* Effective directed edge set of state b of the last lsd_eval_forces / lsd_verify_window call
+ * (T1): kind 0 = network list (r < r_c), 1 = pair-prior list (r < r_c(s_i, s_j)).
+ * Host outputs: start[n_atoms + 1], idx[cap], shifts[cap][3]; *n_edges = total (may exceed cap, then
+ * only cap entries are written).  Rows are sorted by (j, shift).  Synchronises. */
+lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t b, int64_t cap,
+                             int64_t* start, int32_t* idx, int8_t* shifts, int64_t* n_edges);
+
+lsd_status lsd_set_skin(lsd_ctx* ctx, double skin);
+
+/* Number of kernels this library has launched on behalf of ctx (bench.py's gpu_launches). */
+int64_t     lsd_launch_count(const lsd_ctx* ctx);
+const char* lsd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSD_H */

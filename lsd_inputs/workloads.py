@@ -131,13 +131,13 @@ def make_mlip(F: int, T: int, R: int, cutoff: float, ns: int, seed: int, alpha: 
 # reference configuration.  Written by oracle/calibrate_alpha.py (calls only oracle/);
 # stored here as plain data so that the product path never needs the oracle.
 ALPHA = {
-    ("cfg2", "target"): 1.0,
-    ("cfg2", "draft"): 1.0,
-    ("cfg3", "target"): 1.0,
-    ("cfg4", "target"): 1.0,
-    ("cfg4", "draft"): 1.0,
-    ("cfg5", "target"): 1.0,
-    ("cfg5", "draft"): 1.0,
+    ("cfg2", "target"): 1.849763e-01,
+    ("cfg2", "draft"): 1.924046e-01,
+    ("cfg3", "target"): 1.553548e-01,
+    ("cfg4", "target"): 3.928412e-02,
+    ("cfg4", "draft"): 6.446018e-02,
+    ("cfg5", "target"): 1.926644e-02,
+    ("cfg5", "draft"): 4.538489e-01,
 }
 
 

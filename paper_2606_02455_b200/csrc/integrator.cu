@@ -1,0 +1,247 @@
+// ABOBA half-steps, counter-based Philox noise, and the reflection-coupling transport map.
+// PAPER.md:60-66 (Eq. 2), :101-111 (Eq. 7, 8), :421-425 (Alg. 1), :584-604 (DRAFT_STEP / VERIFY_STEP).
+// State is fp64, component-major [3][n].
+#include "lsd_internal.h"
+
+namespace {
+
+constexpr double kTwoPowM32 = 1.0 / 4294967296.0;
+
+// Philox4x32-10 (Salmon et al., SC'11).  Counter = (step lo, step hi, atom, tag), key = seed (R5).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// three standard normals per (step, atom): Box-Muller in fp64 on (w + 1/2) 2^-32 (R5)
+__device__ __forceinline__ void normals3(uint64_t seed, uint64_t step, uint32_t atom, uint32_t tag, double xi[3])
+{
+    uint32_t w[4];
+    philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), atom, tag, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+    const double u0 = ((double)w[0] + 0.5) * kTwoPowM32, u1 = ((double)w[1] + 0.5) * kTwoPowM32;
+    const double u2 = ((double)w[2] + 0.5) * kTwoPowM32, u3 = ((double)w[3] + 0.5) * kTwoPowM32;
+    const double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+    double s, c;
+    sincospi(2.0 * u1, &s, &c);
+    xi[0] = r0 * c; xi[1] = r0 * s;
+    xi[2] = r1 * cospi(2.0 * u3);
+}
+
+__device__ __forceinline__ double uniform53(uint64_t seed, uint64_t step)
+{
+    uint32_t w[4];
+    philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), 0xFFFFFFFFu, 1u, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+    return ((double)(w[0] >> 5) * 67108864.0 + (double)(w[1] >> 6) + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+// A(1/2): q_half = q + (dt/2) p / m  (Eq. 2 first line; map f of Thm 3.1).  Also checks the Verlet skin.
+__global__ void k_half_a(int n, const double* __restrict__ q, const double* __restrict__ p, const double* __restrict__ mass,
+                         double hdt, double* __restrict__ qhalf, const double* __restrict__ qref, double skin_half2, int* flags)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double m = mass[i];
+    double d2 = 0.0;
+    bool bad = false;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double v = q[c * n + i] + hdt * p[c * n + i] / m;
+        qhalf[c * n + i] = v;
+        if (qref) { const double d = v - qref[c * n + i]; d2 += d * d; }
+        bad |= !isfinite(v);
+    }
+    if (qref && d2 > skin_half2) atomicOr(flags, LSD_FLAG_SKIN);
+    if (bad) atomicOr(flags, LSD_FLAG_NONFINITE);
+}
+
+// B O B (= Eq. 7 Gaussian draw) followed by A(1/2):  p' = c1 p + b F + sigma xi;  q' = q_half + (dt/2) p'/m
+__global__ void k_bob_a(int n, uint64_t seed, uint64_t step, const double* __restrict__ p_prev, const double* __restrict__ Ft,
+                        const double* __restrict__ qhalf, const double* __restrict__ mass, const double* __restrict__ sigma,
+                        double c1, double b, double hdt, double* __restrict__ q_new, double* __restrict__ p_new)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double xi[3];
+    normals3(seed, step, (uint32_t)i, 0u, xi);
+    const double m = mass[i], sg = sigma[i];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double pn = c1 * p_prev[c * n + i] + b * Ft[c * n + i] + sg * xi[c];
+        p_new[c * n + i] = pn;
+        q_new[c * n + i] = qhalf[c * n + i] + hdt * pn / m;
+    }
+}
+
+__global__ void k_initial_momenta(int n, uint64_t seed, const double* __restrict__ mass, double kT, double* __restrict__ p)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double xi[3];
+    normals3(seed, 0, (uint32_t)i, 2u, xi);
+    const double s = sqrt(mass[i] * kT);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[c * n + i] = s * xi[c];
+}
+
+// ---- transport, stage 1: per-block partial sums of S1 = xi.d and S2 = d.d, d = (b/sigma)(F~ - F)  (Eq. 8; R6, R13).
+// grid (nblk, K).  Fixed-order reduction: thread-serial over a strided slice, xor-shuffle tree in the warp,
+// warps summed in index order by thread 0.  fp64 throughout.
+constexpr int kTrThreads = 256;
+
+__global__ void __launch_bounds__(kTrThreads)
+k_transport_partial(int n, uint64_t seed, uint64_t n0, const double* __restrict__ Ft, const double* __restrict__ Fg,
+                    const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg)
+{
+    const int j = blockIdx.y;                      // step j+1 of the window
+    const size_t base = (size_t)j * 3 * n;
+    double s1 = 0.0, s2 = 0.0;
+    for (int i = blockIdx.x * kTrThreads + threadIdx.x; i < n; i += gridDim.x * kTrThreads) {
+        double xi[3];
+        normals3(seed, n0 + (uint64_t)j + 1, (uint32_t)i, 0u, xi);
+        const double bs = b / sigma[i];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double d = bs * (Ft[base + (size_t)c * n + i] - Fg[base + (size_t)c * n + i]);
+            s1 += xi[c] * d;
+            s2 += d * d;
+            if (xi_dbg) xi_dbg[base + (size_t)c * n + i] = xi[c];
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    __shared__ double sh1[kTrThreads / 32], sh2[kTrThreads / 32];
+    if ((threadIdx.x & 31) == 0) { sh1[threadIdx.x >> 5] = s1; sh2[threadIdx.x >> 5] = s2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, c = 0.0;
+        for (int w = 0; w < kTrThreads / 32; ++w) { a += sh1[w]; c += sh2[w]; }
+        partial[((size_t)j * gridDim.x + blockIdx.x) * 2 + 0] = a;
+        partial[((size_t)j * gridDim.x + blockIdx.x) * 2 + 1] = c;
+    }
+}
+
+// ---- stage 2: ell_j = -S1 - S2/2, u_j, accept iff S2 == 0 or ln u <= min(0, ell) (R7, R8); first-reject scan (:424).
+__global__ void k_transport_final(int K, int nblk, uint64_t seed, uint64_t n0, const double* __restrict__ partial,
+                                  double* S1, double* S2, double* ell, double* lnu, int* reject, const int* flags,
+                                  TransportResult* result)
+{
+    __shared__ int rej[LSD_MAX_K];
+    __shared__ double beta[LSD_MAX_K];
+    const int j = threadIdx.x;
+    if (j < K) {
+        double a = 0.0, c = 0.0;
+        for (int blk = 0; blk < nblk; ++blk) { a += partial[((size_t)j * nblk + blk) * 2]; c += partial[((size_t)j * nblk + blk) * 2 + 1]; }
+        const double l = -a - 0.5 * c;
+        const double lu = log(uniform53(seed, n0 + (uint64_t)j + 1));
+        const int r = (c > 0.0 && lu > fmin(0.0, l)) ? 1 : 0;
+        S1[j] = a; S2[j] = c; ell[j] = l; lnu[j] = lu; reject[j] = r;
+        rej[j] = r;
+        beta[j] = erf(sqrt(c) / sqrt(8.0));           // Eq. 9
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int l = 0;
+        for (int t = 0; t < K; ++t) if (rej[t]) { l = t + 1; break; }   // l = min{j : x_j != y_j}
+        const int nc = l ? l : K;                                      // R3 (no bonus step), R4 (x_l counts)
+        double bs = 0.0;
+        for (int t = 0; t < nc; ++t) bs += beta[t];
+        result->first_reject = l; result->n_commit = nc; result->flags = *flags; result->beta_sum = bs;
+    }
+}
+
+// ---- stage 3: override of the first rejected step and map g (Eq. 8 else-branch; :602), or commit of y_K.
+__global__ void k_commit(int n, int K, uint64_t seed, uint64_t n0, const TransportResult* __restrict__ result,
+                         const double* __restrict__ S1, const double* __restrict__ S2, const double* __restrict__ Ft,
+                         const double* __restrict__ Fg, const double* __restrict__ qhalf, const double* __restrict__ pstart,
+                         double* __restrict__ yq, double* __restrict__ yp, const double* __restrict__ mass,
+                         const double* __restrict__ sigma, double c1, double b, double hdt, double* __restrict__ q_base,
+                         double* __restrict__ p_base)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (result->flags != 0) return;                  // skin / overflow / non-finite: nothing is committed
+    const int l = result->first_reject;
+    if (l == 0) {
+        const size_t base = (size_t)(K - 1) * 3 * n;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { q_base[c * n + i] = yq[base + (size_t)c * n + i]; p_base[c * n + i] = yp[base + (size_t)c * n + i]; }
+        return;
+    }
+    const size_t base = (size_t)(l - 1) * 3 * n;
+    const double* pprev = (l == 1) ? pstart : yp + (size_t)(l - 2) * 3 * n;
+    double xi[3];
+    normals3(seed, n0 + (uint64_t)l, (uint32_t)i, 0u, xi);
+    const double sg = sigma[i], m = mass[i], ratio = S1[l - 1] / S2[l - 1];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double F = Fg[base + (size_t)c * n + i];
+        const double d = b / sg * (Ft[base + (size_t)c * n + i] - F);
+        const double ps = c1 * pprev[c * n + i] + b * F + sg * (xi[c] - 2.0 * ratio * d);
+        const double qs = qhalf[base + (size_t)c * n + i] + hdt * ps / m;
+        p_base[c * n + i] = ps; q_base[c * n + i] = qs;
+        yp[base + (size_t)c * n + i] = ps; yq[base + (size_t)c * n + i] = qs;     // x_l replaces y_l in the committed window
+    }
+}
+
+}  // namespace
+
+int transport_blocks(int n)
+{
+    int nb = (n + kTrThreads * 4 - 1) / (kTrThreads * 4);
+    if (nb < 1) nb = 1;
+    if (nb > 148) nb = 148;
+    return nb;
+}
+
+void launch_half_a(Launcher L, int n, const double* q, const double* p, const double* mass, double hdt,
+                   double* qhalf, const double* qref, double skin_half2, int* flags)
+{
+    k_half_a<<<(n + 255) / 256, 256, 0, L.s>>>(n, q, p, mass, hdt, qhalf, qref, skin_half2, flags);
+    LSD_COUNT(L);
+}
+
+void launch_bob_a(Launcher L, int n, uint64_t seed, uint64_t step, const double* p_prev, const double* Ft,
+                  const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
+                  double* q_new, double* p_new)
+{
+    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, step, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new);
+    LSD_COUNT(L);
+}
+
+void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p)
+{
+    k_initial_momenta<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, mass, kT, p);
+    LSD_COUNT(L);
+}
+
+void launch_transport(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const double* Ft, const double* Fg,
+                      const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg)
+{
+    k_transport_partial<<<dim3(nblk, K), kTrThreads, 0, L.s>>>(n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg);
+    LSD_COUNT(L);
+    k_transport_final<<<1, LSD_MAX_K, 0, L.s>>>(K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
+    LSD_COUNT(L);
+}
+
+void launch_commit(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const TransportResult* result,
+                   const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
+                   const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
+                   double c1, double b, double hdt, double* q_base, double* p_base)
+{
+    k_commit<<<(n + 127) / 128, 128, 0, L.s>>>(n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
+                                               c1, b, hdt, q_base, p_base);
+    LSD_COUNT(L);
+}

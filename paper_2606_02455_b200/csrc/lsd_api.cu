@@ -1,0 +1,680 @@
+// C ABI of liblsd_b200.so (include/lsd.h): context, window slots, call sequencing.  No torch types, no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "lsd_internal.h"
+
+namespace {
+
+thread_local std::string g_init_error;
+
+struct WindowSlot {
+    int K = 0;
+    int drafted = 0, verified = 0;
+    uint64_t n0 = 0;
+    double *qstart = nullptr, *pstart = nullptr;             // [3][n]
+    double *qhalf = nullptr, *Ft = nullptr, *yq = nullptr, *yp = nullptr;   // [kmax][3][n]
+    int* img = nullptr;                                      // [n] images of the reference (start) state
+    VerletList vl_mlip, vl_pair;
+    int* flags = nullptr;
+    cudaEvent_t ev_drafted = nullptr;
+};
+
+}  // namespace
+
+struct lsd_ctx {
+    lsd_config cfg{};
+    SysDev sys;
+    PotDev pot[2];
+    std::vector<void*> allocs;
+    double c1 = 0, b = 0, hdt = 0, kT = 0;
+    double *q = nullptr, *p = nullptr;
+    int64_t step = 0;
+    WindowSlot slot[2];
+    int verify_idx = 0, pending = 0, last_slot = -1, last_K = 0, last_l = 0, last_nc = 0, transported = 0;
+    MlipWork work[2];
+    CompactList cl_mlip[2], cl_pair[2];
+    const int* cl_img[2] = {nullptr, nullptr};
+    int bmax[2] = {1, 1};
+    CellGrid grid;
+    double rc_mlip_max = 0, rc_pair_max = 0;
+    int cap_mlip = 0, cap_pair = 0;
+    double* Fg = nullptr;
+    double *partial = nullptr, *S1 = nullptr, *S2 = nullptr, *ell = nullptr, *lnu = nullptr, *xi_dbg = nullptr;
+    int* reject = nullptr;
+    int nblk = 1;
+    TransportResult* result = nullptr;
+    TransportResult* result_host = nullptr;
+    // lsd_eval_forces scratch
+    double *q_eval = nullptr, *F_eval = nullptr, *e_eval = nullptr;
+    int* img_eval = nullptr; int* flags_eval = nullptr;
+    VerletList vl_eval_mlip, vl_eval_pair;
+    cudaStream_t side = nullptr;
+    int64_t launches = 0;
+    lsd_stats stats{};
+    std::string err;
+};
+
+namespace {
+
+#define CK(expr)                                                                                             \
+    do {                                                                                                     \
+        cudaError_t e__ = (expr);                                                                            \
+        if (e__ != cudaSuccess) {                                                                            \
+            char buf__[512];                                                                                 \
+            snprintf(buf__, sizeof buf__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            ctx->err = buf__;                                                                                \
+            return e__ == cudaErrorMemoryAllocation ? LSD_ERR_OOM : LSD_ERR_CUDA;                            \
+        }                                                                                                    \
+    } while (0)
+
+lsd_status fail(lsd_ctx* ctx, lsd_status s, const char* msg) { if (ctx) ctx->err = msg; else g_init_error = msg; return s; }
+
+template <typename T> lsd_status dalloc(lsd_ctx* ctx, T** p, size_t count)
+{
+    void* v = nullptr;
+    CK(cudaMalloc(&v, std::max<size_t>(count, 1) * sizeof(T)));
+    ctx->allocs.push_back(v);
+    *p = (T*)v;
+    return LSD_OK;
+}
+template <typename T> lsd_status upload(lsd_ctx* ctx, T** p, const T* host, size_t count)
+{
+    lsd_status s = dalloc(ctx, p, count);
+    if (s) return s;
+    if (count) CK(cudaMemcpy(*p, host, count * sizeof(T), cudaMemcpyHostToDevice));
+    return LSD_OK;
+}
+#define TRY(expr) do { lsd_status s__ = (expr); if (s__ != LSD_OK) return s__; } while (0)
+
+Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, &ctx->launches}; }
+
+lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
+{
+    d.F = m.width; d.T = m.n_blocks; d.R = m.n_rbf; d.ns = m.n_species; d.rc = (float)m.cutoff; d.alpha = (float)m.energy_scale;
+    const int F = d.F, R = d.R, T = d.T;
+    const double* w = m.weights;
+    std::vector<float> buf;
+    auto up = [&](const double* src, int rows, int cols, bool transpose, float** out) -> lsd_status {
+        buf.resize((size_t)rows * cols);
+        if (!transpose) for (size_t i = 0; i < buf.size(); ++i) buf[i] = (float)src[i];
+        else for (int r = 0; r < rows; ++r) for (int c = 0; c < cols; ++c) buf[(size_t)c * rows + r] = (float)src[(size_t)r * cols + c];
+        return upload(ctx, out, buf.data(), buf.size());
+    };
+    TRY(up(w, m.n_species, F, false, &d.emb));
+    const double* blk = w + (size_t)m.n_species * F;
+    const size_t per_block = (size_t)4 * F * F + (size_t)F * R;
+    d.WinT.resize(T); d.Win.resize(T); d.Wf1T.resize(T); d.Wf2T.resize(T); d.Wo1T.resize(T); d.Wo1.resize(T); d.Wo2T.resize(T); d.Wo2.resize(T);
+    for (int t = 0; t < T; ++t) {
+        const double* Win = blk + t * per_block; const double* Wf1 = Win + (size_t)F * F; const double* Wf2 = Wf1 + (size_t)F * R;
+        const double* Wo1 = Wf2 + (size_t)F * F; const double* Wo2 = Wo1 + (size_t)F * F;
+        TRY(up(Win, F, F, true, &d.WinT[t])); TRY(up(Win, F, F, false, &d.Win[t]));
+        TRY(up(Wf1, F, R, true, &d.Wf1T[t])); TRY(up(Wf2, F, F, true, &d.Wf2T[t]));
+        TRY(up(Wo1, F, F, true, &d.Wo1T[t])); TRY(up(Wo1, F, F, false, &d.Wo1[t]));
+        TRY(up(Wo2, F, F, true, &d.Wo2T[t])); TRY(up(Wo2, F, F, false, &d.Wo2[t]));
+    }
+    const double* Wr1 = blk + (size_t)T * per_block;
+    TRY(up(Wr1, F / 2, F, false, &d.Wr1));
+    TRY(up(Wr1 + (size_t)(F / 2) * F, 1, F / 2, false, &d.wr2));
+    return LSD_OK;
+}
+
+lsd_status upload_potential(lsd_ctx* ctx, const lsd_potential& p, PotDev& d)
+{
+    d.ns = p.n_species; d.use_bonded = p.use_bonded;
+    const int ns = p.n_species;
+    TRY(upload(ctx, &d.pair, p.pair, (size_t)ns * ns * LSD_PAIR_COLS));
+    std::vector<double> rc2((size_t)ns * ns, 0.0), tether(ns, 0.0);
+    d.pair_rcmax = 0.0; d.has_tether = 0;
+    for (int a = 0; a < ns * ns; ++a) {
+        const double* pp = p.pair + (size_t)a * LSD_PAIR_COLS;
+        double rc = 0.0;
+        if (pp[0] != 0.0) rc = std::max(rc, pp[2]);
+        if (pp[3] != 0.0) rc = std::max(rc, pp[6]);
+        rc2[a] = rc * rc;
+        d.pair_rcmax = std::max(d.pair_rcmax, rc);
+    }
+    for (int s = 0; s < ns; ++s) { tether[s] = p.pair[((size_t)s * ns + s) * LSD_PAIR_COLS + 7]; if (tether[s] != 0.0) d.has_tether = 1; }
+    TRY(upload(ctx, &d.pair_rc2, rc2.data(), rc2.size()));
+    TRY(upload(ctx, &d.tether, tether.data(), tether.size()));
+    if (p.mlip.width > 0) TRY(upload_mlip(ctx, p.mlip, d.mlip));
+    return LSD_OK;
+}
+
+lsd_status alloc_verlet(lsd_ctx* ctx, VerletList& vl, int cap, double rc)
+{
+    vl.cap = cap; vl.rc = rc;
+    TRY(dalloc(ctx, &vl.count, ctx->sys.n));
+    TRY(dalloc(ctx, &vl.keys, (size_t)ctx->sys.n * cap));
+    return LSD_OK;
+}
+lsd_status alloc_compact(lsd_ctx* ctx, CompactList& cl, int cap, int bmax)
+{
+    cl.cap = cap; cl.bmax = bmax;
+    TRY(dalloc(ctx, &cl.count, (size_t)ctx->sys.n * bmax));
+    TRY(dalloc(ctx, &cl.keys, (size_t)ctx->sys.n * bmax * cap));
+    return LSD_OK;
+}
+lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
+{
+    const size_t rows = (size_t)ctx->sys.n * bmax, e = rows * net.F;
+    w.bmax = bmax;
+    TRY(dalloc(ctx, &w.x, e)); TRY(dalloc(ctx, &w.m, e)); TRY(dalloc(ctx, &w.mbar, e)); TRY(dalloc(ctx, &w.xbar, e)); TRY(dalloc(ctx, &w.ybar, e));
+    w.y.resize(net.T); w.h.resize(net.T);
+    for (int t = 0; t < net.T; ++t) { TRY(dalloc(ctx, &w.y[t], e)); TRY(dalloc(ctx, &w.h[t], e)); }
+    TRY(dalloc(ctx, &w.e_atom, rows));
+    return LSD_OK;
+}
+
+// Probe the neighbour-row capacity on the current base state (synchronises).
+lsd_status probe_capacity(lsd_ctx* ctx, double rc_skin, int* cap_out)
+{
+    const int n = ctx->sys.n;
+    VerletList tmp; tmp.cap = 512; tmp.rc = rc_skin;
+    int *count = nullptr, *img = nullptr, *flags = nullptr; uint32_t* keys = nullptr;
+    CK(cudaMalloc(&count, sizeof(int) * n)); CK(cudaMalloc(&keys, sizeof(uint32_t) * (size_t)n * tmp.cap));
+    CK(cudaMalloc(&img, sizeof(int) * n)); CK(cudaMalloc(&flags, sizeof(int)));
+    CK(cudaMemset(flags, 0, sizeof(int)));
+    tmp.count = count; tmp.keys = keys;
+    Launcher L = mk(ctx, nullptr);
+    cellgrid_setup(ctx->grid, ctx->sys, rc_skin);
+    launch_pack_ref(L, ctx->sys, ctx->q, img);
+    launch_build_verlet(L, ctx->sys, ctx->grid, ctx->q, img, rc_skin, tmp, flags);
+    CK(cudaDeviceSynchronize());
+    std::vector<int> h(n);
+    CK(cudaMemcpy(h.data(), count, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    int hf = 0; CK(cudaMemcpy(&hf, flags, sizeof(int), cudaMemcpyDeviceToHost));
+    cudaFree(count); cudaFree(keys); cudaFree(img); cudaFree(flags);
+    if (hf & LSD_FLAG_OVERFLOW) return fail(ctx, LSD_ERR_NBR_OVERFLOW, "neighbour row exceeds 512 entries (cutoff + skin too large for this density)");
+    int mx = 0; for (int v : h) mx = std::max(mx, v);
+    int cap = (int)(mx * 1.25) + 8;
+    cap = (cap + 7) / 8 * 8;
+    *cap_out = std::min(cap, 512);
+    return LSD_OK;
+}
+
+lsd_status setup_lists(lsd_ctx* ctx)
+{
+    const double skin = ctx->cfg.skin;
+    ctx->rc_mlip_max = std::max((double)ctx->pot[0].mlip.rc, (double)ctx->pot[1].mlip.rc);
+    ctx->rc_pair_max = std::max(ctx->pot[0].pair_rcmax, ctx->pot[1].pair_rcmax);
+    const double rmax = std::max(ctx->rc_mlip_max, ctx->rc_pair_max) + skin;
+    if (ctx->sys.periodic) for (int c = 0; c < 3; ++c)
+        if (ctx->sys.box[c] < 2.0 * rmax) return fail(ctx, LSD_ERR_INVALID_ARG, "periodic box must be >= 2 (r_c + skin) in every dimension (single minimum image, R10)");
+    ctx->cap_mlip = ctx->cap_pair = 0;
+    if (ctx->rc_mlip_max > 0) TRY(probe_capacity(ctx, ctx->rc_mlip_max + skin, &ctx->cap_mlip));
+    if (ctx->rc_pair_max > 0) TRY(probe_capacity(ctx, ctx->rc_pair_max + skin, &ctx->cap_pair));
+    for (int s = 0; s < 2; ++s) {
+        if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->slot[s].vl_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
+        if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->slot[s].vl_pair, ctx->cap_pair, ctx->rc_pair_max));
+    }
+    if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->vl_eval_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
+    if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->vl_eval_pair, ctx->cap_pair, ctx->rc_pair_max));
+    for (int w = 0; w < 2; ++w) {
+        if (ctx->pot[w].mlip.F > 0) TRY(alloc_compact(ctx, ctx->cl_mlip[w], ctx->cap_mlip, ctx->bmax[w]));
+        if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w]));
+    }
+    return LSD_OK;
+}
+
+// Window-shared lists from the reference state qref (a1).
+void build_lists(lsd_ctx* ctx, Launcher L, const double* qref, int* img, VerletList& vm, VerletList& vp, int* flags)
+{
+    launch_pack_ref(L, ctx->sys, qref, img);
+    if (ctx->cap_mlip) {
+        cellgrid_setup(ctx->grid, ctx->sys, ctx->rc_mlip_max + ctx->cfg.skin);
+        launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_mlip_max + ctx->cfg.skin, vm, flags);
+    }
+    if (ctx->cap_pair) {
+        cellgrid_setup(ctx->grid, ctx->sys, ctx->rc_pair_max + ctx->cfg.skin);
+        launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_pair_max + ctx->cfg.skin, vp, flags);
+    }
+}
+
+// One batched force evaluation of potential `which` on B <= bmax[which] states (a0 / a2).
+void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, const int* img, const VerletList& vm,
+                 const VerletList& vp, double* F, int* flags, double* e_atom)
+{
+    PotDev& pot = ctx->pot[which];
+    ctx->cl_img[which] = img;
+    CompactList* pl = nullptr;
+    if (pot.pair_rcmax > 0) {
+        launch_compact(L, ctx->sys, B, q, img, vp, 0.0, pot.pair_rc2, ctx->cl_pair[which], flags);
+        pl = &ctx->cl_pair[which];
+    }
+    launch_prior_forces(L, ctx->sys, pot, B, q, img, pl, F);
+    if (pot.mlip.F > 0) {
+        const double rc = (double)pot.mlip.rc;
+        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags);
+        if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(pot.mlip))
+            mlip_forward_backward_bf16tc(L, ctx->sys, pot.mlip, ctx->work[which], B, q, img, ctx->cl_mlip[which], F, e_atom);
+        else
+            mlip_forward_backward_fp32(L, ctx->sys, pot.mlip, ctx->work[which], B, q, img, ctx->cl_mlip[which], F, e_atom);
+    }
+}
+
+lsd_status flags_to_status(lsd_ctx* ctx, int flags)
+{
+    if (flags & LSD_FLAG_NONFINITE) return fail(ctx, LSD_ERR_NONFINITE, "non-finite positions in the window");
+    if (flags & LSD_FLAG_OVERFLOW) return fail(ctx, LSD_ERR_NBR_OVERFLOW, "neighbour row capacity exceeded (call lsd_set_skin to re-size the lists)");
+    if (flags & LSD_FLAG_SKIN) return fail(ctx, LSD_ERR_SKIN_VIOLATED, "an atom moved more than skin/2 from the list's reference state");
+    return LSD_OK;
+}
+
+lsd_status copy_out(lsd_ctx* ctx, void* dst, const void* src_dev, size_t bytes, int where)
+{
+    CK(cudaMemcpy(dst, src_dev, bytes, where == LSD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice));
+    return LSD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lsd_version(void) { return "lsd-b200 0.1 (sm_100a)"; }
+
+const char* lsd_last_error(const lsd_ctx* ctx) { return ctx ? ctx->err.c_str() : g_init_error.c_str(); }
+
+int64_t lsd_launch_count(const lsd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+void lsd_destroy(lsd_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaDeviceSynchronize();
+    for (void* p : ctx->allocs) cudaFree(p);
+    cudaFree(ctx->grid.cell_count); cudaFree(ctx->grid.cell_start); cudaFree(ctx->grid.cell_cursor);
+    cudaFree(ctx->grid.cell_atoms); cudaFree(ctx->grid.atom_cell);
+    for (int s = 0; s < 2; ++s) if (ctx->slot[s].ev_drafted) cudaEventDestroy(ctx->slot[s].ev_drafted);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    if (ctx->result_host) cudaFreeHost(ctx->result_host);
+    delete ctx;
+}
+
+static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_system* sys, const lsd_potential* draft,
+                            const lsd_potential* target, const double* q0, const double* p0)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(ctx, LSD_ERR_CUDA, "no CUDA device: liblsd_b200 has no CPU fallback");
+    ctx->cfg = *cfg;
+    const int n = sys->n_atoms, kmax = cfg->k_max;
+    if (n < 1 || sys->n_species < 1 || !q0) return fail(ctx, LSD_ERR_INVALID_ARG, "n_atoms, n_species must be >= 1 and q0 non-null");
+    if (kmax < 1 || kmax > LSD_MAX_K) return fail(ctx, LSD_ERR_INVALID_ARG, "k_max must be in 1..64");
+    if (cfg->scheme != LSD_SCHEME_ABOBA) return fail(ctx, LSD_ERR_UNSUPPORTED, "only LSD_SCHEME_ABOBA is implemented (DESIGN.md R1)");
+    if (cfg->precision != LSD_FP32 && cfg->precision != LSD_BF16_TC) return fail(ctx, LSD_ERR_INVALID_ARG, "precision must be LSD_FP32 or LSD_BF16_TC");
+    if (!(cfg->dt_fs > 0) || !(cfg->friction_per_fs > 0) || !(cfg->temperature_K > 0) || !(cfg->skin > 0)) return fail(ctx, LSD_ERR_INVALID_ARG, "dt, friction, temperature and skin must be positive");
+    for (const lsd_potential* p : {draft, target}) {
+        if (p->n_species != sys->n_species) return fail(ctx, LSD_ERR_INVALID_ARG, "potential and system disagree on n_species");
+        const int F = p->mlip.width;
+        if (F != 0) {
+            if (F != 32 && F != 64 && F != 128) return fail(ctx, LSD_ERR_UNSUPPORTED, "MLIP width must be 32, 64 or 128");
+            if (p->mlip.n_rbf != LSD_NRBF) return fail(ctx, LSD_ERR_UNSUPPORTED, "MLIP n_rbf must be 32");
+            if (p->mlip.n_blocks < 1 || p->mlip.n_species != sys->n_species || !(p->mlip.cutoff > 0) || !p->mlip.weights) return fail(ctx, LSD_ERR_INVALID_ARG, "bad MLIP description");
+        }
+    }
+    for (int i = 0; i < n; ++i) if (sys->species[i] < 0 || sys->species[i] >= sys->n_species) return fail(ctx, LSD_ERR_INVALID_ARG, "species index out of range");
+
+    SysDev& S = ctx->sys;
+    S.n = n; S.ns = sys->n_species; S.periodic = sys->periodic;
+    for (int c = 0; c < 3; ++c) S.box[c] = sys->box[c];
+    ctx->kT = LSD_KB_EV * cfg->temperature_K;
+    ctx->c1 = std::exp(-cfg->friction_per_fs * cfg->dt_fs);
+    ctx->b = (1.0 + ctx->c1) * cfg->dt_fs / 2.0;
+    ctx->hdt = cfg->dt_fs / 2.0;
+    std::vector<double> mass(n), sigma(n);
+    for (int i = 0; i < n; ++i) {
+        mass[i] = sys->mass_amu[i] * LSD_AMU_EV;
+        sigma[i] = std::sqrt(sys->mass_amu[i] * LSD_AMU_EV * LSD_KB_EV * cfg->temperature_K * (1.0 - ctx->c1 * ctx->c1));   // Eq. 7 covariance
+    }
+    TRY(upload(ctx, &S.species, sys->species, n));
+    TRY(upload(ctx, &S.mass, mass.data(), n));
+    TRY(upload(ctx, &S.sigma, sigma.data(), n));
+    S.n_bonds = sys->n_bonds; S.n_angles = sys->n_angles;
+    if (S.n_bonds) { TRY(upload(ctx, &S.bonds, sys->bonds, (size_t)2 * S.n_bonds)); TRY(upload(ctx, &S.bond_k, sys->bond_k, S.n_bonds)); TRY(upload(ctx, &S.bond_r0, sys->bond_r0, S.n_bonds)); }
+    if (S.n_angles) { TRY(upload(ctx, &S.angles, sys->angles, (size_t)3 * S.n_angles)); TRY(upload(ctx, &S.angle_k, sys->angle_k, S.n_angles)); TRY(upload(ctx, &S.angle_t0, sys->angle_theta0, S.n_angles)); }
+    {   // per-atom bonded-term lists (gather form; bonds first, then angles, in input order)
+        std::vector<std::vector<int>> per(n);
+        for (int t = 0; t < S.n_bonds; ++t) for (int k = 0; k < 2; ++k) {
+            const int a = sys->bonds[2 * t + k];
+            if (a < 0 || a >= n) return fail(ctx, LSD_ERR_INVALID_ARG, "bond atom index out of range");
+            per[a].push_back(t);
+        }
+        for (int t = 0; t < S.n_angles; ++t) for (int k = 0; k < 3; ++k) {
+            const int a = sys->angles[3 * t + k];
+            if (a < 0 || a >= n) return fail(ctx, LSD_ERR_INVALID_ARG, "angle atom index out of range");
+            per[a].push_back(S.n_bonds + t);
+        }
+        std::vector<int> start(n + 1, 0), term;
+        for (int i = 0; i < n; ++i) { start[i + 1] = start[i] + (int)per[i].size(); term.insert(term.end(), per[i].begin(), per[i].end()); }
+        TRY(upload(ctx, &S.bt_start, start.data(), start.size()));
+        TRY(upload(ctx, &S.bt_term, term.data(), term.size()));
+    }
+    TRY(upload_potential(ctx, *draft, ctx->pot[LSD_DRAFT]));
+    TRY(upload_potential(ctx, *target, ctx->pot[LSD_TARGET]));
+    ctx->bmax[LSD_DRAFT] = 1; ctx->bmax[LSD_TARGET] = kmax;
+
+    const size_t n3 = (size_t)3 * n;
+    TRY(upload(ctx, &ctx->q, q0, n3));
+    TRY(dalloc(ctx, &ctx->p, n3));
+    if (p0) CK(cudaMemcpy(ctx->p, p0, n3 * sizeof(double), cudaMemcpyHostToDevice));
+    else launch_initial_momenta(mk(ctx, nullptr), n, cfg->seed, S.mass, ctx->kT, ctx->p);
+    TRY(setup_lists(ctx));
+    for (int s = 0; s < 2; ++s) {
+        WindowSlot& w = ctx->slot[s];
+        TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
+        TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
+        TRY(dalloc(ctx, &w.img, n)); TRY(dalloc(ctx, &w.flags, 1));
+        CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
+    }
+    for (int w = 0; w < 2; ++w) if (ctx->pot[w].mlip.F > 0) TRY(alloc_work(ctx, ctx->pot[w].mlip, ctx->work[w], ctx->bmax[w]));
+    TRY(dalloc(ctx, &ctx->Fg, n3 * kmax));
+    ctx->nblk = transport_blocks(n);
+    TRY(dalloc(ctx, &ctx->partial, (size_t)2 * ctx->nblk * kmax));
+    TRY(dalloc(ctx, &ctx->S1, kmax)); TRY(dalloc(ctx, &ctx->S2, kmax)); TRY(dalloc(ctx, &ctx->ell, kmax)); TRY(dalloc(ctx, &ctx->lnu, kmax));
+    TRY(dalloc(ctx, &ctx->reject, kmax)); TRY(dalloc(ctx, &ctx->result, 1));
+    TRY(dalloc(ctx, &ctx->q_eval, n3 * kmax)); TRY(dalloc(ctx, &ctx->F_eval, n3 * kmax)); TRY(dalloc(ctx, &ctx->e_eval, (size_t)n * kmax));
+    TRY(dalloc(ctx, &ctx->img_eval, n)); TRY(dalloc(ctx, &ctx->flags_eval, 1));
+    CK(cudaMallocHost(&ctx->result_host, sizeof(TransportResult)));
+    CK(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+    CK(cudaDeviceSynchronize());
+    CK(cudaGetLastError());
+    return LSD_OK;
+}
+
+lsd_status lsd_init(const lsd_config* cfg, const lsd_system* sys, const lsd_potential* draft, const lsd_potential* target,
+                    const double* q0, const double* p0, lsd_ctx** out)
+{
+    if (!cfg || !sys || !draft || !target || !out) return fail(nullptr, LSD_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    lsd_ctx* ctx = new (std::nothrow) lsd_ctx();
+    if (!ctx) return fail(nullptr, LSD_ERR_OOM, "host allocation failed");
+    lsd_status s = init_impl(ctx, cfg, sys, draft, target, q0, p0);
+    if (s != LSD_OK) { g_init_error = ctx->err; lsd_destroy(ctx); return s; }
+    *out = ctx;
+    return LSD_OK;
+}
+
+lsd_status lsd_set_skin(lsd_ctx* ctx, double skin)
+{
+    if (!ctx || !(skin > 0)) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    ctx->cfg.skin = skin;
+    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
+    return setup_lists(ctx);      // old rows stay allocated until lsd_destroy
+}
+
+lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    if (K < 1 || K > ctx->cfg.k_max) return fail(ctx, LSD_ERR_INVALID_ARG, "K must be in 1..k_max");
+    if (ctx->pending >= 2) return fail(ctx, LSD_ERR_STATE, "two unverified windows are already drafted");
+    const int n = ctx->sys.n;
+    const size_t n3 = (size_t)3 * n;
+    const int si = (ctx->verify_idx + ctx->pending) & 1;
+    WindowSlot& w = ctx->slot[si];
+    cudaStream_t st = (cudaStream_t)stream;
+    Launcher L = mk(ctx, stream);
+    if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));          // a discarded rollout into this slot may still run
+    if (ctx->pending == 0) {
+        CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(w.pstart, ctx->p, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        w.n0 = (uint64_t)ctx->step;
+    } else {                                                                  // speculative: continue from y_K of the unverified window
+        WindowSlot& pv = ctx->slot[si ^ 1];
+        CK(cudaStreamWaitEvent(st, pv.ev_drafted, 0));
+        CK(cudaMemcpyAsync(w.qstart, pv.yq + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(w.pstart, pv.yp + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        w.n0 = pv.n0 + (uint64_t)pv.K;
+    }
+    CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
+    build_lists(ctx, L, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
+    const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
+    for (int j = 1; j <= K; ++j) {                                            // serial in j
+        const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
+        const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
+        double* qh = w.qhalf + n3 * (j - 1);
+        launch_half_a(L, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
+        eval_forces(ctx, L, LSD_DRAFT, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
+        launch_bob_a(L, n, ctx->cfg.seed, w.n0 + (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
+                     ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1));
+    }
+    CK(cudaEventRecord(w.ev_drafted, st));
+    w.K = K; w.drafted = 1; w.verified = 0;
+    ctx->pending++;
+    CK(cudaGetLastError());
+    return LSD_OK;
+}
+
+lsd_status lsd_verify_window(lsd_ctx* ctx, int32_t K, void* stream)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    WindowSlot& w = ctx->slot[ctx->verify_idx];
+    if (ctx->pending < 1 || !w.drafted) return fail(ctx, LSD_ERR_STATE, "no drafted window to verify");
+    if (K != w.K) return fail(ctx, LSD_ERR_INVALID_ARG, "K differs from the drafted window length");
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
+    eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr);
+    w.verified = 1;
+    CK(cudaGetLastError());
+    return LSD_OK;
+}
+
+lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* first_reject, int32_t* n_commit)
+{
+    if (!ctx || !first_reject || !n_commit) return LSD_ERR_INVALID_ARG;
+    WindowSlot& w = ctx->slot[ctx->verify_idx];
+    if (ctx->pending < 1 || !w.verified) return fail(ctx, LSD_ERR_STATE, "lsd_verify_window has not run on this window");
+    if (K != w.K) return fail(ctx, LSD_ERR_INVALID_ARG, "K differs from the drafted window length");
+    cudaStream_t st = (cudaStream_t)stream;
+    Launcher L = mk(ctx, stream);
+    const int n = ctx->sys.n;
+    launch_transport(L, n, K, ctx->cfg.seed, w.n0, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk, ctx->S1, ctx->S2,
+                     ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
+    launch_commit(L, n, K, ctx->cfg.seed, w.n0, ctx->result, ctx->S1, ctx->S2, w.Ft, ctx->Fg, w.qhalf, w.pstart, w.yq, w.yp,
+                  ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p);
+    CK(cudaMemcpyAsync(ctx->result_host, ctx->result, sizeof(TransportResult), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    const TransportResult r = *ctx->result_host;
+    ctx->last_slot = ctx->verify_idx; ctx->last_K = K;
+    if (r.flags) {                                             // nothing committed: drop every drafted window
+        ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
+        ctx->transported = 0;
+        return flags_to_status(ctx, r.flags);
+    }
+    ctx->last_l = r.first_reject; ctx->last_nc = r.n_commit; ctx->transported = 1;
+    ctx->stats.beta_sum += r.beta_sum;
+    *first_reject = r.first_reject; *n_commit = r.n_commit;
+    return LSD_OK;
+}
+
+lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    if (!ctx->transported) return fail(ctx, LSD_ERR_STATE, "lsd_transport_accept has not run on this window");
+    if (first_reject != ctx->last_l) return fail(ctx, LSD_ERR_INVALID_ARG, "first_reject differs from the value lsd_transport_accept returned");
+    WindowSlot& w = ctx->slot[ctx->verify_idx];
+    ctx->step += ctx->last_nc;
+    ctx->stats.windows++; ctx->stats.committed_steps += ctx->last_nc; ctx->stats.rejections += first_reject ? 1 : 0; ctx->stats.step = ctx->step;
+    w.drafted = 0; w.verified = 0;
+    ctx->verify_idx ^= 1; ctx->pending--;
+    if (first_reject != 0 && ctx->pending > 0) {              // flush the speculative window
+        ctx->slot[ctx->verify_idx].drafted = 0;
+        ctx->pending = 0;
+    }
+    ctx->transported = 0;
+    return LSD_OK;
+}
+
+lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    if (K < 1 || K > ctx->cfg.k_max || n_steps < 0) return fail(ctx, LSD_ERR_INVALID_ARG, "bad K or n_steps");
+    int64_t remaining = n_steps;
+    while (remaining > 0) {
+        if (ctx->pending == 0) TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining), stream));
+        const int k = ctx->slot[ctx->verify_idx].K;
+        TRY(lsd_verify_window(ctx, k, stream));
+        if (overlap && remaining - k > 0 && ctx->pending == 1)
+            TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining - k), ctx->side));   // speculative, second stream
+        int32_t l = 0, nc = 0;
+        TRY(lsd_transport_accept(ctx, k, stream, &l, &nc));
+        TRY(lsd_rollback(ctx, l));
+        remaining -= nc;
+        if (ctx->pending == 1 && ctx->slot[ctx->verify_idx].K > remaining) {   // cannot happen with the K choice above; defensive
+            CK(cudaStreamSynchronize(ctx->side));
+            ctx->pending = 0; ctx->slot[ctx->verify_idx].drafted = 0;
+        }
+    }
+    if (ctx->pending) { CK(cudaStreamSynchronize(ctx->side)); ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; }
+    return LSD_OK;
+}
+
+lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int32_t where)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
+    if (q) TRY(copy_out(ctx, q, ctx->q, bytes, where));
+    if (p) TRY(copy_out(ctx, p, ctx->p, bytes, where));
+    if (step) *step = ctx->step;
+    return LSD_OK;
+}
+
+lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t step, int32_t where)
+{
+    if (!ctx || !q || !p) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
+    const cudaMemcpyKind kind = where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    CK(cudaMemcpy(ctx->q, q, bytes, kind));
+    CK(cudaMemcpy(ctx->p, p, bytes, kind));
+    ctx->step = step; ctx->stats.step = step;
+    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
+    return LSD_OK;
+}
+
+lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out)
+{
+    if (!ctx || !out) return LSD_ERR_INVALID_ARG;
+    *out = ctx->stats; out->step = ctx->step;
+    return LSD_OK;
+}
+
+lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    if (ctx->last_slot < 0) return fail(ctx, LSD_ERR_STATE, "no window has been transported yet");
+    if (j < 1 || j > ctx->last_nc) return fail(ctx, LSD_ERR_INVALID_ARG, "j must be in 1..n_commit");
+    CK(cudaDeviceSynchronize());
+    const WindowSlot& w = ctx->slot[ctx->last_slot];
+    const size_t n3 = (size_t)3 * ctx->sys.n;
+    if (q) TRY(copy_out(ctx, q, w.yq + n3 * (j - 1), n3 * sizeof(double), where));
+    if (p) TRY(copy_out(ctx, p, w.yp + n3 * (j - 1), n3 * sizeof(double), where));
+    return LSD_OK;
+}
+
+lsd_status lsd_get_window_debug(lsd_ctx* ctx, int32_t what, void* out, int32_t where)
+{
+    if (!ctx || !out) return LSD_ERR_INVALID_ARG;
+    if (ctx->last_slot < 0) return fail(ctx, LSD_ERR_STATE, "no window has been transported yet");
+    CK(cudaDeviceSynchronize());
+    const WindowSlot& w = ctx->slot[ctx->last_slot];
+    const int K = ctx->last_K;
+    const size_t big = (size_t)3 * ctx->sys.n * K * sizeof(double), small = (size_t)K * sizeof(double);
+    switch (what) {
+        case LSD_DBG_QHALF:   return copy_out(ctx, out, w.qhalf, big, where);
+        case LSD_DBG_FDRAFT:  return copy_out(ctx, out, w.Ft, big, where);
+        case LSD_DBG_FTARGET: return copy_out(ctx, out, ctx->Fg, big, where);
+        case LSD_DBG_YP:      return copy_out(ctx, out, w.yp, big, where);
+        case LSD_DBG_YQ:      return copy_out(ctx, out, w.yq, big, where);
+        case LSD_DBG_S1:      return copy_out(ctx, out, ctx->S1, small, where);
+        case LSD_DBG_S2:      return copy_out(ctx, out, ctx->S2, small, where);
+        case LSD_DBG_ELL:     return copy_out(ctx, out, ctx->ell, small, where);
+        case LSD_DBG_LNU:     return copy_out(ctx, out, ctx->lnu, small, where);
+        case LSD_DBG_REJECT:  return copy_out(ctx, out, ctx->reject, (size_t)K * sizeof(int), where);
+        case LSD_DBG_XI: {
+            if (!ctx->xi_dbg) TRY(dalloc(ctx, &ctx->xi_dbg, (size_t)3 * ctx->sys.n * ctx->cfg.k_max));
+            launch_transport(mk(ctx, nullptr), ctx->sys.n, K, ctx->cfg.seed, w.n0, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk,
+                             ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
+            CK(cudaDeviceSynchronize());
+            return copy_out(ctx, out, ctx->xi_dbg, big, where);
+        }
+        default: return fail(ctx, LSD_ERR_INVALID_ARG, "unknown debug row");
+    }
+}
+
+lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const double* q, double* F, double* energy_nn,
+                           int32_t where, void* stream)
+{
+    if (!ctx || !q || !F || (which != LSD_DRAFT && which != LSD_TARGET)) return LSD_ERR_INVALID_ARG;
+    if (n_states < 1 || n_states > ctx->cfg.k_max) return fail(ctx, LSD_ERR_INVALID_ARG, "n_states must be in 1..k_max");
+    cudaStream_t st = (cudaStream_t)stream;
+    Launcher L = mk(ctx, stream);
+    const int n = ctx->sys.n;
+    const size_t n3 = (size_t)3 * n;
+    const cudaMemcpyKind in_kind = where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    const cudaMemcpyKind out_kind = where == LSD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    CK(cudaMemcpyAsync(ctx->q_eval, q, n3 * n_states * sizeof(double), in_kind, st));
+    CK(cudaMemsetAsync(ctx->flags_eval, 0, sizeof(int), st));
+    build_lists(ctx, L, ctx->q_eval, ctx->img_eval, ctx->vl_eval_mlip, ctx->vl_eval_pair, ctx->flags_eval);
+    const double sh = 0.5 * ctx->cfg.skin;
+    launch_check_skin(L, n, n_states, ctx->q_eval, ctx->q_eval, sh * sh, ctx->flags_eval);
+    const int bm = ctx->bmax[which];
+    for (int b0 = 0; b0 < n_states; b0 += bm) {
+        const int B = std::min(bm, n_states - b0);
+        eval_forces(ctx, L, which, B, ctx->q_eval + n3 * b0, ctx->img_eval, ctx->vl_eval_mlip, ctx->vl_eval_pair, ctx->F_eval + n3 * b0,
+                    ctx->flags_eval, ctx->pot[which].mlip.F > 0 ? ctx->work[which].e_atom : nullptr);
+        if (energy_nn && ctx->pot[which].mlip.F > 0)
+            CK(cudaMemcpyAsync(ctx->e_eval + (size_t)n * b0, ctx->work[which].e_atom, (size_t)n * B * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    }
+    CK(cudaMemcpyAsync(F, ctx->F_eval, n3 * n_states * sizeof(double), out_kind, st));
+    if (energy_nn) {
+        if (ctx->pot[which].mlip.F > 0) CK(cudaMemcpyAsync(energy_nn, ctx->e_eval, (size_t)n * n_states * sizeof(double), out_kind, st));
+        else if (where == LSD_HOST) std::memset(energy_nn, 0, (size_t)n * n_states * sizeof(double));
+        else CK(cudaMemsetAsync(energy_nn, 0, (size_t)n * n_states * sizeof(double), st));
+    }
+    int hf = 0;
+    CK(cudaMemcpyAsync(&hf, ctx->flags_eval, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    return flags_to_status(ctx, hf);
+}
+
+lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t b, int64_t cap, int64_t* start, int32_t* idx,
+                             int8_t* shifts, int64_t* n_edges)
+{
+    if (!ctx || !start || !n_edges || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
+    const CompactList& cl = kind == 0 ? ctx->cl_mlip[which] : ctx->cl_pair[which];
+    if (!cl.count || !ctx->cl_img[which]) return fail(ctx, LSD_ERR_STATE, "this potential has no such list (or no evaluation has run yet)");
+    if (b < 0 || b >= cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "state index out of range");
+    CK(cudaDeviceSynchronize());
+    const int n = ctx->sys.n;
+    std::vector<int> count(n), img(n);
+    std::vector<uint32_t> keys((size_t)n * cl.cap);
+    CK(cudaMemcpy(count.data(), cl.count + (size_t)b * n, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(keys.data(), cl.keys + (size_t)b * n * cl.cap, sizeof(uint32_t) * keys.size(), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(img.data(), ctx->cl_img[which], sizeof(int) * n, cudaMemcpyDeviceToHost));
+    auto unpack = [](int v, int* o) { o[0] = (v & 1023) - 512; o[1] = ((v >> 10) & 1023) - 512; o[2] = ((v >> 20) & 1023) - 512; };
+    int64_t e = 0;
+    for (int i = 0; i < n; ++i) {
+        start[i] = e;
+        int ii[3]; unpack(img[i], ii);
+        for (int k = 0; k < count[i]; ++k, ++e) {
+            if (e >= cap || !idx || !shifts) continue;
+            const uint32_t key = keys[(size_t)i * cl.cap + k];
+            const int j = (int)(key >> 5), code = (int)(key & 31u);
+            int jj[3]; unpack(img[j], jj);
+            idx[e] = j;
+            shifts[3 * e + 0] = (int8_t)(code / 9 - 1 + ii[0] - jj[0]);
+            shifts[3 * e + 1] = (int8_t)((code / 3) % 3 - 1 + ii[1] - jj[1]);
+            shifts[3 * e + 2] = (int8_t)(code % 3 - 1 + ii[2] - jj[2]);
+        }
+    }
+    start[n] = e; *n_edges = e;
+    return LSD_OK;
+}
+
+}  // extern "C"

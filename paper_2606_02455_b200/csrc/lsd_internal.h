@@ -1,0 +1,132 @@
+// Internal declarations shared by the translation units of liblsd_b200.so (sm_100a only).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "lsd.h"
+
+#define LSD_KB_EV   8.617333262e-5   // eV / K
+#define LSD_AMU_EV  103.642696       // eV fs^2 / A^2 per amu
+#define LSD_NRBF    32               // R (M1)
+#define LSD_MAX_K   64
+
+// flags raised on the device during a window
+#define LSD_FLAG_SKIN      1
+#define LSD_FLAG_OVERFLOW  2
+#define LSD_FLAG_NONFINITE 4
+
+struct SysDev {
+    int n = 0, ns = 0, periodic = 0;
+    double box[3] = {0, 0, 0};
+    int* species = nullptr;          // [n]
+    double* mass = nullptr;          // [n] internal units (amu * LSD_AMU_EV)
+    double* sigma = nullptr;         // [n] sqrt(m kT (1 - c1^2))
+    // bonded terms, gather form: per atom list of (term, role)
+    int n_bonds = 0, n_angles = 0;
+    int* bonds = nullptr; double* bond_k = nullptr; double* bond_r0 = nullptr;
+    int* angles = nullptr; double* angle_k = nullptr; double* angle_t0 = nullptr;
+    int* bt_start = nullptr;         // [n+1]
+    int* bt_term = nullptr;          // term id: bonds 0..nb-1, angles nb..nb+na-1 ; role packed in high bits
+};
+
+struct MlipDev {
+    int F = 0, T = 0, R = LSD_NRBF, ns = 0;
+    float rc = 0.f, alpha = 0.f;
+    float* emb = nullptr;                       // [ns][F]
+    // per block, fp32, all stored k-major [K][N] for  C[rows][N] = A[rows][K] * W[K][N]
+    std::vector<float*> WinT, Win, Wf1T, Wf2T, Wo1T, Wo1, Wo2T, Wo2;
+    float* Wr1 = nullptr;                       // [F/2][F]
+    float* wr2 = nullptr;                       // [F/2]
+    // bf16 copies for the tcgen05 path (K-major operands), filled when precision == LSD_BF16_TC
+    std::vector<void*> Wf1_bf16, Wf2_bf16;
+};
+
+struct PotDev {
+    int ns = 0, use_bonded = 0;
+    double* pair = nullptr;          // [ns*ns*8]
+    double* pair_rc2 = nullptr;      // [ns*ns] squared cutoff of the pair term (0 = none)
+    double* tether = nullptr;        // [ns]
+    double pair_rcmax = 0.0;
+    int has_tether = 0;
+    MlipDev mlip;
+};
+
+struct VerletList {                  // window-shared candidate list (r < rc + skin at the reference state)
+    int cap = 0;
+    double rc = 0.0;                 // largest cutoff served
+    int* count = nullptr;            // [n]
+    uint32_t* keys = nullptr;        // [n][cap]  key = (j << 5) | shiftcode, sorted ascending
+};
+
+struct CompactList {                 // per-state exact list (r < rc), rows padded with 0xFFFFFFFF
+    int cap = 0, bmax = 0;
+    int* count = nullptr;            // [bmax*n]
+    uint32_t* keys = nullptr;        // [bmax*n][cap]
+};
+
+struct CellGrid {
+    int nc[3] = {1, 1, 1};
+    int ncell = 1;
+    int* cell_count = nullptr;       // [ncell]
+    int* cell_start = nullptr;       // [ncell+1]
+    int* cell_cursor = nullptr;      // [ncell]
+    int* cell_atoms = nullptr;       // [n]
+    int* atom_cell = nullptr;        // [n]
+    int cap_cells = 0;
+};
+
+struct MlipWork {                    // activations of one batched evaluation (kept for the analytic backward, M9)
+    int bmax = 0;
+    float *x = nullptr, *m = nullptr, *mbar = nullptr, *xbar = nullptr, *ybar = nullptr;
+    std::vector<float*> y, h;        // [T] each [bmax*n][F]
+    double* e_atom = nullptr;        // [bmax*n]
+};
+
+struct Launcher {                    // stream + launch counter
+    cudaStream_t s;
+    int64_t* counter;
+};
+#define LSD_COUNT(L) (++(*(L).counter))
+
+// ---- integrator.cu
+void launch_half_a(Launcher L, int n, const double* q, const double* p, const double* mass, double hdt,
+                   double* qhalf, const double* qref, double skin_half2, int* flags);
+void launch_bob_a(Launcher L, int n, uint64_t seed, uint64_t step, const double* p_prev, const double* Ft,
+                  const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
+                  double* q_new, double* p_new);
+void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p);
+struct TransportResult { int first_reject, n_commit, flags, pad; double beta_sum; };
+void launch_transport(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const double* Ft, const double* Fg,
+                      const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg);
+void launch_commit(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const TransportResult* result,
+                   const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
+                   const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
+                   double c1, double b, double hdt, double* q_base, double* p_base);
+int transport_blocks(int n);
+
+// ---- neighbor.cu
+void cellgrid_setup(CellGrid& g, const SysDev& sys, double rc_skin);
+void launch_pack_ref(Launcher L, const SysDev& sys, const double* qref, int* img);
+void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const double* qref, const int* img,
+                         double rc_skin, VerletList& vl, int* flags);
+void launch_compact(Launcher L, const SysDev& sys, int B, const double* q /*[B][3][n]*/, const int* img,
+                    const VerletList& vl, double rc2_single, const double* pair_rc2 /*or null*/, CompactList& cl, int* flags);
+void launch_check_skin(Launcher L, int n, int B, const double* q, const double* qref, double skin_half2, int* flags);
+
+// ---- prior.cu
+void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B, const double* q, const int* img,
+                         const CompactList* pairlist, double* F /*[B][3][n], overwritten*/);
+
+// ---- mlip_simt.cu
+void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);
+size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
+
+// ---- mlip_tc.cu (bf16 tcgen05 filter path)
+bool mlip_tc_supported(const MlipDev& net);
+void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                  const int* img, const CompactList& cl, double* F, double* e_atom);

@@ -1,0 +1,417 @@
+// SchNet-style MLIP (M1-M9): forward pass and hand-derived analytic force backward, fp32 on the FMA pipes.
+// No autograd, no float atomics: every per-atom sum runs in the order of the atom's sorted neighbour row, inside
+// one warp, so results are bit-reproducible and independent of the batch size (draft == target => F~ == F bitwise).
+//
+// Structure of every kernel: persistent CTAs, the block's weight matrices resident in shared memory, each warp
+// loops over work items and multiplies an 8-row tile by the resident matrix (rows = edges of one atom for the
+// filter MLP, rows = atoms for the atom-wise layers).
+//
+//   forward block t :  y = W_in x ;  m_a = sum_j y_j . w_aj ;  h = W_o1 m ;  x += W_o2 ssp(h)
+//   filter          :  w(r) = (W_f2 ssp(W_f1 g(r))) f_c(r)
+//   backward block t:  hbar = logistic(h) . (W_o2^T xbar) ;  mbar = W_o1^T hbar ;
+//                      ybar_a = sum_j mbar_j . w_aj ;
+//                      F_a   += sum_j [ sum_f (mbar_a y_j + mbar_j y_a)_f w'_aj,f ] rhat_aj ;   xbar += W_in^T ybar
+#include <algorithm>
+#include "lsd_internal.h"
+
+namespace {
+
+constexpr int kWarps = 8;
+constexpr int kThreads = kWarps * 32;
+constexpr float kLn2 = 0.69314718055994530942f;
+
+__device__ __forceinline__ float ssp(float x) { return fmaxf(x, 0.f) + log1pf(expf(-fabsf(x))) - kLn2; }          // M3
+__device__ __forceinline__ float logistic(float x) { return 1.f / (1.f + expf(-x)); }
+__device__ __forceinline__ void img_unpack(int v, int& ix, int& iy, int& iz) { ix = (v & 1023) - 512; iy = ((v >> 10) & 1023) - 512; iz = ((v >> 20) & 1023) - 512; }
+
+template <int CPT> struct Vec;
+template <> struct Vec<4> { using T = float4; };
+template <> struct Vec<2> { using T = float2; };
+template <> struct Vec<1> { using T = float; };
+
+template <int CPT> __device__ __forceinline__ void ldv(const float* p, float (&v)[CPT])
+{
+    typename Vec<CPT>::T t = *reinterpret_cast<const typename Vec<CPT>::T*>(p);
+    const float* f = reinterpret_cast<const float*>(&t);
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) v[c] = f[c];
+}
+template <int CPT> __device__ __forceinline__ void stv(float* p, const float (&v)[CPT])
+{
+    typename Vec<CPT>::T t;
+    float* f = reinterpret_cast<float*>(&t);
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) f[c] = v[c];
+    *reinterpret_cast<typename Vec<CPT>::T*>(p) = t;
+}
+
+// acc[8][CPT] = A[8][KD] (shared, row-major, leading dimension lda) * W[KD][F] (shared); lane owns channels lane*CPT..
+template <int KD, int F>
+__device__ __forceinline__ void warp_gemm8(const float* __restrict__ As, int lda, const float* __restrict__ Ws, int lane, float (&acc)[8][F / 32])
+{
+    constexpr int CPT = F / 32;
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) acc[r][c] = 0.f;
+#pragma unroll 2
+    for (int k4 = 0; k4 < KD / 4; ++k4) {
+        float4 a[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) a[r] = *reinterpret_cast<const float4*>(As + r * lda + 4 * k4);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+            float w[CPT];
+            ldv<CPT>(Ws + (4 * k4 + kk) * F + lane * CPT, w);
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const float av = kk == 0 ? a[r].x : kk == 1 ? a[r].y : kk == 2 ? a[r].z : a[r].w;
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) acc[r][c] = fmaf(av, w[c], acc[r][c]);
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void load_weights(float* dst, const float* __restrict__ src, int count)
+{
+    for (int i = threadIdx.x * 4; i < count; i += kThreads * 4) *reinterpret_cast<float4*>(dst + i) = *reinterpret_cast<const float4*>(src + i);
+}
+
+// ------------------------------------------------------------------------------------------------ embedding (M4)
+__global__ void k_embed(int total, int n, int F, const int* __restrict__ species, const float* __restrict__ emb, float* __restrict__ x)
+{
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (size_t)total * F) return;
+    const int g = (int)(t / F), f = (int)(t % F);
+    x[t] = emb[species[g % n] * F + f];
+}
+
+// ------------------------------------------------------------------------------------------------ atom-wise layers
+enum DenseMode { DENSE_IN = 0, DENSE_OUT = 1, BWD_OUT = 2, BWD_IN = 3 };
+
+// DENSE_IN : out = in * W0                                   (y = W_in x)
+// DENSE_OUT: aux = in * W0 ; io += ssp(aux) * W1             (h = W_o1 m ; x += W_o2 ssp(h))
+// BWD_OUT  : out = (logistic(aux) . (in * W0)) * W1          (mbar = W_o1^T (logistic(h) . W_o2^T xbar))
+// BWD_IN   : io += in * W0                                   (xbar += W_in^T ybar)
+template <int F, int MODE>
+__global__ void __launch_bounds__(kThreads, 1)
+k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, const float* __restrict__ W1,
+        float* __restrict__ aux, float* __restrict__ out)
+{
+    constexpr int CPT = F / 32, LDA = F + 4;
+    constexpr bool TWO = (MODE == DENSE_OUT || MODE == BWD_OUT);
+    extern __shared__ __align__(16) float smem[];
+    float* Ws0 = smem;
+    float* Ws1 = Ws0 + F * F;
+    float* Asw = Ws0 + (TWO ? 2 : 1) * F * F + (threadIdx.x >> 5) * 8 * LDA;
+    load_weights(Ws0, W0, F * F);
+    if (TWO) load_weights(Ws1, W1, F * F);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ntiles = (total + 7) / 8;
+    for (int tile = blockIdx.x * kWarps + warp; tile < ntiles; tile += gridDim.x * kWarps) {
+        const int g0 = tile * 8;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            float v[CPT];
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) v[c] = 0.f;
+            if (g0 + r < total) ldv<CPT>(in + (size_t)(g0 + r) * F + lane * CPT, v);
+            stv<CPT>(Asw + r * LDA + lane * CPT, v);
+        }
+        __syncwarp();
+        float acc[8][CPT];
+        warp_gemm8<F, F>(Asw, LDA, Ws0, lane, acc);
+        if (MODE == DENSE_IN) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) if (g0 + r < total) stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc[r]);
+        } else if (MODE == BWD_IN) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) if (g0 + r < total) {
+                float v[CPT];
+                ldv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, v);
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) v[c] += acc[r][c];
+                stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, v);
+            }
+        } else {
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                float v[CPT];
+                if (MODE == DENSE_OUT) {
+                    if (g0 + r < total) stv<CPT>(aux + (size_t)(g0 + r) * F + lane * CPT, acc[r]);      // keep h for the backward
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) v[c] = ssp(acc[r][c]);
+                } else {
+                    float hv[CPT];
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) hv[c] = 0.f;
+                    if (g0 + r < total) ldv<CPT>(aux + (size_t)(g0 + r) * F + lane * CPT, hv);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) v[c] = logistic(hv[c]) * acc[r][c];
+                }
+                stv<CPT>(Asw + r * LDA + lane * CPT, v);
+            }
+            __syncwarp();
+            float acc2[8][CPT];
+            warp_gemm8<F, F>(Asw, LDA, Ws1, lane, acc2);
+#pragma unroll
+            for (int r = 0; r < 8; ++r) if (g0 + r < total) {
+                if (MODE == DENSE_OUT) {
+                    float v[CPT];
+                    ldv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, v);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) v[c] += acc2[r][c];
+                    stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, v);
+                } else {
+                    stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
+                }
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ readout (M6) + xbar seed
+// z = W_r1 x ; e = alpha w_r2 . ssp(z) ; xbar = alpha W_r1^T (logistic(z) . w_r2).  One warp per atom.
+template <int F>
+__global__ void __launch_bounds__(kThreads)
+k_readout(int total, float alpha, const float* __restrict__ x, const float* __restrict__ Wr1, const float* __restrict__ wr2,
+          float* __restrict__ xbar, double* __restrict__ e_atom)
+{
+    constexpr int H = F / 2, LD = F + 1;
+    extern __shared__ __align__(16) float smem[];
+    float* Ws = smem;                       // [H][F+1]
+    float* w2 = Ws + H * LD;                // [H]
+    float* xs = w2 + H + (threadIdx.x >> 5) * (F + H);   // per warp: x[F], s[H]
+    for (int i = threadIdx.x; i < H * F; i += kThreads) Ws[(i / F) * LD + (i % F)] = Wr1[i];
+    for (int i = threadIdx.x; i < H; i += kThreads) w2[i] = wr2[i];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* ss = xs + F;
+    for (int g = blockIdx.x * kWarps + warp; g < total; g += gridDim.x * kWarps) {
+        for (int f = lane; f < F; f += 32) xs[f] = x[(size_t)g * F + f];
+        __syncwarp();
+        float e = 0.f;
+        for (int k = lane; k < H; k += 32) {
+            float z = 0.f;
+            for (int f = 0; f < F; ++f) z = fmaf(Ws[k * LD + f], xs[f], z);
+            e += w2[k] * ssp(z);
+            ss[k] = logistic(z) * w2[k];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        __syncwarp();
+        for (int f = lane; f < F; f += 32) {
+            float v = 0.f;
+            for (int k = 0; k < H; ++k) v = fmaf(Ws[k * LD + f], ss[k], v);
+            xbar[(size_t)g * F + f] = alpha * v;
+        }
+        if (lane == 0 && e_atom) e_atom[g] = (double)(alpha * e);
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ continuous-filter convolution
+struct EdgeArgs {
+    int total, n, cap;
+    const int* count; const uint32_t* keys; const int* img;
+    const double* q;                  // [B][3][n]
+    double box[3];
+    float rc, inv_rc, delta, inv_delta2;
+    const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major)
+    const float* y;                   // [total][F]
+    float* m_out;                     // FWD: m
+    const float* mbar; float* ybar;   // BWD
+    double* Fout;                     // BWD: [B][3][n], accumulated
+};
+
+template <int F, bool BWD>
+__global__ void __launch_bounds__(kThreads, 1)
+k_edge(EdgeArgs a)
+{
+    constexpr int CPT = F / 32, LDA = F + 4, LDG = LSD_NRBF + 4, SPW = BWD ? 4 : 8;
+    extern __shared__ __align__(16) float smem[];
+    float* Wf1 = smem;                                   // [32][F]
+    float* Wf2 = Wf1 + LSD_NRBF * F;                     // [F][F]
+    float* Gs = Wf2 + F * F + (threadIdx.x >> 5) * (8 * LDG + 8 * LDA);
+    float* As = Gs + 8 * LDG;
+    load_weights(Wf1, a.Wf1, LSD_NRBF * F);
+    load_weights(Wf2, a.Wf2, F * F);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n = a.n;
+    for (int g = blockIdx.x * kWarps + warp; g < a.total; g += gridDim.x * kWarps) {
+        const int b = g / n, i = g % n;
+        const double* qb = a.q + (size_t)b * 3 * n;
+        const int cnt = a.count[g];
+        const uint32_t* row = a.keys + (size_t)g * a.cap;
+        const double qi0 = qb[i], qi1 = qb[n + i], qi2 = qb[2 * n + i];
+        int iix, iiy, iiz; img_unpack(a.img[i], iix, iiy, iiz);
+        float part[CPT], ya[CPT], mba[CPT];
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) part[c] = 0.f;
+        if (BWD) { ldv<CPT>(a.y + (size_t)g * F + lane * CPT, ya); ldv<CPT>(a.mbar + (size_t)g * F + lane * CPT, mba); }
+        double fx = 0.0, fy = 0.0, fz = 0.0;
+        for (int u0 = 0; u0 < cnt; u0 += SPW) {
+            // --- geometry of the unit's slots (lanes 0..SPW-1), fp64 displacement -> fp32
+            const int slot = u0 + lane;
+            const bool valid = lane < SPW && slot < cnt;
+            float r = 0.f, fc = 0.f, fcp = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
+            int jrow = g;
+            if (valid) {
+                const uint32_t key = row[slot];
+                const int j = (int)(key >> 5), code = (int)(key & 31u);
+                int jx, jy, jz; img_unpack(a.img[j], jx, jy, jz);
+                const double d0 = (qb[j] - qi0) + (double)(code / 9 - 1 + iix - jx) * a.box[0];
+                const double d1 = (qb[n + j] - qi1) + (double)((code / 3) % 3 - 1 + iiy - jy) * a.box[1];
+                const double d2 = (qb[2 * n + j] - qi2) + (double)(code % 3 - 1 + iiz - jz) * a.box[2];
+                const double rd = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+                r = (float)rd; ux = (float)(d0 / rd); uy = (float)(d1 / rd); uz = (float)(d2 / rd);
+                const float t = r * a.inv_rc;
+                if (t < 1.f) {                                                            // M2
+                    float sn, cs; sincospif(t, &sn, &cs);
+                    fc = 0.5f * (cs + 1.f); fcp = -0.5f * 3.14159265358979323846f * a.inv_rc * sn;
+                }
+                jrow = b * n + j;
+            }
+            // --- radial basis rows (M1): lane k holds basis k; BWD interleaves value / r-derivative rows
+#pragma unroll
+            for (int e = 0; e < SPW; ++e) {
+                const float re = __shfl_sync(0xffffffffu, r, e);
+                const bool ve = (u0 + e) < cnt;
+                const float x = re - (float)lane * a.delta;
+                const float gk = ve ? expf(-0.5f * x * x * a.inv_delta2) : 0.f;
+                if (BWD) { Gs[(2 * e) * LDG + lane] = gk; Gs[(2 * e + 1) * LDG + lane] = -gk * x * a.inv_delta2; }
+                else Gs[e * LDG + lane] = gk;
+            }
+            __syncwarp();
+            float acc[8][CPT];
+            warp_gemm8<LSD_NRBF, F>(Gs, LDG, Wf1, lane, acc);
+            // --- activation (M3) -> A operand of the second layer
+            if (BWD) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    float v0[CPT], v1[CPT];
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) { v0[c] = ssp(acc[2 * e][c]); v1[c] = logistic(acc[2 * e][c]) * acc[2 * e + 1][c]; }
+                    stv<CPT>(As + (2 * e) * LDA + lane * CPT, v0);
+                    stv<CPT>(As + (2 * e + 1) * LDA + lane * CPT, v1);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    float v0[CPT];
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) v0[c] = ssp(acc[e][c]);
+                    stv<CPT>(As + e * LDA + lane * CPT, v0);
+                }
+            }
+            __syncwarp();
+            warp_gemm8<F, F>(As, LDA, Wf2, lane, acc);
+            // --- epilogue: cfconv gather (and its adjoints)
+#pragma unroll
+            for (int e = 0; e < SPW; ++e) {
+                const int jr = __shfl_sync(0xffffffffu, jrow, e);
+                const float fce = __shfl_sync(0xffffffffu, fc, e);
+                float yj[CPT];
+                if (!BWD) {
+                    ldv<CPT>(a.y + (size_t)jr * F + lane * CPT, yj);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) part[c] = fmaf(yj[c], acc[e][c] * fce, part[c]);
+                } else {
+                    const float fcpe = __shfl_sync(0xffffffffu, fcp, e);
+                    const float uxe = __shfl_sync(0xffffffffu, ux, e), uye = __shfl_sync(0xffffffffu, uy, e), uze = __shfl_sync(0xffffffffu, uz, e);
+                    float mbj[CPT];
+                    ldv<CPT>(a.y + (size_t)jr * F + lane * CPT, yj);
+                    ldv<CPT>(a.mbar + (size_t)jr * F + lane * CPT, mbj);
+                    float gp = 0.f;
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) {
+                        const float w = acc[2 * e][c] * fce;
+                        const float wp = acc[2 * e + 1][c] * fce + acc[2 * e][c] * fcpe;
+                        part[c] = fmaf(mbj[c], w, part[c]);
+                        gp = fmaf(fmaf(mba[c], yj[c], mbj[c] * ya[c]), wp, gp);
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) gp += __shfl_xor_sync(0xffffffffu, gp, o);
+                    fx += (double)(gp * uxe); fy += (double)(gp * uye); fz += (double)(gp * uze);
+                }
+            }
+            __syncwarp();
+        }
+        if (!BWD) stv<CPT>(a.m_out + (size_t)g * F + lane * CPT, part);
+        else {
+            if (a.ybar) stv<CPT>(a.ybar + (size_t)g * F + lane * CPT, part);
+            if (lane == 0) {
+                double* Fb = a.Fout + (size_t)b * 3 * n;
+                Fb[i] += fx; Fb[n + i] += fy; Fb[2 * n + i] += fz;
+            }
+        }
+    }
+}
+
+template <int F> size_t smem_dense(bool two) { return sizeof(float) * ((two ? 2 : 1) * F * F + kWarps * 8 * (F + 4)); }
+template <int F> size_t smem_edge() { return sizeof(float) * (LSD_NRBF * F + F * F + kWarps * (8 * (LSD_NRBF + 4) + 8 * (F + 4))); }
+template <int F> size_t smem_readout() { return sizeof(float) * ((F / 2) * (F + 1) + F / 2 + kWarps * (F + F / 2)); }
+
+int g_num_sms = 0;
+int num_sms() { if (!g_num_sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev); if (g_num_sms <= 0) g_num_sms = 148; } return g_num_sms; }
+
+template <typename K> void set_smem(K kernel, size_t bytes) { cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes); }
+
+template <int F>
+void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q, const int* img,
+              const CompactList& cl, double* Fout, double* e_atom)
+{
+    const int total = B * sys.n;
+    static bool configured = false;
+    if (!configured) {
+        set_smem(k_dense<F, DENSE_IN>, smem_dense<F>(false)); set_smem(k_dense<F, BWD_IN>, smem_dense<F>(false));
+        set_smem(k_dense<F, DENSE_OUT>, smem_dense<F>(true)); set_smem(k_dense<F, BWD_OUT>, smem_dense<F>(true));
+        set_smem(k_edge<F, false>, smem_edge<F>()); set_smem(k_edge<F, true>, smem_edge<F>());
+        set_smem(k_readout<F>, smem_readout<F>());
+        configured = true;
+    }
+    const int sms = num_sms();
+    const int grid_tiles = std::max(1, std::min(sms, (total + kWarps * 8 - 1) / (kWarps * 8)));
+    const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
+    k_embed<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, w.x); LSD_COUNT(L);
+    EdgeArgs ea{};
+    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.img = img; ea.q = q;
+    for (int c = 0; c < 3; ++c) ea.box[c] = sys.box[c];
+    ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
+    for (int t = 0; t < net.T; ++t) {
+        k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t]); LSD_COUNT(L);
+        ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
+        k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
+        k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x); LSD_COUNT(L);
+    }
+    k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
+    for (int t = net.T - 1; t >= 0; --t) {
+        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar); LSD_COUNT(L);
+        ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
+        k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
+        if (t > 0) { k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar); LSD_COUNT(L); }
+    }
+}
+
+}  // namespace
+
+size_t mlip_work_bytes(const MlipDev& net, int n, int bmax)
+{
+    return sizeof(float) * (size_t)n * bmax * net.F * (5 + 2 * net.T) + sizeof(double) * (size_t)n * bmax;
+}
+
+void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                const int* img, const CompactList& cl, double* F, double* e_atom)
+{
+    switch (net.F) {
+        case 32:  run_fp32<32>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
+        case 64:  run_fp32<64>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
+        case 128: run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
+        default: break;
+    }
+}
