@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LSD window-verification hot path on B200.
+
+A "step" is one pass of the whole hot path over one window of K draft steps:
+draft rollout -> window-shared neighbour lists -> batched target forces -> transport map + first-reject scan ->
+override/commit -> rollback.  `value` = atom-steps verified per second (K * N * steps * n_gpus / time);
+committed ("accepted target-exact") MD steps/s is reported beside it.  One JSON line on stdout (rank 0).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl reference]
+
+Multi-GPU (weak scaling): every rank runs an independent replica of the workload (its own seed); there is no
+data-path collective.  --impl reference times the CPU oracle (oracle/, fp64, as it stands).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "batched force-eval atom-steps/s (whole verified window; accepted target-exact MD steps/s beside it)"
+UNIT = "atom-steps/s"
+
+# bounded oracle samples: same per-atom cost as the full workload, sized for ~10-30 s of CPU work
+CPU_SAMPLES = {
+    "cfg1": dict(kw={}, K=4, windows=200),
+    "cfg2": dict(kw={}, K=16, windows=40),
+    "cfg3": dict(kw={"n_grid": 7}, K=2, windows=1),
+    "cfg4": dict(kw={"n_atoms": 1000}, K=2, windows=1),
+    "cfg5": dict(kw={"cells": (6, 6, 6)}, K=2, windows=1),
+}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], bf16=d.get("bf16_tflops_sustained", d["bf16_tflops"]), bf16_burst=d["bf16_tflops"],
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, bf16=1400.0, bf16_burst=1590.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i", str(self.index)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, col in (("hw_slowdown", 5), ("hw_thermal_slowdown", 6), ("sw_thermal_slowdown", 7), ("sw_power_cap", 8)):
+                if len(r) > col and r[col].lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=sorted(reasons), samples=len(sm))
+
+
+def cpu_baseline(name, steps=1):
+    """The oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    import lsd_inputs as L
+    import oracle
+    s = CPU_SAMPLES[name]
+    w = L.make_workload(name, **s["kw"])
+    p0 = oracle.initial_momenta(w)
+    oracle.lsd_window(w, w.q0, p0, 0, K=1, debug=False)                 # warm (build + page-in)
+    q, p, n = w.q0, p0, 0
+    atom_steps = committed = 0
+    t0 = time.perf_counter()
+    for _ in range(steps * s["windows"]):
+        r = oracle.lsd_window(w, q, p, n, K=s["K"], debug=True)         # debug=True: all K target evaluations, like the batched GPU call
+        q, p, n = r["q"], r["p"], n + r["n_commit"]
+        atom_steps += s["K"] * w.n_atoms
+        committed += r["n_commit"]
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return dict(value=atom_steps / dt, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{name} scaled to {w.n_atoms} atoms ({s['kw'] or 'full size'}), {steps * s['windows']} window(s) of K={s['K']}, fp64, {dt:.1f} s",
+                committed_md_steps_per_s=committed / dt, seconds=dt)
+
+
+def run_reference(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    per = []
+    base = None
+    for _ in range(args.warmup if args.warmup < 1 else 1):
+        cpu_baseline(args.workload, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        base = cpu_baseline(args.workload, 1)
+        per.append(base["value"])
+    dt = time.perf_counter() - t0
+    val = float(np.mean(per))
+    line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * dt / max(args.steps, 1), higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=args.workload, note="CPU oracle (oracle/lsd_oracle.c) on a bounded sample; each step = one sample"),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=base["cores"], kind="oracle", sample=base["sample"]),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--precision", default=None, choices=[None, "fp32", "bf16"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--overlap", type=int, default=0, help="1: time lsd_run with the speculative second-stream rollout instead of explicit calls")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import lsd_inputs as L
+    import paper_2606_02455_b200 as P
+
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    P.load_library()
+    peaks = load_peaks()
+
+    w = L.make_workload(args.workload)
+    K, N = w.K, w.n_atoms
+    prec = {"fp32": P.LSD_FP32, "bf16": P.LSD_BF16_TC, None: None}[args.precision]
+    ctx = P.context_from_workload(w, precision=prec, seed=w.seed + 1000 * rank)
+    stream = torch.cuda.Stream()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    tgt = w.target.mlip
+    work_bytes = 0 if tgt is None else 4 * N * K * tgt.width * (5 + 2 * tgt.n_blocks)
+    need_flush = work_bytes < 2 * 126e6
+
+    def one_window():
+        if args.overlap:
+            P.lsd_run(ctx.h, K, K, overlap=True, stream=stream)
+            return None
+        return ctx.window(K, stream)
+
+    for _ in range(args.warmup):
+        one_window()
+    torch.cuda.synchronize()
+    steps_before = P.lsd_get_stats(ctx.h)["committed_steps"]
+    launches_before = P.lsd_launch_count(ctx.h)
+    P.lsd_profile(ctx.h, True)
+    sampler = ClockSampler(local)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for s in range(args.steps):
+        if need_flush:
+            flush.fill_(s & 0xFF)
+        ev[s][0].record(stream)
+        one_window()
+        ev[s][1].record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    prof = P.lsd_get_profile(ctx.h)
+    P.lsd_profile(ctx.h, False)
+    launches = P.lsd_launch_count(ctx.h) - launches_before
+    committed = P.lsd_get_stats(ctx.h)["committed_steps"] - steps_before
+    edges = P.lsd_get_edge_count(ctx.h, P.LSD_TARGET, 0, K) if tgt is not None else 0
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        c = torch.tensor([float(committed)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        committed_all = float(c.item())
+    else:
+        committed_all = float(committed)
+    value = K * N * args.steps * world / (ms * 1e-3)
+
+    # ---- end-to-end through the C ABI with HOST buffers (pinned): upload x_n, run the window, read x_{n+commit} back
+    qh = torch.empty((3, N), dtype=torch.float64).pin_memory()
+    ph = torch.empty((3, N), dtype=torch.float64).pin_memory()
+    step0 = P.lsd_get_state(ctx.h, qh.numpy(), ph.numpy())
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        P.lsd_set_state(ctx.h, qh.numpy(), ph.numpy(), step0)
+        ctx.window(K, stream)
+        step0 = P.lsd_get_state(ctx.h, qh.numpy(), ph.numpy())
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = dict(value=K * N * args.steps * world / e2e_s, unit=UNIT, h2d_bytes_per_step=2 * 3 * N * 8, d2h_bytes_per_step=2 * 3 * N * 8 + 8,
+               ms_per_step=1e3 * e2e_s / args.steps)
+
+    # ---- roofline of the dominant kernel: the MLIP edge backward kernel (filter value + tangent, cfconv adjoints)
+    roofline = None
+    dtype = "f64"
+    if tgt is not None:
+        F, R, T = tgt.width, tgt.n_rbf, tgt.n_blocks
+        eb = prof["mlip_edge_bwd"]
+        flops_per_launch = edges * (2 * R * F + 2 * F * F + 6 * F)        # strict algorithmic count of the backward edge pass
+        avg_ms = eb["ms"] / max(eb["launches"], 1)
+        achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
+        use_tc = (prec if prec is not None else (P.LSD_BF16_TC if w.precision == "bf16" else P.LSD_FP32)) == P.LSD_BF16_TC and P.lsd_tc_enabled(ctx.h)
+        if use_tc:
+            bound, peak, dtype = "tensor", peaks["bf16"], "bf16"
+            peak_note = f"bf16 dense sustained, {peaks['source']}"
+        else:
+            bound, dtype = "alu", "f32"
+            peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12         # fp32 FMA lanes x 2 flop x max SM clock
+            peak_note = "fp32 FMA pipe: 148 SMs x 128 lanes x 2 flop x clocks.max.sm (derived, DESIGN.md)"
+        mlip_ms = prof["mlip_edge_bwd"]["ms"] + prof["mlip_edge_fwd"]["ms"] + prof["mlip_dense"]["ms"]
+        roofline = dict(bound=bound, achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak, traffic=None,
+                        kernel="k_edge<F,true> (MLIP edge backward)", avg_launch_ms=avg_ms, launches=eb["launches"],
+                        algorithmic_flops_per_launch=flops_per_launch, directed_edges_per_window=edges, peak_note=peak_note,
+                        share_of_step=eb["ms"] / ms if ms > 0 else None,
+                        a2_strict_tflops=edges * T * (2 * R * F + 2 * F * F + 8 * F) / (mlip_ms * 1e-3) / 1e12 if mlip_ms > 0 else None,
+                        stage_ms_per_step={k: v["ms"] / args.steps for k, v in prof.items() if v["launches"]})
+
+    if rank == 0:
+        line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms / args.steps,
+                    higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
+                    config=dict(workload=args.workload, n_atoms=N, window_K=K, atoms_per_window=K * N, integrator="ABOBA (Eq. 2)",
+                                l2="flushed between timed steps (256 MiB write)" if need_flush else "working set larger than L2",
+                                overlap=bool(args.overlap), replicas=world, peaks=peaks["source"]),
+                    committed_md_steps_per_s=committed_all / (ms * 1e-3), committed_per_window=committed_all / (args.steps * world),
+                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline)
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = {k: v for k, v in cpu_baseline(args.workload).items() if k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -185,11 +185,26 @@ lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const 
 lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t b, int64_t cap,
                              int64_t* start, int32_t* idx, int8_t* shifts, int64_t* n_edges);
 
+/* Re-size the window-shared lists for a new skin (synchronises; drops drafted windows).  lsd_run calls it with
+ * 2 x skin when a window reports SKIN_VIOLATED and redoes that window. */
 lsd_status lsd_set_skin(lsd_ctx* ctx, double skin);
+
+/* Total number of directed edges in the exact lists of the first n_states states of the last evaluation of
+ * potential `which` (kind as in lsd_get_neighbors).  Synchronises. */
+lsd_status lsd_get_edge_count(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t n_states, int64_t* total);
+
+/* Per-kernel-class device timing with CUDA events on the launching stream (used by bench.py for the roofline).
+ * Classes: 0 neighbour lists, 1 priors, 2 MLIP atom-wise layers, 3 MLIP edge forward, 4 MLIP edge backward,
+ * 5 integrator, 6 transport.  lsd_profile(1) starts (and clears), lsd_profile(0) stops.  lsd_get_profile
+ * synchronises and returns accumulated milliseconds and launch counts, ms[8], count[8]. */
+lsd_status lsd_profile(lsd_ctx* ctx, int32_t enable);
+lsd_status lsd_get_profile(lsd_ctx* ctx, double* ms, int64_t* count);
 
 /* Number of kernels this library has launched on behalf of ctx (bench.py's gpu_launches). */
 int64_t     lsd_launch_count(const lsd_ctx* ctx);
 const char* lsd_version(void);
+/* 1 if the target network's filter contractions run on the bf16 tcgen05 path in this context, else 0. */
+int32_t     lsd_tc_enabled(const lsd_ctx* ctx);
 
 #ifdef __cplusplus
 }

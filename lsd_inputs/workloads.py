@@ -194,7 +194,7 @@ def _cfg2(n_chain: int = 22) -> Workload:
     return Workload("cfg2", n_chain, 4, species, _HCNO_MASS[species], np.zeros(3), False, q,
                     bonds, np.full(len(bonds), 20.0), np.full(len(bonds), r0),
                     angles, np.full(len(angles), 2.0), np.full(len(angles), th0),
-                    drf, tgt, 300.0, 0.01, 0.5, 16, 1, 10000, "fp32", skin=0.5)
+                    drf, tgt, 300.0, 0.01, 0.5, 16, 1, 10000, "fp32", skin=2.0)
 
 
 # --------------------------------------------------------------------------- cfg 3
@@ -239,7 +239,7 @@ def _cfg3(n_grid: int = 8) -> Workload:
     return Workload(name, 3 * nm, 2, species, mass, np.full(3, L), True, q,
                     bonds, np.full(len(bonds), 20.0), np.full(len(bonds), roh),
                     angles, np.full(len(angles), 2.0), np.full(len(angles), th),
-                    drf, tgt, 300.0, 0.01, 0.5, 16, 3, 1000, "fp32", skin=0.5)
+                    drf, tgt, 300.0, 0.01, 0.5, 16, 3, 1000, "fp32", skin=1.2)
 
 
 # --------------------------------------------------------------------------- cfg 4

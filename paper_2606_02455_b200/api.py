@@ -21,7 +21,7 @@ _STATUS = {0: "LSD_OK", -1: "LSD_ERR_INVALID_ARG", -2: "LSD_ERR_CUDA", -3: "LSD_
 
 EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_rollout", "lsd_verify_window", "lsd_transport_accept",
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
-                    "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version"]
+                    "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled"]
 
 
 class LsdError(RuntimeError):
@@ -224,8 +224,31 @@ def lsd_get_neighbors(h, which, kind, b, n_atoms):
     return start, idx[: ne.value].copy(), sh[: ne.value].copy()
 
 
+def lsd_get_edge_count(h, which, kind, n_states) -> int:
+    t = C.c_int64()
+    _check(h, load_library().lsd_get_edge_count(h, C.c_int32(which), C.c_int32(kind), C.c_int32(n_states), C.byref(t)))
+    return int(t.value)
+
+
 def lsd_set_skin(h, skin):
     _check(h, load_library().lsd_set_skin(h, C.c_double(skin)))
+
+
+PROFILE_CLASSES = ["neighbor", "prior", "mlip_dense", "mlip_edge_fwd", "mlip_edge_bwd", "integrator", "transport", "other"]
+
+
+def lsd_profile(h, enable=True):
+    _check(h, load_library().lsd_profile(h, C.c_int32(int(enable))))
+
+
+def lsd_get_profile(h) -> dict:
+    ms, cnt = (C.c_double * 8)(), (C.c_int64 * 8)()
+    _check(h, load_library().lsd_get_profile(h, ms, cnt))
+    return {name: dict(ms=ms[i], launches=cnt[i]) for i, name in enumerate(PROFILE_CLASSES)}
+
+
+def lsd_tc_enabled(h) -> bool:
+    return bool(load_library().lsd_tc_enabled(h))
 
 
 def lsd_launch_count(h) -> int:

@@ -208,16 +208,20 @@ int transport_blocks(int n)
 void launch_half_a(Launcher L, int n, const double* q, const double* p, const double* mass, double hdt,
                    double* qhalf, const double* qref, double skin_half2, int* flags)
 {
+    const int pid = prof_begin(L, PROF_INTEG);
     k_half_a<<<(n + 255) / 256, 256, 0, L.s>>>(n, q, p, mass, hdt, qhalf, qref, skin_half2, flags);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }
 
 void launch_bob_a(Launcher L, int n, uint64_t seed, uint64_t step, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
                   double* q_new, double* p_new)
 {
+    const int pid = prof_begin(L, PROF_INTEG);
     k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, step, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }
 
 void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p)
@@ -230,10 +234,12 @@ void launch_transport(Launcher L, int n, int K, uint64_t seed, uint64_t n0, cons
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
                       double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg)
 {
+    const int pid = prof_begin(L, PROF_TRANSPORT);
     k_transport_partial<<<dim3(nblk, K), kTrThreads, 0, L.s>>>(n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg);
     LSD_COUNT(L);
     k_transport_final<<<1, LSD_MAX_K, 0, L.s>>>(K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }
 
 void launch_commit(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const TransportResult* result,
@@ -241,7 +247,9 @@ void launch_commit(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const T
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
                    double c1, double b, double hdt, double* q_base, double* p_base)
 {
+    const int pid = prof_begin(L, PROF_TRANSPORT);
     k_commit<<<(n + 127) / 128, 128, 0, L.s>>>(n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
                                                c1, b, hdt, q_base, p_base);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }

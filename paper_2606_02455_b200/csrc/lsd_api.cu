@@ -54,6 +54,7 @@ struct lsd_ctx {
     VerletList vl_eval_mlip, vl_eval_pair;
     cudaStream_t side = nullptr;
     int64_t launches = 0;
+    Prof prof;
     lsd_stats stats{};
     std::string err;
 };
@@ -90,7 +91,7 @@ template <typename T> lsd_status upload(lsd_ctx* ctx, T** p, const T* host, size
 }
 #define TRY(expr) do { lsd_status s__ = (expr); if (s__ != LSD_OK) return s__; } while (0)
 
-Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, &ctx->launches}; }
+Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, &ctx->launches, &ctx->prof}; }
 
 lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
 {
@@ -280,6 +281,11 @@ const char* lsd_last_error(const lsd_ctx* ctx) { return ctx ? ctx->err.c_str() :
 
 int64_t lsd_launch_count(const lsd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int32_t lsd_tc_enabled(const lsd_ctx* ctx)
+{
+    return ctx && ctx->cfg.precision == LSD_BF16_TC && ctx->pot[LSD_TARGET].mlip.F > 0 && mlip_tc_supported(ctx->pot[LSD_TARGET].mlip) ? 1 : 0;
+}
+
 void lsd_destroy(lsd_ctx* ctx)
 {
     if (!ctx) return;
@@ -288,6 +294,7 @@ void lsd_destroy(lsd_ctx* ctx)
     cudaFree(ctx->grid.cell_count); cudaFree(ctx->grid.cell_start); cudaFree(ctx->grid.cell_cursor);
     cudaFree(ctx->grid.cell_atoms); cudaFree(ctx->grid.atom_cell);
     for (int s = 0; s < 2; ++s) if (ctx->slot[s].ev_drafted) cudaEventDestroy(ctx->slot[s].ev_drafted);
+    for (cudaEvent_t e : ctx->prof.ev) cudaEventDestroy(e);
     if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->result_host) cudaFreeHost(ctx->result_host);
     delete ctx;
@@ -520,7 +527,13 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
         if (overlap && remaining - k > 0 && ctx->pending == 1)
             TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining - k), ctx->side));   // speculative, second stream
         int32_t l = 0, nc = 0;
-        TRY(lsd_transport_accept(ctx, k, stream, &l, &nc));
+        lsd_status ts = lsd_transport_accept(ctx, k, stream, &l, &nc);
+        if (ts == LSD_ERR_SKIN_VIOLATED || ts == LSD_ERR_NBR_OVERFLOW) {   // answered by a rebuild with a larger skin, never by an incomplete list
+            CK(cudaStreamSynchronize(ctx->side));
+            TRY(lsd_set_skin(ctx, ts == LSD_ERR_SKIN_VIOLATED ? 2.0 * ctx->cfg.skin : ctx->cfg.skin));
+            continue;
+        }
+        TRY(ts);
         TRY(lsd_rollback(ctx, l));
         remaining -= nc;
         if (ctx->pending == 1 && ctx->slot[ctx->verify_idx].K > remaining) {   // cannot happen with the K choice above; defensive
@@ -641,6 +654,50 @@ lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const 
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
     return flags_to_status(ctx, hf);
+}
+
+lsd_status lsd_get_edge_count(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t n_states, int64_t* total)
+{
+    if (!ctx || !total || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
+    const CompactList& cl = kind == 0 ? ctx->cl_mlip[which] : ctx->cl_pair[which];
+    *total = 0;
+    if (!cl.count) return LSD_OK;
+    if (n_states < 1 || n_states > cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "n_states out of range");
+    CK(cudaDeviceSynchronize());
+    std::vector<int> count((size_t)ctx->sys.n * n_states);
+    CK(cudaMemcpy(count.data(), cl.count, sizeof(int) * count.size(), cudaMemcpyDeviceToHost));
+    int64_t t = 0; for (int v : count) t += v;
+    *total = t;
+    return LSD_OK;
+}
+
+lsd_status lsd_profile(lsd_ctx* ctx, int32_t enable)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    Prof& p = ctx->prof;
+    if (enable && p.ev.empty()) {
+        p.ev.resize(2 * 16384); p.cls.resize(16384);
+        for (auto& e : p.ev) CK(cudaEventCreate(&e));
+    }
+    p.on = enable != 0; p.used = 0;
+    for (int c = 0; c < PROF_NCLASS; ++c) { p.ms[c] = 0; p.cnt[c] = 0; }
+    return LSD_OK;
+}
+
+lsd_status lsd_get_profile(lsd_ctx* ctx, double* ms, int64_t* count)
+{
+    if (!ctx || !ms || !count) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    Prof& p = ctx->prof;
+    for (int i = 0; i < p.used; ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, p.ev[2 * i], p.ev[2 * i + 1]));
+        p.ms[p.cls[i]] += t; p.cnt[p.cls[i]]++;
+    }
+    p.used = 0;
+    for (int c = 0; c < PROF_NCLASS; ++c) { ms[c] = p.ms[c]; count[c] = p.cnt[c]; }
+    return LSD_OK;
 }
 
 lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t b, int64_t cap, int64_t* start, int32_t* idx,

@@ -85,11 +85,32 @@ struct MlipWork {                    // activations of one batched evaluation (k
     double* e_atom = nullptr;        // [bmax*n]
 };
 
-struct Launcher {                    // stream + launch counter
+// optional per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline numbers)
+enum ProfClass { PROF_NBR = 0, PROF_PRIOR = 1, PROF_DENSE = 2, PROF_EDGE_FWD = 3, PROF_EDGE_BWD = 4, PROF_INTEG = 5, PROF_TRANSPORT = 6, PROF_NCLASS = 8 };
+struct Prof {
+    bool on = false;
+    std::vector<cudaEvent_t> ev;     // pairs
+    std::vector<int> cls;
+    int used = 0;
+    double ms[PROF_NCLASS] = {0};
+    int64_t cnt[PROF_NCLASS] = {0};
+};
+struct Launcher {                    // stream + launch counter (+ profiler)
     cudaStream_t s;
     int64_t* counter;
+    Prof* prof = nullptr;
 };
 #define LSD_COUNT(L) (++(*(L).counter))
+inline int prof_begin(const Launcher& L, int cls)
+{
+    Prof* p = L.prof;
+    if (!p || !p->on || (size_t)(2 * p->used + 2) > p->ev.size()) return -1;
+    const int id = p->used++;
+    p->cls[id] = cls;
+    cudaEventRecord(p->ev[2 * id], L.s);
+    return id;
+}
+inline void prof_end(const Launcher& L, int id) { if (id >= 0) cudaEventRecord(L.prof->ev[2 * id + 1], L.s); }
 
 // ---- integrator.cu
 void launch_half_a(Launcher L, int n, const double* q, const double* p, const double* mass, double hdt,

@@ -384,17 +384,29 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     for (int c = 0; c < 3; ++c) ea.box[c] = sys.box[c];
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
     for (int t = 0; t < net.T; ++t) {
+        int pid = prof_begin(L, PROF_DENSE);
         k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t]); LSD_COUNT(L);
+        prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
+        pid = prof_begin(L, PROF_EDGE_FWD);
         k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
+        prof_end(L, pid);
+        pid = prof_begin(L, PROF_DENSE);
         k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x); LSD_COUNT(L);
+        prof_end(L, pid);
     }
+    int pidr = prof_begin(L, PROF_DENSE);
     k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
+    prof_end(L, pidr);
     for (int t = net.T - 1; t >= 0; --t) {
+        int pid = prof_begin(L, PROF_DENSE);
         k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar); LSD_COUNT(L);
+        prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
+        pid = prof_begin(L, PROF_EDGE_BWD);
         k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
-        if (t > 0) { k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar); LSD_COUNT(L); }
+        prof_end(L, pid);
+        if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar); LSD_COUNT(L); prof_end(L, pid); }
     }
 }
 

@@ -257,6 +257,7 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
                          double rc_skin, VerletList& vl, int* flags)
 {
     const int n = sys.n;
+    const int pid = prof_begin(L, PROF_NBR);
     GridC gc; gc.nc[0] = g.nc[0]; gc.nc[1] = g.nc[1]; gc.nc[2] = g.nc[2];
     cudaMemsetAsync(g.cell_count, 0, sizeof(int) * g.ncell, L.s);
     k_cell_count<<<(n + 255) / 256, 256, 0, L.s>>>(n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_count); LSD_COUNT(L);
@@ -265,6 +266,7 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
     k_build_verlet<<<(n + kVlWarps - 1) / kVlWarps, kVlWarps * 32, 0, L.s>>>(n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_start,
                                                                              g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }
 
 void launch_compact(Launcher L, const SysDev& sys, int B, const double* q, const int* img, const VerletList& vl,
@@ -272,9 +274,11 @@ void launch_compact(Launcher L, const SysDev& sys, int B, const double* q, const
 {
     const size_t warps = (size_t)sys.n * B;
     const int blocks = (int)((warps * 32 + 255) / 256);
+    const int pid = prof_begin(L, PROF_NBR);
     k_compact<<<blocks, 256, 0, L.s>>>(sys.n, B, make_box(sys), q, img, sys.species, sys.ns, vl.count, vl.keys, vl.cap, rc2_single,
                                        pair_rc2, cl.cap, cl.count, cl.keys, flags);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }
 
 void launch_check_skin(Launcher L, int n, int B, const double* q, const double* qref, double skin_half2, int* flags)

@@ -106,9 +106,11 @@ void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B
     BoxC box; for (int c = 0; c < 3; ++c) box.L[c] = sys.box[c]; box.periodic = sys.periodic;
     const size_t warps = (size_t)sys.n * B;
     const int blocks = (int)((warps * 32 + 255) / 256);
+    const int pid = prof_begin(L, PROF_PRIOR);
     k_prior<<<blocks, 256, 0, L.s>>>(sys.n, B, box, q, img, sys.species, sys.ns, pot.pair, pot.has_tether ? pot.tether : nullptr,
                                      pl ? pl->count : nullptr, pl ? pl->keys : nullptr, pl ? pl->cap : 0,
                                      pot.use_bonded && (sys.n_bonds + sys.n_angles) > 0, sys.bt_start, sys.bt_term, sys.n_bonds, sys.bonds,
                                      sys.bond_k, sys.bond_r0, sys.angles, sys.angle_k, sys.angle_t0, F);
     LSD_COUNT(L);
+    prof_end(L, pid);
 }

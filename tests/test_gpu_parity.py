@@ -36,7 +36,7 @@ def t2_error(Fg, Fo):
     return float((np.linalg.norm(Fg - Fo, axis=1) / np.maximum(nrm, rms)).max())
 
 
-CASES = [("cfg1", {}), ("cfg2", {}), ("cfg3", {"n_grid": 4}), ("cfg4", {"n_atoms": 500}), ("cfg5", {"cells": (4, 4, 3)})]
+CASES = [("cfg1", {}), ("cfg2", {}), ("cfg3", {"n_grid": 7}), ("cfg4", {"n_atoms": 500}), ("cfg5", {"cells": (4, 4, 4)})]
 
 
 def _states(w, B, seed=0, unwrap=True):
@@ -129,7 +129,7 @@ def test_lsd_cfg1_end_to_end_decisions_and_positions(P, orc):
     ctx.close()
 
 
-@pytest.mark.parametrize("name,kw,K", [("cfg2", {}, 16), ("cfg3", {"n_grid": 4}, 4), ("cfg4", {"n_atoms": 500}, 4), ("cfg5", {"cells": (4, 4, 3)}, 4)])
+@pytest.mark.parametrize("name,kw,K", [("cfg2", {}, 16), ("cfg3", {"n_grid": 7}, 4), ("cfg4", {"n_atoms": 500}, 4), ("cfg5", {"cells": (4, 4, 4)}, 4)])
 def test_stagewise_transport_parity(P, orc, name, kw, K):
     """T3: the oracle's transport map is fed the GPU's own F~, F, q_half: S1, S2, ell, decisions, l, n_commit and the
     overridden state must match (decisions bit-for-bit outside the band); one integrator step from a common state
@@ -185,7 +185,7 @@ def test_stagewise_transport_parity(P, orc, name, kw, K):
     ctx.close()
 
 
-@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", {}), ("cfg5", {"cells": (4, 4, 3)})])
+@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", {}), ("cfg5", {"cells": (4, 4, 4)})])
 def test_draft_equals_target_accepts_everything(P, orc, name, kw):
     """draft = target: F~ and F are bit-identical (batch-invariant kernels), S2 == 0, acceptance exactly 1."""
     w = L.with_target_as_draft(L.make_workload(name, **kw))

@@ -13,7 +13,7 @@ def test_every_declared_symbol_is_exported():
     build.build()
     lib = P.load_library()
     header = open(os.path.join(ROOT, "include", "lsd.h")).read()
-    declared = set(re.findall(r"^(?:lsd_status|void|const char\*|int64_t)\s+(lsd_[a-z_]+)\s*\(", header, re.M))
+    declared = set(re.findall(r"^(?:lsd_status|void|const char\*|int64_t|int32_t)\s+(lsd_[a-z_]+)\s*\(", header, re.M))
     assert declared, "no declarations found"
     for name in sorted(declared):
         assert hasattr(lib, name), f"{name} declared in include/lsd.h but not exported"
