@@ -31,11 +31,11 @@ UNIT = "atom-steps/s"
 
 # bounded oracle samples: same per-atom cost as the full workload, sized for ~10-30 s of CPU work
 CPU_SAMPLES = {
-    "cfg1": dict(kw={}, K=4, windows=200),
-    "cfg2": dict(kw={}, K=16, windows=40),
-    "cfg3": dict(kw={"n_grid": 7}, K=2, windows=1),
-    "cfg4": dict(kw={"n_atoms": 1000}, K=2, windows=1),
-    "cfg5": dict(kw={"cells": (6, 6, 6)}, K=2, windows=1),
+    "cfg1": dict(kw={}, K=4, windows=4000),
+    "cfg2": dict(kw={}, K=16, windows=150),
+    "cfg3": dict(kw={"n_grid": 7}, K=4, windows=12),
+    "cfg4": dict(kw={"n_atoms": 1000}, K=4, windows=4),
+    "cfg5": dict(kw={"cells": (6, 6, 6)}, K=4, windows=4),
 }
 
 

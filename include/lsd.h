@@ -195,7 +195,8 @@ lsd_status lsd_get_edge_count(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t
 
 /* Per-kernel-class device timing with CUDA events on the launching stream (used by bench.py for the roofline).
  * Classes: 0 neighbour lists, 1 priors, 2 MLIP atom-wise layers, 3 MLIP edge forward, 4 MLIP edge backward,
- * 5 integrator, 6 transport.  lsd_profile(1) starts (and clears), lsd_profile(0) stops.  lsd_get_profile
+ * 5 integrator, 6 transport, 7 all MLIP kernels of the draft potential (classes 2-4 then hold the target's only).
+ * lsd_profile(1) starts (and clears), lsd_profile(0) stops.  lsd_get_profile
  * synchronises and returns accumulated milliseconds and launch counts, ms[8], count[8]. */
 lsd_status lsd_profile(lsd_ctx* ctx, int32_t enable);
 lsd_status lsd_get_profile(lsd_ctx* ctx, double* ms, int64_t* count);

@@ -234,7 +234,7 @@ def lsd_set_skin(h, skin):
     _check(h, load_library().lsd_set_skin(h, C.c_double(skin)))
 
 
-PROFILE_CLASSES = ["neighbor", "prior", "mlip_dense", "mlip_edge_fwd", "mlip_edge_bwd", "integrator", "transport", "other"]
+PROFILE_CLASSES = ["neighbor", "prior", "mlip_dense", "mlip_edge_fwd", "mlip_edge_bwd", "integrator", "transport", "draft_mlip"]
 
 
 def lsd_profile(h, enable=True):

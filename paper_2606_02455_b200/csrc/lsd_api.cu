@@ -240,6 +240,7 @@ void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, co
                  const VerletList& vp, double* F, int* flags, double* e_atom)
 {
     PotDev& pot = ctx->pot[which];
+    L.draft = which == LSD_DRAFT;
     ctx->cl_img[which] = img;
     CompactList* pl = nullptr;
     if (pot.pair_rcmax > 0) {

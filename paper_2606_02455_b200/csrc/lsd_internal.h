@@ -86,7 +86,7 @@ struct MlipWork {                    // activations of one batched evaluation (k
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline numbers)
-enum ProfClass { PROF_NBR = 0, PROF_PRIOR = 1, PROF_DENSE = 2, PROF_EDGE_FWD = 3, PROF_EDGE_BWD = 4, PROF_INTEG = 5, PROF_TRANSPORT = 6, PROF_NCLASS = 8 };
+enum ProfClass { PROF_NBR = 0, PROF_PRIOR = 1, PROF_DENSE = 2, PROF_EDGE_FWD = 3, PROF_EDGE_BWD = 4, PROF_INTEG = 5, PROF_TRANSPORT = 6, PROF_DRAFT_MLIP = 7, PROF_NCLASS = 8 };
 struct Prof {
     bool on = false;
     std::vector<cudaEvent_t> ev;     // pairs
@@ -99,6 +99,7 @@ struct Launcher {                    // stream + launch counter (+ profiler)
     cudaStream_t s;
     int64_t* counter;
     Prof* prof = nullptr;
+    int draft = 0;                   // 1: kernels of the draft potential (their MLIP launches are timed as one class)
 };
 #define LSD_COUNT(L) (++(*(L).counter))
 inline int prof_begin(const Launcher& L, int cls)
@@ -106,6 +107,7 @@ inline int prof_begin(const Launcher& L, int cls)
     Prof* p = L.prof;
     if (!p || !p->on || (size_t)(2 * p->used + 2) > p->ev.size()) return -1;
     const int id = p->used++;
+    if (L.draft && (cls == PROF_DENSE || cls == PROF_EDGE_FWD || cls == PROF_EDGE_BWD)) cls = PROF_DRAFT_MLIP;
     p->cls[id] = cls;
     cudaEventRecord(p->ev[2 * id], L.s);
     return id;
