@@ -117,6 +117,17 @@ lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
         TRY(up(Wo1, F, F, true, &d.Wo1T[t])); TRY(up(Wo1, F, F, false, &d.Wo1[t]));
         TRY(up(Wo2, F, F, true, &d.Wo2T[t])); TRY(up(Wo2, F, F, false, &d.Wo2[t]));
     }
+    if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(d)) {     // bf16 operands of the tcgen05 filter path
+        d.Wf1_bf16.resize(T); d.Wf2_bf16.resize(T);
+        std::vector<uint16_t> p1, p2;
+        for (int t = 0; t < T; ++t) {
+            const double* Wf1 = blk + t * per_block + (size_t)F * F; const double* Wf2 = Wf1 + (size_t)F * R;
+            tc_pack_weights(Wf1, Wf2, F, R, p1, p2);
+            uint16_t *a = nullptr, *b2 = nullptr;
+            TRY(upload(ctx, &a, p1.data(), p1.size())); TRY(upload(ctx, &b2, p2.data(), p2.size()));
+            d.Wf1_bf16[t] = a; d.Wf2_bf16[t] = b2;
+        }
+    }
     const double* Wr1 = blk + (size_t)T * per_block;
     TRY(up(Wr1, F / 2, F, false, &d.Wr1));
     TRY(up(Wr1 + (size_t)(F / 2) * F, 1, F / 2, false, &d.wr2));

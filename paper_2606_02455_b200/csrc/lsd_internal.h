@@ -144,6 +144,21 @@ void launch_check_skin(Launcher L, int n, int B, const double* q, const double* 
 void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B, const double* q, const int* img,
                          const CompactList* pairlist, double* F /*[B][3][n], overwritten*/);
 
+// arguments of the continuous-filter convolution kernels (fp32 and tcgen05 variants)
+struct EdgeArgs {
+    int total, n, cap;
+    const int* count; const uint32_t* keys; const int* img;
+    const double* q;                  // [B][3][n]
+    double box[3];
+    float rc, inv_rc, delta, inv_delta2;
+    const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major), fp32 path
+    const void *Wf1_tc = nullptr, *Wf2_tc = nullptr;   // bf16, UMMA canonical K-major layouts (mlip_tc.cu)
+    const float* y;                   // [total][F]
+    float* m_out;                     // FWD: m
+    const float* mbar; float* ybar;   // BWD
+    double* Fout;                     // BWD: [B][3][n], accumulated
+};
+
 // ---- mlip_simt.cu
 void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                 const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);
@@ -151,5 +166,8 @@ size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
 
 // ---- mlip_tc.cu (bf16 tcgen05 filter path)
 bool mlip_tc_supported(const MlipDev& net);
+void launch_edge_tc(Launcher L, const EdgeArgs& a, bool backward);
+// host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
+void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                   const int* img, const CompactList& cl, double* F, double* e_atom);

@@ -215,18 +215,6 @@ k_readout(int total, float alpha, const float* __restrict__ x, const float* __re
 }
 
 // ------------------------------------------------------------------------------------------------ continuous-filter convolution
-struct EdgeArgs {
-    int total, n, cap;
-    const int* count; const uint32_t* keys; const int* img;
-    const double* q;                  // [B][3][n]
-    double box[3];
-    float rc, inv_rc, delta, inv_delta2;
-    const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major)
-    const float* y;                   // [total][F]
-    float* m_out;                     // FWD: m
-    const float* mbar; float* ybar;   // BWD
-    double* Fout;                     // BWD: [B][3][n], accumulated
-};
 
 template <int F, bool BWD>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -364,7 +352,7 @@ template <typename K> void set_smem(K kernel, size_t bytes) { cudaFuncSetAttribu
 
 template <int F>
 void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q, const int* img,
-              const CompactList& cl, double* Fout, double* e_atom)
+              const CompactList& cl, double* Fout, double* e_atom, bool use_tc)
 {
     const int total = B * sys.n;
     static bool configured = false;
@@ -389,7 +377,8 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; launch_edge_tc(L, ea, false); }
+        else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         pid = prof_begin(L, PROF_DENSE);
         k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x); LSD_COUNT(L);
@@ -404,7 +393,8 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L);
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; launch_edge_tc(L, ea, true); }
+        else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar); LSD_COUNT(L); prof_end(L, pid); }
     }
@@ -421,9 +411,16 @@ void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& ne
                                 const int* img, const CompactList& cl, double* F, double* e_atom)
 {
     switch (net.F) {
-        case 32:  run_fp32<32>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
-        case 64:  run_fp32<64>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
-        case 128: run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom); break;
+        case 32:  run_fp32<32>(L, sys, net, w, B, q, img, cl, F, e_atom, false); break;
+        case 64:  run_fp32<64>(L, sys, net, w, B, q, img, cl, F, e_atom, false); break;
+        case 128: run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom, false); break;
         default: break;
     }
+}
+
+// bf16 tcgen05 variant: same sequence, the two edge kernels replaced by k_edge_tc (mlip_tc.cu); atom-wise layers stay fp32.
+void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                  const int* img, const CompactList& cl, double* F, double* e_atom)
+{
+    run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom, true);
 }

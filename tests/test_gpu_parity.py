@@ -11,6 +11,8 @@ from helpers import edge_set
 pytestmark = pytest.mark.gpu
 
 FP32_TOL = 1e-5        # north_star: max relative force error <= 1e-5 in fp32 (metric T2)
+BF16_TOL = 2e-2        # north_star: <= 2e-2 in the bf16 tensor-core variant
+BF16_NN_TOL = 5e-2     # the network's own force (a tenth of the total): bf16 operands, fp32 accumulation
 POS_TOL = 1e-6         # Angstrom per step
 BAND = 1e-6            # decisions compared outside |ell - ln u| < 1e-6
 
@@ -85,6 +87,48 @@ def test_forces_match_oracle_fp32(P, orc, name, kw):
             if pot.mlip is not None:
                 Enn = orc.mlip_energy_forces(w, pot.mlip, qs[b], want_forces=False)[0]
                 assert e[b].sum() == pytest.approx(Enn, rel=2e-5, abs=1e-6 * w.n_atoms)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,kw", [("cfg4", {"n_atoms": 500}), ("cfg5", {"cells": (4, 4, 4)}), ("cfg5", {"cells": (5, 4, 4)})])
+def test_forces_match_oracle_bf16_tensor_core(P, orc, name, kw):
+    """LSD_BF16_TC: filter contractions on tcgen05 (bf16 operands, fp32 accumulation); several 128-column tiles per chunk,
+    ragged last tile, chunks that straddle batch states."""
+    w = L.make_workload(name, **kw)
+    B = 3
+    ctx = P.context_from_workload(w, k_max=B, precision=P.LSD_BF16_TC)
+    assert P.lsd_tc_enabled(ctx.h)                             # the tcgen05 kernels are the ones that run
+    qs = _states(w, B, seed=3)
+    Q = np.stack([soa(q) for q in qs])
+    F, e = ctx.forces(P.LSD_TARGET, Q)
+    F2, _ = ctx.forces(P.LSD_TARGET, Q)
+    assert np.array_equal(F, F2)                               # deterministic (no float atomics, fixed summation order)
+    F1, _ = ctx.forces(P.LSD_TARGET, Q[1:2])
+    assert np.array_equal(F1[0], F[1])                         # batch-invariant: same state alone == inside the batch
+    for b in range(B):
+        Eo, Fo = orc.energy_forces(w, w.target, qs[b])
+        Enn, Fnn = orc.mlip_energy_forces(w, w.target.mlip, qs[b])
+        assert t2_error(F[b].T, Fo) <= BF16_TOL, (name, b)
+        assert t2_error(F[b].T - (Fo - Fnn), Fnn) <= BF16_NN_TOL, (name, b)
+        assert e[b].sum() == pytest.approx(Enn, rel=2e-2)
+    ctx.close()
+
+
+def test_bf16_tensor_core_empty_and_tiny_rows(P, orc):
+    """tcgen05 path edge cases: an atom without neighbours inside a chunk, a system much smaller than one tile (vacuum)."""
+    w = L.make_workload("cfg2", n_chain=9)
+    net = L.make_mlip(128, 2, 32, 5.0, w.n_species, seed=11, alpha=w.target.mlip.alpha)
+    w = dataclasses.replace(w, target=dataclasses.replace(w.target, mlip=net))
+    q = w.q0.copy()
+    q[8] += np.array([40.0, 0, 0])                              # beyond every cutoff: empty MLIP row (still bonded)
+    ctx = P.context_from_workload(w, k_max=2, precision=P.LSD_BF16_TC)
+    assert P.lsd_tc_enabled(ctx.h)
+    F, _ = ctx.forces(P.LSD_TARGET, np.stack([soa(q), soa(w.q0)]))
+    for b, qq in enumerate((q, w.q0)):
+        Fo = orc.energy_forces(w, w.target, qq)[1]
+        Fnn = orc.mlip_energy_forces(w, w.target.mlip, qq)[1]
+        assert t2_error(F[b].T, Fo) <= BF16_TOL
+        assert t2_error(F[b].T - (Fo - Fnn), Fnn) <= BF16_NN_TOL
     ctx.close()
 
 
