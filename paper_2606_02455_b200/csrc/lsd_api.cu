@@ -163,11 +163,12 @@ lsd_status alloc_verlet(lsd_ctx* ctx, VerletList& vl, int cap, double rc)
     TRY(dalloc(ctx, &vl.keys, (size_t)ctx->sys.n * cap));
     return LSD_OK;
 }
-lsd_status alloc_compact(lsd_ctx* ctx, CompactList& cl, int cap, int bmax)
+lsd_status alloc_compact(lsd_ctx* ctx, CompactList& cl, int cap, int bmax, bool records)
 {
     cl.cap = cap; cl.bmax = bmax;
     TRY(dalloc(ctx, &cl.count, (size_t)ctx->sys.n * bmax));
     TRY(dalloc(ctx, &cl.keys, (size_t)ctx->sys.n * bmax * cap));
+    if (records) TRY(dalloc(ctx, &cl.recs, (size_t)ctx->sys.n * bmax * cap));
     return LSD_OK;
 }
 lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
@@ -178,6 +179,11 @@ lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
     w.y.resize(net.T); w.h.resize(net.T);
     for (int t = 0; t < net.T; ++t) { TRY(dalloc(ctx, &w.y[t], e)); TRY(dalloc(ctx, &w.h[t], e)); }
     TRY(dalloc(ctx, &w.e_atom, rows));
+    if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(net)) {
+        w.y16.resize(net.T);
+        for (int t = 0; t < net.T; ++t) TRY(dalloc(ctx, &w.y16[t], e));
+        TRY(dalloc(ctx, &w.mbar16, e));
+    }
     return LSD_OK;
 }
 
@@ -226,8 +232,8 @@ lsd_status setup_lists(lsd_ctx* ctx)
     if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->vl_eval_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
     if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->vl_eval_pair, ctx->cap_pair, ctx->rc_pair_max));
     for (int w = 0; w < 2; ++w) {
-        if (ctx->pot[w].mlip.F > 0) TRY(alloc_compact(ctx, ctx->cl_mlip[w], ctx->cap_mlip, ctx->bmax[w]));
-        if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w]));
+        if (ctx->pot[w].mlip.F > 0) TRY(alloc_compact(ctx, ctx->cl_mlip[w], ctx->cap_mlip, ctx->bmax[w], true));
+        if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w], false));
     }
     return LSD_OK;
 }
@@ -261,7 +267,7 @@ void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, co
     launch_prior_forces(L, ctx->sys, pot, B, q, img, pl, F);
     if (pot.mlip.F > 0) {
         const double rc = (double)pot.mlip.rc;
-        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags);
+        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
         if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(pot.mlip))
             mlip_forward_backward_bf16tc(L, ctx->sys, pot.mlip, ctx->work[which], B, q, img, ctx->cl_mlip[which], F, e_atom);
         else

@@ -61,10 +61,15 @@ struct VerletList {                  // window-shared candidate list (r < rc + s
     uint32_t* keys = nullptr;        // [n][cap]  key = (j << 5) | shiftcode, sorted ascending
 };
 
+// geometry of one directed edge i <- j of one state, written once per batched evaluation by k_compact and read by
+// every block's forward and backward edge kernel: r = |q_j - q_i + s L|, unit vector, cosine cutoff (M2) and its slope
+struct __align__(16) EdgeRec { float r, fc, fcp, ux, uy, uz; int jrow, pad; };   // jrow = b*n + j (row of the gathered features)
+
 struct CompactList {                 // per-state exact list (r < rc), rows padded with 0xFFFFFFFF
     int cap = 0, bmax = 0;
     int* count = nullptr;            // [bmax*n]
     uint32_t* keys = nullptr;        // [bmax*n][cap]
+    EdgeRec* recs = nullptr;         // [bmax*n][cap], MLIP lists only
 };
 
 struct CellGrid {
@@ -82,6 +87,8 @@ struct MlipWork {                    // activations of one batched evaluation (k
     int bmax = 0;
     float *x = nullptr, *m = nullptr, *mbar = nullptr, *xbar = nullptr, *ybar = nullptr;
     std::vector<float*> y, h;        // [T] each [bmax*n][F]
+    std::vector<uint16_t*> y16;      // [T] bf16 copies of y gathered by the tcgen05 edge kernels (LSD_BF16_TC only)
+    uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
     double* e_atom = nullptr;        // [bmax*n]
 };
 
@@ -137,7 +144,8 @@ void launch_pack_ref(Launcher L, const SysDev& sys, const double* qref, int* img
 void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const double* qref, const int* img,
                          double rc_skin, VerletList& vl, int* flags);
 void launch_compact(Launcher L, const SysDev& sys, int B, const double* q /*[B][3][n]*/, const int* img,
-                    const VerletList& vl, double rc2_single, const double* pair_rc2 /*or null*/, CompactList& cl, int* flags);
+                    const VerletList& vl, double rc2_single, const double* pair_rc2 /*or null*/, CompactList& cl, int* flags,
+                    float rc_records = 0.f /* > 0: also write cl.recs with the cutoff function of this radius */);
 void launch_check_skin(Launcher L, int n, int B, const double* q, const double* qref, double skin_half2, int* flags);
 
 // ---- prior.cu
@@ -147,13 +155,12 @@ void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B
 // arguments of the continuous-filter convolution kernels (fp32 and tcgen05 variants)
 struct EdgeArgs {
     int total, n, cap;
-    const int* count; const uint32_t* keys; const int* img;
-    const double* q;                  // [B][3][n]
-    double box[3];
+    const int* count; const uint32_t* keys; const EdgeRec* recs;
     float rc, inv_rc, delta, inv_delta2;
     const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major), fp32 path
     const void *Wf1_tc = nullptr, *Wf2_tc = nullptr;   // bf16, UMMA canonical K-major layouts (mlip_tc.cu)
     const float* y;                   // [total][F]
+    const uint16_t *y16 = nullptr, *mbar16 = nullptr;   // bf16 rows gathered by the tcgen05 kernels
     float* m_out;                     // FWD: m
     const float* mbar; float* ybar;   // BWD
     double* Fout;                     // BWD: [B][3][n], accumulated

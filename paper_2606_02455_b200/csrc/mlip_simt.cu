@@ -11,6 +11,7 @@
 //   backward block t:  hbar = logistic(h) . (W_o2^T xbar) ;  mbar = W_o1^T hbar ;
 //                      ybar_a = sum_j mbar_j . w_aj ;
 //                      F_a   += sum_j [ sum_f (mbar_a y_j + mbar_j y_a)_f w'_aj,f ] rhat_aj ;   xbar += W_in^T ybar
+#include <cuda_bf16.h>
 #include <algorithm>
 #include "lsd_internal.h"
 
@@ -22,7 +23,6 @@ constexpr float kLn2 = 0.69314718055994530942f;
 
 __device__ __forceinline__ float ssp(float x) { return fmaxf(x, 0.f) + log1pf(expf(-fabsf(x))) - kLn2; }          // M3
 __device__ __forceinline__ float logistic(float x) { return 1.f / (1.f + expf(-x)); }
-__device__ __forceinline__ void img_unpack(int v, int& ix, int& iy, int& iz) { ix = (v & 1023) - 512; iy = ((v >> 10) & 1023) - 512; iz = ((v >> 20) & 1023) - 512; }
 
 template <int CPT> struct Vec;
 template <> struct Vec<4> { using T = float4; };
@@ -44,6 +44,12 @@ template <int CPT> __device__ __forceinline__ void stv(float* p, const float (&v
     for (int c = 0; c < CPT; ++c) f[c] = v[c];
     *reinterpret_cast<typename Vec<CPT>::T*>(p) = t;
 }
+
+// bf16 (round to nearest even) copy of a lane's channels
+__device__ __forceinline__ uint32_t bf16x2(float lo, float hi) { const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi); return *reinterpret_cast<const uint32_t*>(&v); }
+__device__ __forceinline__ void st16(uint16_t* p, const float (&v)[4]) { *reinterpret_cast<uint2*>(p) = make_uint2(bf16x2(v[0], v[1]), bf16x2(v[2], v[3])); }
+__device__ __forceinline__ void st16(uint16_t* p, const float (&v)[2]) { *reinterpret_cast<uint32_t*>(p) = bf16x2(v[0], v[1]); }
+__device__ __forceinline__ void st16(uint16_t* p, const float (&v)[1]) { const __nv_bfloat16 h = __float2bfloat16_rn(v[0]); *p = *reinterpret_cast<const uint16_t*>(&h); }
 
 // acc[8][CPT] = A[8][KD] (shared, row-major, leading dimension lda) * W[KD][F] (shared); lane owns channels lane*CPT..
 template <int KD, int F>
@@ -97,7 +103,7 @@ enum DenseMode { DENSE_IN = 0, DENSE_OUT = 1, BWD_OUT = 2, BWD_IN = 3 };
 template <int F, int MODE>
 __global__ void __launch_bounds__(kThreads, 1)
 k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, const float* __restrict__ W1,
-        float* __restrict__ aux, float* __restrict__ out)
+        float* __restrict__ aux, float* __restrict__ out, uint16_t* __restrict__ out16)
 {
     constexpr int CPT = F / 32, LDA = F + 4;
     constexpr bool TWO = (MODE == DENSE_OUT || MODE == BWD_OUT);
@@ -125,7 +131,10 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
         warp_gemm8<F, F>(Asw, LDA, Ws0, lane, acc);
         if (MODE == DENSE_IN) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r) if (g0 + r < total) stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc[r]);
+            for (int r = 0; r < 8; ++r) if (g0 + r < total) {
+                stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc[r]);
+                if (out16) st16(out16 + (size_t)(g0 + r) * F + lane * CPT, acc[r]);
+            }
         } else if (MODE == BWD_IN) {
 #pragma unroll
             for (int r = 0; r < 8; ++r) if (g0 + r < total) {
@@ -167,6 +176,7 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
                     stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, v);
                 } else {
                     stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
+                    if (out16) st16(out16 + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
                 }
             }
         }
@@ -233,37 +243,23 @@ k_edge(EdgeArgs a)
     const int n = a.n;
     for (int g = blockIdx.x * kWarps + warp; g < a.total; g += gridDim.x * kWarps) {
         const int b = g / n, i = g % n;
-        const double* qb = a.q + (size_t)b * 3 * n;
         const int cnt = a.count[g];
-        const uint32_t* row = a.keys + (size_t)g * a.cap;
-        const double qi0 = qb[i], qi1 = qb[n + i], qi2 = qb[2 * n + i];
-        int iix, iiy, iiz; img_unpack(a.img[i], iix, iiy, iiz);
+        const EdgeRec* row = a.recs + (size_t)g * a.cap;
         float part[CPT], ya[CPT], mba[CPT];
 #pragma unroll
         for (int c = 0; c < CPT; ++c) part[c] = 0.f;
         if (BWD) { ldv<CPT>(a.y + (size_t)g * F + lane * CPT, ya); ldv<CPT>(a.mbar + (size_t)g * F + lane * CPT, mba); }
         double fx = 0.0, fy = 0.0, fz = 0.0;
         for (int u0 = 0; u0 < cnt; u0 += SPW) {
-            // --- geometry of the unit's slots (lanes 0..SPW-1), fp64 displacement -> fp32
+            // --- geometry of the unit's slots (lanes 0..SPW-1): edge records written by k_compact (fp64 -> fp32 once)
             const int slot = u0 + lane;
             const bool valid = lane < SPW && slot < cnt;
             float r = 0.f, fc = 0.f, fcp = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
             int jrow = g;
             if (valid) {
-                const uint32_t key = row[slot];
-                const int j = (int)(key >> 5), code = (int)(key & 31u);
-                int jx, jy, jz; img_unpack(a.img[j], jx, jy, jz);
-                const double d0 = (qb[j] - qi0) + (double)(code / 9 - 1 + iix - jx) * a.box[0];
-                const double d1 = (qb[n + j] - qi1) + (double)((code / 3) % 3 - 1 + iiy - jy) * a.box[1];
-                const double d2 = (qb[2 * n + j] - qi2) + (double)(code % 3 - 1 + iiz - jz) * a.box[2];
-                const double rd = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-                r = (float)rd; ux = (float)(d0 / rd); uy = (float)(d1 / rd); uz = (float)(d2 / rd);
-                const float t = r * a.inv_rc;
-                if (t < 1.f) {                                                            // M2
-                    float sn, cs; sincospif(t, &sn, &cs);
-                    fc = 0.5f * (cs + 1.f); fcp = -0.5f * 3.14159265358979323846f * a.inv_rc * sn;
-                }
-                jrow = b * n + j;
+                const float4 e0 = *reinterpret_cast<const float4*>(row + slot);
+                const float4 e1 = *(reinterpret_cast<const float4*>(row + slot) + 1);
+                r = e0.x; fc = e0.y; fcp = e0.z; ux = e0.w; uy = e1.x; uz = e1.y; jrow = __float_as_int(e1.z);
             }
             // --- radial basis rows (M1): lane k holds basis k; BWD interleaves value / r-derivative rows
 #pragma unroll
@@ -368,20 +364,19 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
     k_embed<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, w.x); LSD_COUNT(L);
     EdgeArgs ea{};
-    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.img = img; ea.q = q;
-    for (int c = 0; c < 3; ++c) ea.box[c] = sys.box[c];
+    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs;
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
     for (int t = 0; t < net.T; ++t) {
         int pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t]); LSD_COUNT(L);
+        k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t], use_tc ? w.y16[t] : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; launch_edge_tc(L, ea, false); }
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; launch_edge_tc(L, ea, false); }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x); LSD_COUNT(L);
+        k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x, nullptr); LSD_COUNT(L);
         prof_end(L, pid);
     }
     int pidr = prof_begin(L, PROF_DENSE);
@@ -389,14 +384,14 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     prof_end(L, pidr);
     for (int t = net.T - 1; t >= 0; --t) {
         int pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar); LSD_COUNT(L);
+        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc ? w.mbar16 : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; launch_edge_tc(L, ea, true); }
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; launch_edge_tc(L, ea, true); }
         else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
-        if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar); LSD_COUNT(L); prof_end(L, pid); }
+        if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar, nullptr); LSD_COUNT(L); prof_end(L, pid); }
     }
 }
 

@@ -1,21 +1,24 @@
 // bf16 tcgen05 filter path (LSD_BF16_TC): the continuous-filter convolution of the SchNet-style MLIP (M5, M9)
 // with the two per-edge filter contractions on the 5th-generation tensor cores (sm_100a), fp32 accumulation in TMEM.
 //
-// Orientation ("channels are rows"): for one tile of NT edges
+// Orientation ("channels are rows"): for one tile of edges
 //     D1[F x N] = W_f1[F x R] * G^T[R x N]          G   = radial basis rows (and, backward, their r-derivatives)
 //     D2[F x N] = W_f2[F x F] * A^T[F x N]          A   = ssp(D1) (and, backward, logistic(D1) . D1')
 // so TMEM lane = channel f = thread, TMEM column = edge.  The per-atom sums over edges (m_a, ybar_a, F_a) are then
 // serial sums inside one thread in the order of the atom's sorted neighbour row (deterministic, independent of the
-// batch and of the tiling), and the gathers y_j[f], mbar_j[f] are coalesced 128-byte rows per warp.
+// batch and of the tiling), and every per-channel operand of the epilogue is read from shared memory.
 //
 // One persistent CTA per SM, 4 teams of 128 threads.  The weights (A operands, K-major canonical no-swizzle layout,
-// packed on the host) are resident in shared memory and shared by the teams; each team owns 128 TMEM columns, one
-// B-operand buffer, and walks chunks of kCH consecutive atoms in tiles of 128 MMA columns
-// (forward: 128 edges; backward: 64 edges = 64 value + 64 tangent columns).  Per tile and team:
-//     geometry + radial basis -> smem (B1, K-major)      | MMA1 (2 x K16)  -> TMEM
+// packed on the host) are resident in shared memory and shared by the teams; each team owns 64 TMEM columns, one
+// B-operand buffer and one gather stage, and walks chunks of 64 consecutive atoms of one state.  An atom's row is
+// cut into groups of 16 edge slots (the last one padded with zero records), so a group never straddles two atoms;
+// a tile is 4 groups (forward: 64 edges) or 2 groups (backward: 32 value + 32 tangent columns).  Per tile and team:
+//     cp.async: edge records of the NEXT tile, bf16 feature rows y_j (mbar_j) of THIS tile  -> smem (lands under the MMAs)
+//     radial basis -> smem (B1, K-major)                 | MMA1 (2 x K16)  -> TMEM
 //     TMEM -> activation -> smem (B2, MN-major, bf16)    | MMA2 (8 x K16)  -> TMEM (same columns)
-//     TMEM -> cutoff, cfconv products, gathers, per-atom accumulation in registers.
-// The phases of different teams overlap (MUFU-bound activation of one team with the LSU/FMA-bound epilogue of another).
+//     TMEM -> cutoff, cfconv products and adjoints, per-atom accumulation in registers.
+// The phases of different teams overlap (MUFU-bound activation of one team with the FMA/LSU-bound epilogue of another,
+// both with the tensor pipe).  Edge geometry comes from the records k_compact wrote once per batched evaluation.
 #include <cuda_bf16.h>
 #include <algorithm>
 #include "lsd_internal.h"
@@ -27,15 +30,22 @@ constexpr int kR = LSD_NRBF;            // 32 = K of the first contraction
 constexpr int kTeams = 4;
 constexpr int kTT = 128;                // threads per team
 constexpr int kThreadsTC = kTeams * kTT;
-constexpr int kNCOL = 128;              // MMA N per tile and team
+constexpr int kNCOL = 64;               // MMA N = TMEM columns per team
 constexpr int kCH = 64;                 // atoms per chunk
-constexpr int kW1Bytes = kF * kR * 2;   // 8 KB
-constexpr int kW2Bytes = kF * kF * 2;   // 32 KB
-constexpr int kB2Bytes = kNCOL * kF * 2;  // 32 KB (B1 aliases its first 8 KB)
-constexpr int kEsBytes = 2048;          // per-edge scalars: 64 x 32 B (backward) or 128 x 16 B (forward)
-constexpr int kPrefBytes = 272;         // (kCH + 1) ints, padded
+constexpr int kGE = 16;                 // edge slots per group
+constexpr int kMaxGroups = kCH * (512 / kGE);   // rows hold at most 512 slots (neighbor.cu)
+
+constexpr int kW1Bytes = kF * kR * 2;           // 8 KB
+constexpr int kW2Bytes = kF * kF * 2;           // 32 KB
+constexpr int kB2Bytes = kNCOL * kF * 2;        // 16 KB (B1 aliases its first 4 KB)
+constexpr int kStageBytes = kNCOL * kF * 2;     // 16 KB: forward 64 rows of y_j; backward 32 rows of y_j + 32 rows of mbar_j
+constexpr int kOwnBytes = 2 * 2 * kF * 2;       // backward: (y_a, mbar_a) of the tile's two groups
+constexpr int kRecBytes = 2 * kNCOL * 32;       // double-buffered edge records
+constexpr int kScalBytes = 5 * kNCOL * 4;       // fc, fcp, ux, uy, uz per tile edge
+constexpr int kPrefBytes = 272;                 // (kCH + 1) ints, padded
+constexpr int kCntBytes = kCH * 4;
 constexpr int kFpartBytes = kCH * 4 * 3 * 4;
-constexpr int kTeamBytes = kB2Bytes + kEsBytes + kPrefBytes + kFpartBytes;
+constexpr int kTeamBytes = kB2Bytes + kStageBytes + kOwnBytes + kRecBytes + kScalBytes + kPrefBytes + kCntBytes + kMaxGroups + kFpartBytes;
 constexpr int kSmemTC = kW1Bytes + kW2Bytes + kTeams * kTeamBytes;
 static_assert(kSmemTC <= 227 * 1024, "shared memory budget");
 static_assert(kTeamBytes % 16 == 0, "team regions stay 16-byte aligned");
@@ -43,19 +53,16 @@ static_assert(kTeamBytes % 16 == 0, "team regions stay 16-byte aligned");
 constexpr float kLn2 = 0.69314718055994530942f;
 constexpr float kLog2e = 1.44269504088896340736f;
 
-struct __align__(16) EdgeB { float fc, fcp, ux, uy, uz; int jrow, arow, pad; };   // backward, 32 B
-struct __align__(16) EdgeF { float fc; int jrow, arow, pad; };                    // forward, 16 B
-
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ float ex2f(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2f(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float rcpf(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float tanhf_approx(float x) { float y; asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
     __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&v);
 }
-__device__ __forceinline__ void img_unpack(int v, int& ix, int& iy, int& iz) { ix = (v & 1023) - 512; iy = ((v >> 10) & 1023) - 512; iz = ((v >> 20) & 1023) - 512; }
+__device__ __forceinline__ float bf16_ld(const uint8_t* p) { return __uint_as_float((uint32_t)(*reinterpret_cast<const uint16_t*>(p)) << 16); }
 
 // shared-memory matrix descriptor, canonical layout without swizzle (8 x 16-byte core matrices):
 // start address, leading-dimension byte offset, stride-dimension byte offset (all >> 4), descriptor version 1.
@@ -105,46 +112,23 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
                    "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
                  : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                 : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// geometry of one directed edge (slot of atom row g), identical arithmetic to the fp32 kernel: fp64 displacement -> fp32
-struct EdgeGeom { float r, fc, fcp, ux, uy, uz; int jrow; };
-__device__ __forceinline__ EdgeGeom edge_geometry(const EdgeArgs& a, int g, int slot)
+// 16-byte asynchronous copy global -> shared, L2 only; src_bytes = 0 writes zeros (padding slots)
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes)
 {
-    const int n = a.n, b = g / n, i = g - b * n;
-    const double* qb = a.q + (size_t)b * 3 * n;
-    const uint32_t key = a.keys[(size_t)g * a.cap + slot];
-    const int j = (int)(key >> 5), code = (int)(key & 31u);
-    int iix, iiy, iiz, jx, jy, jz;
-    img_unpack(a.img[i], iix, iiy, iiz);
-    img_unpack(a.img[j], jx, jy, jz);
-    const double d0 = (qb[j] - qb[i]) + (double)(code / 9 - 1 + iix - jx) * a.box[0];
-    const double d1 = (qb[n + j] - qb[n + i]) + (double)((code / 3) % 3 - 1 + iiy - jy) * a.box[1];
-    const double d2 = (qb[2 * n + j] - qb[2 * n + i]) + (double)(code % 3 - 1 + iiz - jz) * a.box[2];
-    const double rd = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-    EdgeGeom o;
-    o.r = (float)rd; o.ux = (float)(d0 / rd); o.uy = (float)(d1 / rd); o.uz = (float)(d2 / rd);
-    o.fc = 0.f; o.fcp = 0.f;
-    const float t = o.r * a.inv_rc;
-    if (t < 1.f) {                                                                        // M2
-        float sn, cs; sincospif(t, &sn, &cs);
-        o.fc = 0.5f * (cs + 1.f); o.fcp = -0.5f * 3.14159265358979323846f * a.inv_rc * sn;
-    }
-    o.jrow = b * n + j;
-    return o;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <bool BWD>
 __global__ void __launch_bounds__(kThreadsTC, 1)
-k_edge_tc(EdgeArgs a, int nchunks)
+k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
 {
-    constexpr int NT = BWD ? 64 : 128;                 // edges per tile
+    constexpr int GPT = BWD ? 2 : 4;                   // groups per tile
+    constexpr int NT = GPT * kGE;                      // edges per tile
+    constexpr int TPE = kTT / NT;                      // threads per edge in the staging phase (2 forward, 4 backward)
+    constexpr int KPT = kR / TPE;                      // radial basis functions per staging thread (16 / 8)
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[kTeams];
     __shared__ uint32_t tmem_base_s;
@@ -165,7 +149,7 @@ k_edge_tc(EdgeArgs a, int nchunks)
         next_chunk = 0;
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(256));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     fence_async_smem();
@@ -174,79 +158,132 @@ k_edge_tc(EdgeArgs a, int nchunks)
     tc_fence_after();
 
     uint8_t* const tb = smem + kW1Bytes + kW2Bytes + team * kTeamBytes;
-    uint8_t* const Bop = tb;                                           // B2 [128 cols][128 k] MN-major; B1 aliases its head
-    EdgeB* const esb = reinterpret_cast<EdgeB*>(tb + kB2Bytes);
-    EdgeF* const esf = reinterpret_cast<EdgeF*>(tb + kB2Bytes);
-    int* const pref = reinterpret_cast<int*>(tb + kB2Bytes + kEsBytes);
-    float* const fpart = reinterpret_cast<float*>(tb + kB2Bytes + kEsBytes + kPrefBytes);
+    uint8_t* const Bop = tb;                                           // B2 [64 cols][128 k] MN-major; B1 aliases its head
+    uint8_t* const stage = Bop + kB2Bytes;
+    uint8_t* const own = stage + kStageBytes;
+    uint8_t* const recs = own + kOwnBytes;                             // [2][NT] EdgeRec
+    float* const scal = reinterpret_cast<float*>(recs + kRecBytes);    // [5][kNCOL]
+    int* const pref = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(scal) + kScalBytes);   // first group of every atom of the chunk
+    int* const cnts = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(pref) + kPrefBytes);
+    uint8_t* const gatom = reinterpret_cast<uint8_t*>(cnts) + kCntBytes;                        // group -> atom of the chunk
+    float* const fpart = reinterpret_cast<float*>(gatom + kMaxGroups);
     const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + kW1Bytes), sB = smem_u32(Bop), bar = smem_u32(&mbar[team]);
+    const uint32_t sStage = smem_u32(stage), sOwn = smem_u32(own), sRecs = smem_u32(recs);
     const uint32_t tmem = tmem_base_s + (uint32_t)(team * kNCOL);
     const uint32_t tlane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t idesc1 = make_idesc(kF, kNCOL, 0), idesc2 = make_idesc(kF, kNCOL, 1);
     uint32_t phase = 0;
     const int n = a.n;
+    const int se = tt / TPE, sp = tt % TPE;            // staging role: edge of the tile, part of its row
+    const float c2 = -0.5f * kLog2e * a.inv_delta2;
 
     for (;;) {
         if (tt == 0) s_chunk[team] = atomicAdd(&next_chunk, 1);
         team_bar(team);
         const int chunk = blockIdx.x + s_chunk[team] * gridDim.x;
         if (chunk >= nchunks) break;
-        const int g0 = chunk * kCH;
-        if (tt < kCH) pref[tt + 1] = (g0 + tt < a.total) ? a.count[g0 + tt] : 0;
+        const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
+        const int g0 = b * n + ci * kCH;                               // first feature row of the chunk
+        const int natoms = min(kCH, n - ci * kCH);
+        if (tt < kCH) { const int c = tt < natoms ? a.count[g0 + tt] : 0; cnts[tt] = c; pref[tt + 1] = (c + kGE - 1) / kGE; }
         team_bar(team);
         if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= kCH; ++i) { s += pref[i]; pref[i] = s; } }
         team_bar(team);
-        const int E = pref[kCH];
+        const int G = pref[kCH];
+        if (tt < kCH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
         {   // atoms without neighbours: their sums are empty
             float* out = BWD ? a.ybar : a.m_out;
-            if (out) for (int i = 0; i < kCH; ++i) if (g0 + i < a.total && pref[i + 1] == pref[i]) out[(size_t)(g0 + i) * kF + tt] = 0.f;
+            if (out) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * kF + tt] = 0.f;
         }
+        team_bar(team);
+
+        // asynchronous copy of the edge records of tile t into buffer t & 1 (zero records for padding slots)
+        auto fetch_records = [&](int t) {
+            for (int idx = tt; idx < NT * 2; idx += kTT) {
+                const int e = idx >> 1, half = idx & 1;
+                const int gi = t * GPT + e / kGE;
+                const EdgeRec* src = a.recs;
+                uint32_t bytes = 0;
+                if (gi < G) {
+                    const int at = gatom[gi];
+                    const int slot = (gi - pref[at]) * kGE + (e & (kGE - 1));
+                    if (slot < cnts[at]) { src = a.recs + (size_t)(g0 + at) * a.cap + slot; bytes = 16; }
+                }
+                cp_async16(sRecs + (uint32_t)(((t & 1) * NT + e) * 32 + half * 16), reinterpret_cast<const uint8_t*>(src) + half * 16, bytes);
+            }
+        };
+        const int ntiles = (G + GPT - 1) / GPT;
+        if (ntiles > 0) fetch_records(0);
+        cp_async_commit();
+
         int cur = -1;
         float part = 0.f, ya = 0.f, mba = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
         auto flush = [&]() {
             if (cur < 0) return;
-            if (!BWD) a.m_out[(size_t)cur * kF + tt] = part;
+            if (!BWD) a.m_out[(size_t)(g0 + cur) * kF + tt] = part;
             else {
-                if (a.ybar) a.ybar[(size_t)cur * kF + tt] = part;
+                if (a.ybar) a.ybar[(size_t)(g0 + cur) * kF + tt] = part;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
                     fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
                 }
-                if (lane == 0) { float* fp = fpart + ((cur - g0) * 4 + (warp & 3)) * 3; fp[0] = fx; fp[1] = fy; fp[2] = fz; }
+                if (lane == 0) { float* fp = fpart + (cur * 4 + (warp & 3)) * 3; fp[0] = fx; fp[1] = fy; fp[2] = fz; }
             }
         };
 
-        for (int base = 0; base < E; base += NT) {
-            // ---- phase 1: geometry and radial basis rows (M1) -> B1, K-major: (n, k) at (n/8)*512 + (k/8)*128 + (n%8)*16 + (k%8)*2
+        for (int t = 0; t < ntiles; ++t) {
+            // ---- phase 1: records of this tile are in shared memory; start the gathers, build the radial basis operand
+            cp_async_wait_all();
+            team_bar(team);                                            // also: everybody is done with the previous tile's buffers
+            if (t + 1 < ntiles) fetch_records(t + 1);
+            const uint8_t* rec = recs + ((t & 1) * NT + se) * 32;
+            const float4 r0 = *reinterpret_cast<const float4*>(rec);   // r, fc, fcp, ux
+            const float4 r1 = *reinterpret_cast<const float4*>(rec + 16);   // uy, uz, jrow, pad
             {
-                const int col = BWD ? (tt & 63) : tt;
-                const bool tang = BWD && tt >= 64;
-                const int e = base + col;
-                uint32_t gp[16];
+                const int jrow = __float_as_int(r1.z);
+                if (!BWD) {                                            // y_j: 16 chunks of 16 B, two threads per edge
+                    const uint8_t* src = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (kF * 2);
 #pragma unroll
-                for (int k = 0; k < 16; ++k) gp[k] = 0u;
-                if (e < E) {
-                    int lo = 0, hi = kCH;
-                    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (pref[mid] <= e) lo = mid; else hi = mid; }
-                    const int g = g0 + lo;
-                    const EdgeGeom ge = edge_geometry(a, g, e - pref[lo]);
-                    if (!tang) {
-                        if (BWD) { EdgeB s; s.fc = ge.fc; s.fcp = ge.fcp; s.ux = ge.ux; s.uy = ge.uy; s.uz = ge.uz; s.jrow = ge.jrow; s.arow = g; s.pad = 0; esb[col] = s; }
-                        else { EdgeF s; s.fc = ge.fc; s.jrow = ge.jrow; s.arow = g; s.pad = 0; esf[col] = s; }
+                    for (int i = 0; i < 8; ++i) cp_async16(sStage + (uint32_t)(se * 256 + (2 * i + sp) * 16), src + (2 * i + sp) * 16, 16);
+                } else {                                               // y_j and mbar_j, four threads per edge
+                    const uint8_t* sy = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (kF * 2);
+                    const uint8_t* sm = reinterpret_cast<const uint8_t*>(a.mbar16) + (size_t)jrow * (kF * 2);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        cp_async16(sStage + (uint32_t)(se * 256 + (4 * i + sp) * 16), sy + (4 * i + sp) * 16, 16);
+                        cp_async16(sStage + (uint32_t)((NT + se) * 256 + (4 * i + sp) * 16), sm + (4 * i + sp) * 16, 16);
                     }
-                    const float c2 = -0.5f * kLog2e * a.inv_delta2;
-#pragma unroll
-                    for (int k = 0; k < kR; k += 2) {
-                        const float x0 = ge.r - (float)k * a.delta, x1 = ge.r - (float)(k + 1) * a.delta;
-                        float v0 = ex2f(c2 * x0 * x0), v1 = ex2f(c2 * x1 * x1);
-                        if (tang) { v0 = -v0 * x0 * a.inv_delta2; v1 = -v1 * x1 * a.inv_delta2; }
-                        gp[k >> 1] = pack_bf16(v0, v1);
+                    if (tt < 64) {                                     // the two groups' own rows (y_a, mbar_a)
+                        const int gq = tt >> 5, arr = (tt >> 4) & 1, ch = tt & 15;
+                        const int gi = min(t * GPT + gq, G - 1);
+                        const size_t arow = (size_t)(g0 + gatom[gi]);
+                        const uint8_t* so = reinterpret_cast<const uint8_t*>(arr ? a.mbar16 : a.y16) + arow * (kF * 2) + ch * 16;
+                        cp_async16(sOwn + (uint32_t)((gq * 2 + arr) * 256 + ch * 16), so, 16);
                     }
                 }
-                const int row = tang ? NT + col : col;
-                uint8_t* dst = Bop + (row >> 3) * 512 + (row & 7) * 16;
+            }
+            cp_async_commit();
+            {   // radial basis (M1) -> B1, K-major: (n, k) at (n/8)*512 + (k/8)*128 + (n%8)*16 + (k%8)*2
+                uint32_t gv[KPT / 2], gt[KPT / 2];
 #pragma unroll
-                for (int kc = 0; kc < 4; ++kc) *reinterpret_cast<uint4*>(dst + kc * 128) = make_uint4(gp[4 * kc], gp[4 * kc + 1], gp[4 * kc + 2], gp[4 * kc + 3]);
+                for (int k = 0; k < KPT; k += 2) {
+                    const float x0 = r0.x - (float)(sp * KPT + k) * a.delta, x1 = x0 - a.delta;
+                    const float v0 = ex2f(c2 * x0 * x0), v1 = ex2f(c2 * x1 * x1);
+                    gv[k >> 1] = pack_bf16(v0, v1);
+                    if (BWD) gt[k >> 1] = pack_bf16(-v0 * x0 * a.inv_delta2, -v1 * x1 * a.inv_delta2);
+                }
+                uint8_t* dst = Bop + (se >> 3) * 512 + (se & 7) * 16 + sp * (KPT / 8) * 128;
+#pragma unroll
+                for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dst + kc * 128) = make_uint4(gv[4 * kc], gv[4 * kc + 1], gv[4 * kc + 2], gv[4 * kc + 3]);
+                if (BWD) {
+                    uint8_t* dt = Bop + ((NT + se) >> 3) * 512 + (se & 7) * 16 + sp * (KPT / 8) * 128;
+#pragma unroll
+                    for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dt + kc * 128) = make_uint4(gt[4 * kc], gt[4 * kc + 1], gt[4 * kc + 2], gt[4 * kc + 3]);
+                }
+                if (sp == 0) {
+                    scal[se] = r0.y;
+                    if (BWD) { scal[kNCOL + se] = r0.z; scal[2 * kNCOL + se] = r0.w; scal[3 * kNCOL + se] = r1.x; scal[4 * kNCOL + se] = r1.y; }
+                }
             }
             fence_async_smem();
             team_bar(team);
@@ -257,11 +294,12 @@ k_edge_tc(EdgeArgs a, int nchunks)
                     umma(tmem, make_desc(sW1 + k16 * 256, 128, (kR / 8) * 128), make_desc(sB + k16 * 256, 128, (kR / 8) * 128), idesc1, k16 > 0);
                 umma_commit(bar);
             }
+            const int ng = min(GPT, G - t * GPT);                      // groups of this tile
             mbar_wait(bar, phase); phase ^= 1u;
             tc_fence_after();
-            const int nval = min(NT, E - base);
             // ---- phase 2: activation (M3) -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's channel
-            for (int c0 = 0; c0 < nval; c0 += 16) {
+            for (int gq = 0; gq < ng; ++gq) {
+                const int c0 = gq * kGE;
                 uint32_t v[16], vp[16];
                 tmem_ld16(tlane + c0, v);
                 if (BWD) tmem_ld16(tlane + NT + c0, vp);
@@ -273,14 +311,9 @@ k_edge_tc(EdgeArgs a, int nchunks)
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const float x = __uint_as_float(v[c + h]);
-                        const float t = ex2f(-fabsf(x) * kLog2e);
-                        const float l = lg2f(1.f + t);
-                        s[h] = fmaf(kLn2, l, fmaxf(x, 0.f)) - kLn2;
-                        if (BWD) {
-                            const float rr = rcpf(1.f + t);
-                            const float sig = x >= 0.f ? rr : t * rr;
-                            d[h] = sig * __uint_as_float(vp[c + h]);
-                        }
+                        const float th = tanhf_approx(0.5f * x);                       // logistic(x) = (1 + tanh(x/2)) / 2
+                        s[h] = fmaf(-kLn2, lg2f(1.f + fabsf(th)), fmaxf(x, 0.f));      // ssp(x) = max(x,0) - ln(1 + |tanh(x/2)|)
+                        if (BWD) d[h] = fmaf(0.5f, th, 0.5f) * __uint_as_float(vp[c + h]);
                     }
                     pa[c >> 1] = pack_bf16(s[0], s[1]);
                     if (BWD) pt[c >> 1] = pack_bf16(d[0], d[1]);
@@ -304,46 +337,59 @@ k_edge_tc(EdgeArgs a, int nchunks)
                     umma(tmem, make_desc(sW2 + k16 * 256, 128, (kF / 8) * 128), make_desc(sB + k16 * 256, 128, (kF / 8) * 128), idesc2, k16 > 0);
                 umma_commit(bar);
             }
+            cp_async_wait_all();                                       // this thread's gathers (and next tile's records) have landed
             mbar_wait(bar, phase); phase ^= 1u;
             tc_fence_after();
+            team_bar(team);                                            // everybody's gathers are visible
             // ---- phase 3: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
-            for (int c0 = 0; c0 < nval; c0 += 8) {
-                uint32_t v[8], vp[8];
-                tmem_ld8(tlane + c0, v);
-                if (BWD) tmem_ld8(tlane + NT + c0, vp);
+            for (int gq = 0; gq < ng; ++gq) {
+                const int c0 = gq * kGE;
+                const int at = gatom[t * GPT + gq];
+                uint32_t v[16], vp[16];
+                tmem_ld16(tlane + c0, v);
+                if (BWD) tmem_ld16(tlane + NT + c0, vp);
+                if (at != cur) {
+                    flush(); cur = at; part = 0.f;
+                    if (BWD) { fx = fy = fz = 0.f; ya = bf16_ld(own + (gq * 2) * 256 + tt * 2); mba = bf16_ld(own + (gq * 2 + 1) * 256 + tt * 2); }
+                }
                 tmem_wait_ld();
+                const uint8_t* sy = stage + c0 * 256 + tt * 2;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    if (c0 + c < nval) {
-                        if (!BWD) {
-                            const EdgeF s = esf[c0 + c];
-                            if (s.arow != cur) { flush(); cur = s.arow; part = 0.f; }
-                            const float yj = a.y[(size_t)s.jrow * kF + tt];
-                            part = fmaf(yj, __uint_as_float(v[c]) * s.fc, part);
-                        } else {
-                            const EdgeB s = esb[c0 + c];
-                            if (s.arow != cur) {
-                                flush(); cur = s.arow; part = 0.f; fx = fy = fz = 0.f;
-                                ya = a.y[(size_t)cur * kF + tt]; mba = a.mbar[(size_t)cur * kF + tt];
-                            }
-                            const float yj = a.y[(size_t)s.jrow * kF + tt], mbj = a.mbar[(size_t)s.jrow * kF + tt];
-                            const float lin = __uint_as_float(v[c]), linp = __uint_as_float(vp[c]);
-                            const float w = lin * s.fc, wp = fmaf(linp, s.fc, lin * s.fcp);
+                for (int c4 = 0; c4 < 16; c4 += 4) {
+                    const float4 fc4 = *reinterpret_cast<const float4*>(scal + c0 + c4);
+                    const float fcs[4] = {fc4.x, fc4.y, fc4.z, fc4.w};
+                    if (!BWD) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            const float yj = bf16_ld(sy + (c4 + c) * 256);
+                            part = fmaf(yj, __uint_as_float(v[c4 + c]) * fcs[c], part);
+                        }
+                    } else {
+                        const float4 fp4 = *reinterpret_cast<const float4*>(scal + kNCOL + c0 + c4);
+                        const float4 ux4 = *reinterpret_cast<const float4*>(scal + 2 * kNCOL + c0 + c4);
+                        const float4 uy4 = *reinterpret_cast<const float4*>(scal + 3 * kNCOL + c0 + c4);
+                        const float4 uz4 = *reinterpret_cast<const float4*>(scal + 4 * kNCOL + c0 + c4);
+                        const float fps[4] = {fp4.x, fp4.y, fp4.z, fp4.w}, uxs[4] = {ux4.x, ux4.y, ux4.z, ux4.w};
+                        const float uys[4] = {uy4.x, uy4.y, uy4.z, uy4.w}, uzs[4] = {uz4.x, uz4.y, uz4.z, uz4.w};
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            const float yj = bf16_ld(sy + (c4 + c) * 256), mbj = bf16_ld(sy + (NT + c4 + c) * 256);
+                            const float lin = __uint_as_float(v[c4 + c]), linp = __uint_as_float(vp[c4 + c]);
+                            const float w = lin * fcs[c], wp = fmaf(linp, fcs[c], lin * fps[c]);
                             part = fmaf(mbj, w, part);
-                            const float gq = fmaf(mba, yj, mbj * ya) * wp;
-                            fx = fmaf(gq, s.ux, fx); fy = fmaf(gq, s.uy, fy); fz = fmaf(gq, s.uz, fz);
+                            const float gq_ = fmaf(mba, yj, mbj * ya) * wp;
+                            fx = fmaf(gq_, uxs[c], fx); fy = fmaf(gq_, uys[c], fy); fz = fmaf(gq_, uzs[c], fz);
                         }
                     }
                 }
             }
             tc_fence_before();
-            team_bar(team);
         }
         flush();
         if (BWD) {
             team_bar(team);
-            if (tt < kCH && pref[tt + 1] > pref[tt]) {
-                const int g = g0 + tt, b = g / n, i = g - b * n;
+            if (tt < natoms && cnts[tt] > 0) {
+                const int i = ci * kCH + tt;
                 const float* fp = fpart + tt * 12;
                 double* Fb = a.Fout + (size_t)b * 3 * n;
                 Fb[i] += (((double)fp[0] + (double)fp[3]) + (double)fp[6]) + (double)fp[9];
@@ -354,7 +400,7 @@ k_edge_tc(EdgeArgs a, int nchunks)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(256));
 }
 
 int tc_num_sms()
@@ -397,9 +443,10 @@ void launch_edge_tc(Launcher L, const EdgeArgs& a, bool backward)
         cudaFuncSetAttribute(k_edge_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTC);
         configured = true;
     }
-    const int nchunks = (a.total + kCH - 1) / kCH;
+    const int cps = (a.n + kCH - 1) / kCH;
+    const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(tc_num_sms(), nchunks));
-    if (backward) k_edge_tc<true><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, nchunks);
-    else k_edge_tc<false><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, nchunks);
+    if (backward) k_edge_tc<true><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, cps, nchunks);
+    else k_edge_tc<false><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, cps, nchunks);
     LSD_COUNT(L);
 }

@@ -178,7 +178,8 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
 __global__ void __launch_bounds__(256)
 k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __restrict__ img, const int* __restrict__ species, int ns,
           const int* __restrict__ vcount, const uint32_t* __restrict__ vkeys, int vcap, double rc2_single,
-          const double* __restrict__ pair_rc2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags)
+          const double* __restrict__ pair_rc2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags,
+          EdgeRec* __restrict__ recs, float inv_rc)
 {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= n * B) return;
@@ -192,23 +193,43 @@ k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __res
     for (int e0 = 0; e0 < vc; e0 += 32) {
         const int e = e0 + lane;
         bool keep = false; uint32_t key = 0xFFFFFFFFu;
+        double d[3] = {0.0, 0.0, 0.0}, r2 = 0.0;
+        int j = 0;
         if (e < vc) {
             key = vkeys[(size_t)i * vcap + e];
-            const int j = (int)(key >> 5), code = (int)(key & 31u);
+            j = (int)(key >> 5);
+            const int code = (int)(key & 31u);
             int jx, jy, jz; img_unpack(img[j], jx, jy, jz);
             const int s[3] = {code / 9 - 1 + iix - jx, (code / 3) % 3 - 1 + iiy - jy, code % 3 - 1 + iiz - jz};
-            double d[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const double x = __dsub_rn(qb[c * n + j], qb[c * n + i]);
                 d[c] = __dadd_rn(x, __dmul_rn((double)s[c], box.L[c]));     // x - k L with k = -s (exact negation)
             }
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+            r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
             const double lim = pair_rc2 ? pair_rc2[si * ns + species[j]] : rc2_single;
             keep = r2 < lim;
         }
         const unsigned m = __ballot_sync(0xffffffffu, keep);
-        if (keep) { const int pos = cnt + __popc(m & ((1u << lane) - 1)); if (pos < cap) out[pos] = key; }
+        if (keep) {
+            const int pos = cnt + __popc(m & ((1u << lane) - 1));
+            if (pos < cap) {
+                out[pos] = key;
+                if (recs) {                                                 // fp64 geometry rounded once to fp32
+                    const double rd = sqrt(r2);
+                    EdgeRec o;
+                    o.r = (float)rd; o.ux = (float)(d[0] / rd); o.uy = (float)(d[1] / rd); o.uz = (float)(d[2] / rd);
+                    o.fc = 0.f; o.fcp = 0.f;
+                    const float t = o.r * inv_rc;
+                    if (t < 1.f) {                                          // M2
+                        float sn, cs; sincospif(t, &sn, &cs);
+                        o.fc = 0.5f * (cs + 1.f); o.fcp = -0.5f * 3.14159265358979323846f * inv_rc * sn;
+                    }
+                    o.jrow = b * n + j; o.pad = 0;
+                    recs[(size_t)warp * cap + pos] = o;
+                }
+            }
+        }
         cnt += __popc(m);
     }
     if (cnt > cap) { if (lane == 0) atomicOr(flags, LSD_FLAG_OVERFLOW); cnt = cap; }
@@ -270,13 +291,14 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
 }
 
 void launch_compact(Launcher L, const SysDev& sys, int B, const double* q, const int* img, const VerletList& vl,
-                    double rc2_single, const double* pair_rc2, CompactList& cl, int* flags)
+                    double rc2_single, const double* pair_rc2, CompactList& cl, int* flags, float rc_records)
 {
     const size_t warps = (size_t)sys.n * B;
     const int blocks = (int)((warps * 32 + 255) / 256);
     const int pid = prof_begin(L, PROF_NBR);
     k_compact<<<blocks, 256, 0, L.s>>>(sys.n, B, make_box(sys), q, img, sys.species, sys.ns, vl.count, vl.keys, vl.cap, rc2_single,
-                                       pair_rc2, cl.cap, cl.count, cl.keys, flags);
+                                       pair_rc2, cl.cap, cl.count, cl.keys, flags, rc_records > 0.f ? cl.recs : nullptr,
+                                       rc_records > 0.f ? 1.f / rc_records : 0.f);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
