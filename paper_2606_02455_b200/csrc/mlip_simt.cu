@@ -372,7 +372,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; launch_edge_tc(L, ea, false); }
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; launch_edge_tc(L, ea, F, false); }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         pid = prof_begin(L, PROF_DENSE);
@@ -388,7 +388,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; launch_edge_tc(L, ea, true); }
+        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; launch_edge_tc(L, ea, F, true); }
         else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar, nullptr); LSD_COUNT(L); prof_end(L, pid); }
@@ -417,5 +417,10 @@ void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& ne
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                   const int* img, const CompactList& cl, double* F, double* e_atom)
 {
-    run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom, true);
+    switch (net.F) {
+        case 32:  run_fp32<32>(L, sys, net, w, B, q, img, cl, F, e_atom, true); break;
+        case 64:  run_fp32<64>(L, sys, net, w, B, q, img, cl, F, e_atom, true); break;
+        case 128: run_fp32<128>(L, sys, net, w, B, q, img, cl, F, e_atom, true); break;
+        default: break;
+    }
 }

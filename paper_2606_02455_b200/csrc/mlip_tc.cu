@@ -8,14 +8,19 @@
 // serial sums inside one thread in the order of the atom's sorted neighbour row (deterministic, independent of the
 // batch and of the tiling), and every per-channel operand of the epilogue is read from shared memory.
 //
-// One persistent CTA per SM, 4 teams of 128 threads.  The weights (A operands, K-major canonical no-swizzle layout,
-// packed on the host) are resident in shared memory and shared by the teams; each team owns 64 TMEM columns, one
-// B-operand buffer and one gather stage, and walks chunks of 64 consecutive atoms of one state.  An atom's row is
-// cut into groups of 16 edge slots (the last one padded with zero records), so a group never straddles two atoms;
-// a tile is 4 groups (forward: 64 edges) or 2 groups (backward: 32 value + 32 tangent columns).  Per tile and team:
+// Widths below 128 fill the 128 accumulator rows with Q = 128 / F independent edge sets: row q F + f is channel f of
+// set q.  The A operand of set q is a 128-row window into [128-F zero rows ; W ; 128-F zero rows] that puts W at rows
+// q F.., so one MMA per set and K-slice accumulates D[q F + f, n] = sum_k W[f, k] B_q[k, n] and adds exact zeros
+// elsewhere (all operand buffers are zero-initialised and only ever hold finite values).
+//
+// One persistent CTA per SM, 4 teams of 128 threads.  The weights (K-major canonical no-swizzle layout, packed on the
+// host) are resident in shared memory and shared by the teams; each team owns 64 TMEM columns, one B-operand buffer
+// and one gather stage, and walks chunks of 64 consecutive atoms of one state (set q owns atoms q 64/Q ..).  An
+// atom's row is cut into groups of 16 edge slots (the last one padded with zero records), so a group never straddles
+// two atoms; a tile is GPT groups per set.  Per tile and team:
 //     cp.async: edge records of the NEXT tile, bf16 feature rows y_j (mbar_j) of THIS tile  -> smem (lands under the MMAs)
-//     radial basis -> smem (B1, K-major)                 | MMA1 (2 x K16)  -> TMEM
-//     TMEM -> activation -> smem (B2, MN-major, bf16)    | MMA2 (8 x K16)  -> TMEM (same columns)
+//     radial basis -> smem (B1, K-major)                 | MMA1 -> TMEM
+//     TMEM -> activation -> smem (B2, MN-major, bf16)    | MMA2 -> TMEM (same columns)
 //     TMEM -> cutoff, cfconv products and adjoints, per-atom accumulation in registers.
 // The phases of different teams overlap (MUFU-bound activation of one team with the FMA/LSU-bound epilogue of another,
 // both with the tensor pipe).  Edge geometry comes from the records k_compact wrote once per batched evaluation.
@@ -25,30 +30,36 @@
 
 namespace {
 
-constexpr int kF = 128;                 // channels = MMA M
-constexpr int kR = LSD_NRBF;            // 32 = K of the first contraction
+constexpr int kR = LSD_NRBF;            // 32 = K of the first contraction (per set)
 constexpr int kTeams = 4;
-constexpr int kTT = 128;                // threads per team
+constexpr int kTT = 128;                // threads per team = accumulator rows
 constexpr int kThreadsTC = kTeams * kTT;
-constexpr int kNCOL = 64;               // MMA N = TMEM columns per team
 constexpr int kCH = 64;                 // atoms per chunk
 constexpr int kGE = 16;                 // edge slots per group
 constexpr int kMaxGroups = kCH * (512 / kGE);   // rows hold at most 512 slots (neighbor.cu)
 
-constexpr int kW1Bytes = kF * kR * 2;           // 8 KB
-constexpr int kW2Bytes = kF * kF * 2;           // 32 KB
-constexpr int kB2Bytes = kNCOL * kF * 2;        // 16 KB (B1 aliases its first 4 KB)
-constexpr int kStageBytes = kNCOL * kF * 2;     // 16 KB: forward 64 rows of y_j; backward 32 rows of y_j + 32 rows of mbar_j
-constexpr int kOwnBytes = 2 * 2 * kF * 2;       // backward: (y_a, mbar_a) of the tile's two groups
-constexpr int kRecBytes = 2 * kNCOL * 32;       // double-buffered edge records
-constexpr int kScalBytes = 5 * kNCOL * 4;       // fc, fcp, ux, uy, uz per tile edge
-constexpr int kPrefBytes = 272;                 // (kCH + 1) ints, padded
-constexpr int kCntBytes = kCH * 4;
-constexpr int kFpartBytes = kCH * 4 * 3 * 4;
-constexpr int kTeamBytes = kB2Bytes + kStageBytes + kOwnBytes + kRecBytes + kScalBytes + kPrefBytes + kCntBytes + kMaxGroups + kFpartBytes;
-constexpr int kSmemTC = kW1Bytes + kW2Bytes + kTeams * kTeamBytes;
-static_assert(kSmemTC <= 227 * 1024, "shared memory budget");
-static_assert(kTeamBytes % 16 == 0, "team regions stay 16-byte aligned");
+template <int F, bool BWD> struct TcCfg {
+    static constexpr int Q = 128 / F;                                   // edge sets
+    static constexpr int GPT = F == 32 ? (BWD ? 1 : 2) : (BWD ? 2 : 4);   // groups per tile and set
+    static constexpr int NT = GPT * kGE;                                // edges per tile and set
+    static constexpr int NCOLS = NT * (BWD ? 2 : 1);                    // MMA N (value [+ tangent] columns)
+    static constexpr int ET = Q * NT;                                   // edges per tile
+    static constexpr int ZROWS = 256 - F;                               // rows of the padded weight images
+    static constexpr int W1Bytes = ZROWS * kR * 2;
+    static constexpr int W2Bytes = ZROWS * F * 2;
+    static constexpr int B2Bytes = NCOLS * 128 * 2;                     // B1 (Q*32 x NCOLS) aliases its head
+    static constexpr int StageBytes = ET * F * 2 * (BWD ? 2 : 1);
+    static constexpr int OwnBytes = BWD ? Q * GPT * 2 * F * 2 : 0;
+    static constexpr int RecBytes = 2 * ET * 32;
+    static constexpr int ScalBytes = (BWD ? 5 : 1) * ET * 4;
+    static constexpr int PrefBytes = 272, CntBytes = kCH * 4;
+    static constexpr int FpartBytes = BWD ? kCH * (F / 32) * 3 * 4 : 0;
+    static constexpr int TeamBytes = B2Bytes + StageBytes + OwnBytes + RecBytes + ScalBytes + PrefBytes + CntBytes + kMaxGroups + FpartBytes;
+    static constexpr int Smem = W1Bytes + W2Bytes + kTeams * TeamBytes;
+    static_assert(Smem <= 227 * 1024, "shared memory budget");
+    static_assert(TeamBytes % 16 == 0 && W1Bytes % 16 == 0 && W2Bytes % 16 == 0, "regions stay 16-byte aligned");
+    static_assert(NCOLS <= 64 && NCOLS % 16 == 0, "TMEM columns per team");
+};
 
 constexpr float kLn2 = 0.69314718055994530942f;
 constexpr float kLog2e = 1.44269504088896340736f;
@@ -97,8 +108,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok = 0;
     while (!ok) {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity), "r"(20000u) : "memory");       // suspend-time hint: sleep instead of spinning
     }
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -121,27 +132,34 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <bool BWD>
+template <int F, bool BWD>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
 {
-    constexpr int GPT = BWD ? 2 : 4;                   // groups per tile
-    constexpr int NT = GPT * kGE;                      // edges per tile
-    constexpr int TPE = kTT / NT;                      // threads per edge in the staging phase (2 forward, 4 backward)
-    constexpr int KPT = kR / TPE;                      // radial basis functions per staging thread (16 / 8)
+    using C = TcCfg<F, BWD>;
+    constexpr int Q = C::Q, GPT = C::GPT, NT = C::NT, NCOLS = C::NCOLS, ET = C::ET;
+    constexpr int AQ = kCH / Q;                        // atoms per set and chunk
+    constexpr int TPE = kTT / ET;                      // threads per edge in the staging phase
+    constexpr int KPT = kR / TPE;                      // radial basis functions per staging thread
+    constexpr int RCH = F / 8;                         // 16-byte chunks per bf16 feature row
+    constexpr int NSW = F >= 64 ? 8 : 4;               // stage swizzle period
+    static_assert(TPE >= 1 && TPE * ET == kTT, "staging roles");
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[kTeams];
     __shared__ uint32_t tmem_base_s;
     __shared__ int next_chunk, s_chunk[kTeams];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, team = tid >> 7, tt = tid & (kTT - 1);
+    const int q = tt / F, f = tt % F;                  // this thread's accumulator row: set q, channel f
 
-    {   // resident A operands (already in the canonical K-major layout)
+    {   // resident A operand images (canonical K-major layout); every other operand buffer starts as zeros
         const uint4* s1 = reinterpret_cast<const uint4*>(a.Wf1_tc);
         const uint4* s2 = reinterpret_cast<const uint4*>(a.Wf2_tc);
         uint4* d1 = reinterpret_cast<uint4*>(smem);
-        uint4* d2 = reinterpret_cast<uint4*>(smem + kW1Bytes);
-        for (int i = tid; i < kW1Bytes / 16; i += kThreadsTC) d1[i] = s1[i];
-        for (int i = tid; i < kW2Bytes / 16; i += kThreadsTC) d2[i] = s2[i];
+        uint4* d2 = reinterpret_cast<uint4*>(smem + C::W1Bytes);
+        for (int i = tid; i < C::W1Bytes / 16; i += kThreadsTC) d1[i] = s1[i];
+        for (int i = tid; i < C::W2Bytes / 16; i += kThreadsTC) d2[i] = s2[i];
+        uint4* z = reinterpret_cast<uint4*>(smem + C::W1Bytes + C::W2Bytes);
+        for (int i = tid; i < kTeams * C::TeamBytes / 16; i += kThreadsTC) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     if (tid == 0) {
         for (int t = 0; t < kTeams; ++t) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar[t])));
@@ -157,25 +175,32 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
     __syncthreads();
     tc_fence_after();
 
-    uint8_t* const tb = smem + kW1Bytes + kW2Bytes + team * kTeamBytes;
-    uint8_t* const Bop = tb;                                           // B2 [64 cols][128 k] MN-major; B1 aliases its head
-    uint8_t* const stage = Bop + kB2Bytes;
-    uint8_t* const own = stage + kStageBytes;
-    uint8_t* const recs = own + kOwnBytes;                             // [2][NT] EdgeRec
-    float* const scal = reinterpret_cast<float*>(recs + kRecBytes);    // [5][kNCOL]
-    int* const pref = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(scal) + kScalBytes);   // first group of every atom of the chunk
-    int* const cnts = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(pref) + kPrefBytes);
-    uint8_t* const gatom = reinterpret_cast<uint8_t*>(cnts) + kCntBytes;                        // group -> atom of the chunk
+    uint8_t* const tb = smem + C::W1Bytes + C::W2Bytes + team * C::TeamBytes;
+    uint8_t* const Bop = tb;                                           // B2 [NCOLS][128 k] MN-major; B1 aliases its head
+    uint8_t* const stage = Bop + C::B2Bytes;
+    uint8_t* const own = stage + C::StageBytes;
+    uint8_t* const recs = own + C::OwnBytes;                           // [2][ET] EdgeRec
+    float* const scal = reinterpret_cast<float*>(recs + C::RecBytes);  // [5][ET]: fc (, fcp, ux, uy, uz)
+    int* const pref = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(scal) + C::ScalBytes);   // first group of every atom of the chunk
+    int* const cnts = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(pref) + C::PrefBytes);
+    uint8_t* const gatom = reinterpret_cast<uint8_t*>(cnts) + C::CntBytes;                      // group -> atom of the chunk
     float* const fpart = reinterpret_cast<float*>(gatom + kMaxGroups);
-    const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + kW1Bytes), sB = smem_u32(Bop), bar = smem_u32(&mbar[team]);
+    const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + C::W1Bytes), sB = smem_u32(Bop), bar = smem_u32(&mbar[team]);
     const uint32_t sStage = smem_u32(stage), sOwn = smem_u32(own), sRecs = smem_u32(recs);
-    const uint32_t tmem = tmem_base_s + (uint32_t)(team * kNCOL);
+    const uint32_t tmem = tmem_base_s + (uint32_t)(team * 64);
     const uint32_t tlane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-    const uint32_t idesc1 = make_idesc(kF, kNCOL, 0), idesc2 = make_idesc(kF, kNCOL, 1);
+    const uint32_t idesc1 = make_idesc(128, NCOLS, 0), idesc2 = make_idesc(128, NCOLS, 1);
     uint32_t phase = 0;
     const int n = a.n;
-    const int se = tt / TPE, sp = tt % TPE;            // staging role: edge of the tile, part of its row
+    const int se = tt / TPE, sp = tt % TPE;            // staging role: edge of the tile (set sq, column sn), part of its row
+    const int sq = se / NT, sn = se % NT;
     const float c2 = -0.5f * kLog2e * a.inv_delta2;
+    // gather stage rows are F/8 chunks of 16 B, chunk c of row e stored at c ^ swz(e) (conflict-free cp.async writes);
+    // this thread's channel sits in chunk f/8: byte offset inside a row for each value of swz(e)
+    int soff[NSW];
+#pragma unroll
+    for (int k = 0; k < NSW; ++k) soff[k] = (((f >> 3) ^ k) << 4) + (f & 7) * 2;
+    auto swz = [](int e) { return F >= 64 ? (e & 7) : ((e >> 1) & 3); };
 
     for (;;) {
         if (tt == 0) s_chunk[team] = atomicAdd(&next_chunk, 1);
@@ -189,45 +214,50 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
         team_bar(team);
         if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= kCH; ++i) { s += pref[i]; pref[i] = s; } }
         team_bar(team);
-        const int G = pref[kCH];
         if (tt < kCH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
         {   // atoms without neighbours: their sums are empty
             float* out = BWD ? a.ybar : a.m_out;
-            if (out) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * kF + tt] = 0.f;
+            if (out && tt < F) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * F + tt] = 0.f;
         }
         team_bar(team);
+        int gmax = 0;
+#pragma unroll
+        for (int k = 0; k < Q; ++k) gmax = max(gmax, pref[(k + 1) * AQ] - pref[k * AQ]);
+        const int ntiles = (gmax + GPT - 1) / GPT;
+        const int gbase = pref[q * AQ], Gq = pref[(q + 1) * AQ] - gbase;      // this thread's set: first group, group count
 
         // asynchronous copy of the edge records of tile t into buffer t & 1 (zero records for padding slots)
         auto fetch_records = [&](int t) {
-            for (int idx = tt; idx < NT * 2; idx += kTT) {
+            for (int idx = tt; idx < ET * 2; idx += kTT) {
                 const int e = idx >> 1, half = idx & 1;
-                const int gi = t * GPT + e / kGE;
+                const int eq = e / NT, en = e % NT;
+                const int gl = t * GPT + en / kGE;
+                const int gb = pref[eq * AQ];
                 const EdgeRec* src = a.recs;
                 uint32_t bytes = 0;
-                if (gi < G) {
-                    const int at = gatom[gi];
-                    const int slot = (gi - pref[at]) * kGE + (e & (kGE - 1));
+                if (gl < pref[(eq + 1) * AQ] - gb) {
+                    const int at = gatom[gb + gl];
+                    const int slot = (gb + gl - pref[at]) * kGE + (en & (kGE - 1));
                     if (slot < cnts[at]) { src = a.recs + (size_t)(g0 + at) * a.cap + slot; bytes = 16; }
                 }
-                cp_async16(sRecs + (uint32_t)(((t & 1) * NT + e) * 32 + half * 16), reinterpret_cast<const uint8_t*>(src) + half * 16, bytes);
+                cp_async16(sRecs + (uint32_t)(((t & 1) * ET + e) * 32 + half * 16), reinterpret_cast<const uint8_t*>(src) + half * 16, bytes);
             }
         };
-        const int ntiles = (G + GPT - 1) / GPT;
         if (ntiles > 0) fetch_records(0);
         cp_async_commit();
 
         int cur = -1;
         float part = 0.f, ya = 0.f, mba = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-        auto flush = [&]() {
+        auto flush = [&]() {                                           // warp-uniform (a warp belongs to one set)
             if (cur < 0) return;
-            if (!BWD) a.m_out[(size_t)(g0 + cur) * kF + tt] = part;
+            if (!BWD) a.m_out[(size_t)(g0 + cur) * F + f] = part;
             else {
-                if (a.ybar) a.ybar[(size_t)(g0 + cur) * kF + tt] = part;
+                if (a.ybar) a.ybar[(size_t)(g0 + cur) * F + f] = part;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
                     fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
                 }
-                if (lane == 0) { float* fp = fpart + (cur * 4 + (warp & 3)) * 3; fp[0] = fx; fp[1] = fy; fp[2] = fz; }
+                if (lane == 0) { float* fp = fpart + (cur * (F / 32) + (f >> 5)) * 3; fp[0] = fx; fp[1] = fy; fp[2] = fz; }
             }
         };
 
@@ -236,34 +266,32 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             cp_async_wait_all();
             team_bar(team);                                            // also: everybody is done with the previous tile's buffers
             if (t + 1 < ntiles) fetch_records(t + 1);
-            const uint8_t* rec = recs + ((t & 1) * NT + se) * 32;
+            const uint8_t* rec = recs + ((t & 1) * ET + se) * 32;
             const float4 r0 = *reinterpret_cast<const float4*>(rec);   // r, fc, fcp, ux
             const float4 r1 = *reinterpret_cast<const float4*>(rec + 16);   // uy, uz, jrow, pad
             {
                 const int jrow = __float_as_int(r1.z);
-                if (!BWD) {                                            // y_j: 16 chunks of 16 B, two threads per edge
-                    const uint8_t* src = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (kF * 2);
+                const uint8_t* sy = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (F * 2);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) cp_async16(sStage + (uint32_t)(se * 256 + (2 * i + sp) * 16), src + (2 * i + sp) * 16, 16);
-                } else {                                               // y_j and mbar_j, four threads per edge
-                    const uint8_t* sy = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (kF * 2);
-                    const uint8_t* sm = reinterpret_cast<const uint8_t*>(a.mbar16) + (size_t)jrow * (kF * 2);
+                for (int i = 0; i < RCH / TPE; ++i)
+                    cp_async16(sStage + (uint32_t)(se * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sy + (TPE * i + sp) * 16, 16);
+                if (BWD) {
+                    const uint8_t* sm = reinterpret_cast<const uint8_t*>(a.mbar16) + (size_t)jrow * (F * 2);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        cp_async16(sStage + (uint32_t)(se * 256 + (4 * i + sp) * 16), sy + (4 * i + sp) * 16, 16);
-                        cp_async16(sStage + (uint32_t)((NT + se) * 256 + (4 * i + sp) * 16), sm + (4 * i + sp) * 16, 16);
-                    }
-                    if (tt < 64) {                                     // the two groups' own rows (y_a, mbar_a)
-                        const int gq = tt >> 5, arr = (tt >> 4) & 1, ch = tt & 15;
-                        const int gi = min(t * GPT + gq, G - 1);
-                        const size_t arow = (size_t)(g0 + gatom[gi]);
-                        const uint8_t* so = reinterpret_cast<const uint8_t*>(arr ? a.mbar16 : a.y16) + arow * (kF * 2) + ch * 16;
-                        cp_async16(sOwn + (uint32_t)((gq * 2 + arr) * 256 + ch * 16), so, 16);
+                    for (int i = 0; i < RCH / TPE; ++i)
+                        cp_async16(sStage + (uint32_t)((ET + se) * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sm + (TPE * i + sp) * 16, 16);
+                    if (tt < Q * GPT * 2 * RCH) {                      // the groups' own rows (y_a, mbar_a)
+                        const int ch = tt % RCH, arr = (tt / RCH) & 1, gs = tt / (2 * RCH);     // gs = set * GPT + group
+                        const int oq = gs / GPT, gl = t * GPT + gs % GPT;
+                        const int gb = pref[oq * AQ], gq_n = pref[(oq + 1) * AQ] - gb;
+                        const size_t arow = (size_t)(g0 + (gq_n > 0 ? gatom[gb + min(gl, gq_n - 1)] : 0));
+                        const uint8_t* so = reinterpret_cast<const uint8_t*>(arr ? a.mbar16 : a.y16) + arow * (F * 2) + ch * 16;
+                        cp_async16(sOwn + (uint32_t)((gs * 2 + arr) * (2 * F) + ch * 16), so, 16);
                     }
                 }
             }
             cp_async_commit();
-            {   // radial basis (M1) -> B1, K-major: (n, k) at (n/8)*512 + (k/8)*128 + (n%8)*16 + (k%8)*2
+            {   // radial basis (M1) -> B1, K-major: (n, k) at (n/8)*Q*512 + (k/8)*128 + (n%8)*16 + (k%8)*2, k = sq*32 + basis index
                 uint32_t gv[KPT / 2], gt[KPT / 2];
 #pragma unroll
                 for (int k = 0; k < KPT; k += 2) {
@@ -272,17 +300,17 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
                     gv[k >> 1] = pack_bf16(v0, v1);
                     if (BWD) gt[k >> 1] = pack_bf16(-v0 * x0 * a.inv_delta2, -v1 * x1 * a.inv_delta2);
                 }
-                uint8_t* dst = Bop + (se >> 3) * 512 + (se & 7) * 16 + sp * (KPT / 8) * 128;
+                uint8_t* dst = Bop + (sn >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
 #pragma unroll
                 for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dst + kc * 128) = make_uint4(gv[4 * kc], gv[4 * kc + 1], gv[4 * kc + 2], gv[4 * kc + 3]);
                 if (BWD) {
-                    uint8_t* dt = Bop + ((NT + se) >> 3) * 512 + (se & 7) * 16 + sp * (KPT / 8) * 128;
+                    uint8_t* dt = Bop + ((NT + sn) >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
 #pragma unroll
                     for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dt + kc * 128) = make_uint4(gt[4 * kc], gt[4 * kc + 1], gt[4 * kc + 2], gt[4 * kc + 3]);
                 }
                 if (sp == 0) {
                     scal[se] = r0.y;
-                    if (BWD) { scal[kNCOL + se] = r0.z; scal[2 * kNCOL + se] = r0.w; scal[3 * kNCOL + se] = r1.x; scal[4 * kNCOL + se] = r1.y; }
+                    if (BWD) { scal[ET + se] = r0.z; scal[2 * ET + se] = r0.w; scal[3 * ET + se] = r1.x; scal[4 * ET + se] = r1.y; }
                 }
             }
             fence_async_smem();
@@ -290,14 +318,17 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             if (tt == 0) {
                 tc_fence_after();
 #pragma unroll
-                for (int k16 = 0; k16 < kR / 16; ++k16)
-                    umma(tmem, make_desc(sW1 + k16 * 256, 128, (kR / 8) * 128), make_desc(sB + k16 * 256, 128, (kR / 8) * 128), idesc1, k16 > 0);
+                for (int k = 0; k < Q; ++k)
+#pragma unroll
+                    for (int k16 = 0; k16 < kR / 16; ++k16)
+                        umma(tmem, make_desc(sW1 + ((128 - F - k * F) / 8) * 512 + k16 * 256, 128, 512),
+                             make_desc(sB + (k * 4 + k16 * 2) * 128, 128, Q * 512), idesc1, (k | k16) > 0);
                 umma_commit(bar);
             }
-            const int ng = min(GPT, G - t * GPT);                      // groups of this tile
+            const int ng = max(0, min(GPT, Gq - t * GPT));             // groups of this tile in this thread's set
             mbar_wait(bar, phase); phase ^= 1u;
             tc_fence_after();
-            // ---- phase 2: activation (M3) -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's channel
+            // ---- phase 2: activation (M3) -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's row
             for (int gq = 0; gq < ng; ++gq) {
                 const int c0 = gq * kGE;
                 uint32_t v[16], vp[16];
@@ -310,9 +341,11 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
                     float s[2], d[2];
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        const float x = __uint_as_float(v[c + h]);
-                        const float th = tanhf_approx(0.5f * x);                       // logistic(x) = (1 + tanh(x/2)) / 2
-                        s[h] = fmaf(-kLn2, lg2f(1.f + fabsf(th)), fmaxf(x, 0.f));      // ssp(x) = max(x,0) - ln(1 + |tanh(x/2)|)
+                        // W_f1 is packed as W_f1 / 2 and W_f2 as 2 W_f2 (exact in bf16): the accumulator holds x / 2 and the
+                        // operand written here is ssp(x) / 2 (and logistic(x) x' / 2)
+                        const float hx = __uint_as_float(v[c + h]);
+                        const float th = tanhf_approx(hx);                             // logistic(x) = (1 + tanh(x/2)) / 2
+                        s[h] = fmaf(-0.5f * kLn2, lg2f(1.f + fabsf(th)), fmaxf(hx, 0.f));   // ssp(x) = max(x,0) - ln(1 + |tanh(x/2)|)
                         if (BWD) d[h] = fmaf(0.5f, th, 0.5f) * __uint_as_float(vp[c + h]);
                     }
                     pa[c >> 1] = pack_bf16(s[0], s[1]);
@@ -333,8 +366,11 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             if (tt == 0) {
                 tc_fence_after();
 #pragma unroll
-                for (int k16 = 0; k16 < kF / 16; ++k16)
-                    umma(tmem, make_desc(sW2 + k16 * 256, 128, (kF / 8) * 128), make_desc(sB + k16 * 256, 128, (kF / 8) * 128), idesc2, k16 > 0);
+                for (int k = 0; k < Q; ++k)
+#pragma unroll
+                    for (int k16 = 0; k16 < F / 16; ++k16)
+                        umma(tmem, make_desc(sW2 + ((128 - F - k * F) / 8) * (F / 8) * 128 + k16 * 256, 128, (F / 8) * 128),
+                             make_desc(sB + (k * (F / 16) + k16) * 256, 128, 2048), idesc2, (k | k16) > 0);
                 umma_commit(bar);
             }
             cp_async_wait_all();                                       // this thread's gathers (and next tile's records) have landed
@@ -344,36 +380,41 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             // ---- phase 3: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
             for (int gq = 0; gq < ng; ++gq) {
                 const int c0 = gq * kGE;
-                const int at = gatom[t * GPT + gq];
+                const int at = gatom[gbase + t * GPT + gq];
                 uint32_t v[16], vp[16];
                 tmem_ld16(tlane + c0, v);
                 if (BWD) tmem_ld16(tlane + NT + c0, vp);
                 if (at != cur) {
                     flush(); cur = at; part = 0.f;
-                    if (BWD) { fx = fy = fz = 0.f; ya = bf16_ld(own + (gq * 2) * 256 + tt * 2); mba = bf16_ld(own + (gq * 2 + 1) * 256 + tt * 2); }
+                    if (BWD) {
+                        fx = fy = fz = 0.f;
+                        ya = bf16_ld(own + ((q * GPT + gq) * 2) * (2 * F) + f * 2); mba = bf16_ld(own + ((q * GPT + gq) * 2 + 1) * (2 * F) + f * 2);
+                    }
                 }
                 tmem_wait_ld();
-                const uint8_t* sy = stage + c0 * 256 + tt * 2;
+                const int e0 = q * NT + c0;                            // stage row / scalar index of the group's first edge
+                const uint8_t* sy = stage + e0 * (2 * F);
 #pragma unroll
                 for (int c4 = 0; c4 < 16; c4 += 4) {
-                    const float4 fc4 = *reinterpret_cast<const float4*>(scal + c0 + c4);
+                    const float4 fc4 = *reinterpret_cast<const float4*>(scal + e0 + c4);
                     const float fcs[4] = {fc4.x, fc4.y, fc4.z, fc4.w};
                     if (!BWD) {
 #pragma unroll
                         for (int c = 0; c < 4; ++c) {
-                            const float yj = bf16_ld(sy + (c4 + c) * 256);
+                            const float yj = bf16_ld(sy + (c4 + c) * (2 * F) + soff[swz(c4 + c)]);
                             part = fmaf(yj, __uint_as_float(v[c4 + c]) * fcs[c], part);
                         }
                     } else {
-                        const float4 fp4 = *reinterpret_cast<const float4*>(scal + kNCOL + c0 + c4);
-                        const float4 ux4 = *reinterpret_cast<const float4*>(scal + 2 * kNCOL + c0 + c4);
-                        const float4 uy4 = *reinterpret_cast<const float4*>(scal + 3 * kNCOL + c0 + c4);
-                        const float4 uz4 = *reinterpret_cast<const float4*>(scal + 4 * kNCOL + c0 + c4);
+                        const float4 fp4 = *reinterpret_cast<const float4*>(scal + ET + e0 + c4);
+                        const float4 ux4 = *reinterpret_cast<const float4*>(scal + 2 * ET + e0 + c4);
+                        const float4 uy4 = *reinterpret_cast<const float4*>(scal + 3 * ET + e0 + c4);
+                        const float4 uz4 = *reinterpret_cast<const float4*>(scal + 4 * ET + e0 + c4);
                         const float fps[4] = {fp4.x, fp4.y, fp4.z, fp4.w}, uxs[4] = {ux4.x, ux4.y, ux4.z, ux4.w};
                         const float uys[4] = {uy4.x, uy4.y, uy4.z, uy4.w}, uzs[4] = {uz4.x, uz4.y, uz4.z, uz4.w};
 #pragma unroll
                         for (int c = 0; c < 4; ++c) {
-                            const float yj = bf16_ld(sy + (c4 + c) * 256), mbj = bf16_ld(sy + (NT + c4 + c) * 256);
+                            const float yj = bf16_ld(sy + (c4 + c) * (2 * F) + soff[swz(c4 + c)]);
+                            const float mbj = bf16_ld(sy + (ET + c4 + c) * (2 * F) + soff[swz(c4 + c)]);
                             const float lin = __uint_as_float(v[c4 + c]), linp = __uint_as_float(vp[c4 + c]);
                             const float w = lin * fcs[c], wp = fmaf(linp, fcs[c], lin * fps[c]);
                             part = fmaf(mbj, w, part);
@@ -390,11 +431,12 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             team_bar(team);
             if (tt < natoms && cnts[tt] > 0) {
                 const int i = ci * kCH + tt;
-                const float* fp = fpart + tt * 12;
+                const float* fp = fpart + tt * (F / 32) * 3;
+                double sx = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll
+                for (int w = 0; w < F / 32; ++w) { sx += (double)fp[3 * w]; sy += (double)fp[3 * w + 1]; sz += (double)fp[3 * w + 2]; }
                 double* Fb = a.Fout + (size_t)b * 3 * n;
-                Fb[i] += (((double)fp[0] + (double)fp[3]) + (double)fp[6]) + (double)fp[9];
-                Fb[n + i] += (((double)fp[1] + (double)fp[4]) + (double)fp[7]) + (double)fp[10];
-                Fb[2 * n + i] += (((double)fp[2] + (double)fp[5]) + (double)fp[8]) + (double)fp[11];
+                Fb[i] += sx; Fb[n + i] += sy; Fb[2 * n + i] += sz;
             }
         }
     }
@@ -419,34 +461,48 @@ uint16_t bf16_rne(double x)
     return (uint16_t)(u >> 16);
 }
 
-}  // namespace
-
-bool mlip_tc_supported(const MlipDev& net) { return net.F == kF && net.R == kR; }
-
-// A operands: (m, k) at byte (m/8)*SBO + (k/8)*128 + (m%8)*16 + (k%8)*2, SBO = (K/8)*128
-void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2)
-{
-    out1.assign((size_t)F * R, 0); out2.assign((size_t)F * F, 0);
-    for (int m = 0; m < F; ++m)
-        for (int k = 0; k < R; ++k)
-            out1[((size_t)(m / 8) * (R / 8) * 128 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_rne(Wf1[(size_t)m * R + k]);
-    for (int m = 0; m < F; ++m)
-        for (int k = 0; k < F; ++k)
-            out2[((size_t)(m / 8) * (F / 8) * 128 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_rne(Wf2[(size_t)m * F + k]);
-}
-
-void launch_edge_tc(Launcher L, const EdgeArgs& a, bool backward)
+template <int F>
+void launch_edge_tc_f(Launcher L, const EdgeArgs& a, bool backward)
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_edge_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTC);
-        cudaFuncSetAttribute(k_edge_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTC);
+        cudaFuncSetAttribute(k_edge_tc<F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, false>::Smem);
+        cudaFuncSetAttribute(k_edge_tc<F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, true>::Smem);
         configured = true;
     }
     const int cps = (a.n + kCH - 1) / kCH;
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(tc_num_sms(), nchunks));
-    if (backward) k_edge_tc<true><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, cps, nchunks);
-    else k_edge_tc<false><<<grid, kThreadsTC, kSmemTC, L.s>>>(a, cps, nchunks);
+    if (backward) k_edge_tc<F, true><<<grid, kThreadsTC, TcCfg<F, true>::Smem, L.s>>>(a, cps, nchunks);
+    else k_edge_tc<F, false><<<grid, kThreadsTC, TcCfg<F, false>::Smem, L.s>>>(a, cps, nchunks);
     LSD_COUNT(L);
+}
+
+}  // namespace
+
+bool mlip_tc_supported(const MlipDev& net) { return (net.F == 32 || net.F == 64 || net.F == 128) && net.R == kR; }
+
+// A operand images: [128-F zero rows ; W/2 or 2W ; 128-F zero rows], (m, k) at byte (m/8)*SBO + (k/8)*128 + (m%8)*16 + (k%8)*2,
+// SBO = (K/8)*128.  W_f1 is stored halved and W_f2 doubled (both exact in bf16), see the activation phase of k_edge_tc.
+void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2)
+{
+    const int zrows = 256 - F, pad = 128 - F;
+    out1.assign((size_t)zrows * R, 0); out2.assign((size_t)zrows * F, 0);
+    for (int r = 0; r < F; ++r) {
+        const int m = pad + r;
+        for (int k = 0; k < R; ++k)
+            out1[((size_t)(m / 8) * (R / 8) * 128 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_rne(0.5 * Wf1[(size_t)r * R + k]);
+        for (int k = 0; k < F; ++k)
+            out2[((size_t)(m / 8) * (F / 8) * 128 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_rne(2.0 * Wf2[(size_t)r * F + k]);
+    }
+}
+
+void launch_edge_tc(Launcher L, const EdgeArgs& a, int F, bool backward)
+{
+    switch (F) {
+        case 32: launch_edge_tc_f<32>(L, a, backward); break;
+        case 64: launch_edge_tc_f<64>(L, a, backward); break;
+        case 128: launch_edge_tc_f<128>(L, a, backward); break;
+        default: break;
+    }
 }
