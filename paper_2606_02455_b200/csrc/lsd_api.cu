@@ -168,7 +168,7 @@ lsd_status alloc_compact(lsd_ctx* ctx, CompactList& cl, int cap, int bmax, bool 
     cl.cap = cap; cl.bmax = bmax;
     TRY(dalloc(ctx, &cl.count, (size_t)ctx->sys.n * bmax));
     TRY(dalloc(ctx, &cl.keys, (size_t)ctx->sys.n * bmax * cap));
-    if (records) TRY(dalloc(ctx, &cl.recs, (size_t)ctx->sys.n * bmax * cap));
+    if (records) TRY(dalloc(ctx, &cl.recs, (size_t)ctx->sys.n * bmax * cap * 8));
     return LSD_OK;
 }
 lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
@@ -209,7 +209,7 @@ lsd_status probe_capacity(lsd_ctx* ctx, double rc_skin, int* cap_out)
     if (hf & LSD_FLAG_OVERFLOW) return fail(ctx, LSD_ERR_NBR_OVERFLOW, "neighbour row exceeds 512 entries (cutoff + skin too large for this density)");
     int mx = 0; for (int v : h) mx = std::max(mx, v);
     int cap = (int)(mx * 1.25) + 8;
-    cap = (cap + 7) / 8 * 8;
+    cap = (cap + 15) / 16 * 16;
     *cap_out = std::min(cap, 512);
     return LSD_OK;
 }

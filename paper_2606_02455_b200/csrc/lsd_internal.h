@@ -61,15 +61,30 @@ struct VerletList {                  // window-shared candidate list (r < rc + s
     uint32_t* keys = nullptr;        // [n][cap]  key = (j << 5) | shiftcode, sorted ascending
 };
 
-// geometry of one directed edge i <- j of one state, written once per batched evaluation by k_compact and read by
-// every block's forward and backward edge kernel: r = |q_j - q_i + s L|, unit vector, cosine cutoff (M2) and its slope
-struct __align__(16) EdgeRec { float r, fc, fcp, ux, uy, uz; int jrow, pad; };   // jrow = b*n + j (row of the gathered features)
+// Geometry of the directed edges i <- j of one state, written once per batched evaluation by k_compact and read by every
+// block's forward and backward edge kernel.  A row (state b, atom i) holds cap/16 groups of 16 slots; a group is a
+// 512-byte block of 8 fields x 16 slots (structure of arrays, so a kernel copies it verbatim and reads float4 runs):
+//   r = |q_j - q_i + s L|, fc, fc' (cosine cutoff M2 and its slope), ux, uy, uz (unit vector), jrow = b*n + j (row of the
+//   gathered features, as int bits), pad.  Slots behind the row's count inside its last group are zero records
+//   (fc = fc' = 0, jrow = own row).
+#define LSD_REC_R 0
+#define LSD_REC_FC 1
+#define LSD_REC_FCP 2
+#define LSD_REC_UX 3
+#define LSD_REC_UY 4
+#define LSD_REC_UZ 5
+#define LSD_REC_JROW 6
+#define LSD_REC_GROUP_FLOATS 128
+__host__ __device__ inline size_t lsd_rec_index(size_t row, int cap, int slot, int field)
+{
+    return row * (size_t)cap * 8 + (size_t)(slot >> 4) * LSD_REC_GROUP_FLOATS + field * 16 + (slot & 15);
+}
 
 struct CompactList {                 // per-state exact list (r < rc), rows padded with 0xFFFFFFFF
     int cap = 0, bmax = 0;
     int* count = nullptr;            // [bmax*n]
     uint32_t* keys = nullptr;        // [bmax*n][cap]
-    EdgeRec* recs = nullptr;         // [bmax*n][cap], MLIP lists only
+    float* recs = nullptr;           // [bmax*n][cap/16][8][16], MLIP lists only (cap is a multiple of 16)
 };
 
 struct CellGrid {
@@ -155,7 +170,7 @@ void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B
 // arguments of the continuous-filter convolution kernels (fp32 and tcgen05 variants)
 struct EdgeArgs {
     int total, n, cap;
-    const int* count; const uint32_t* keys; const EdgeRec* recs;
+    const int* count; const uint32_t* keys; const float* recs;
     float rc, inv_rc, delta, inv_delta2;
     const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major), fp32 path
     const void *Wf1_tc = nullptr, *Wf2_tc = nullptr;   // bf16, UMMA canonical K-major layouts (mlip_tc.cu)

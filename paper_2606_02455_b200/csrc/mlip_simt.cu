@@ -244,7 +244,6 @@ k_edge(EdgeArgs a)
     for (int g = blockIdx.x * kWarps + warp; g < a.total; g += gridDim.x * kWarps) {
         const int b = g / n, i = g % n;
         const int cnt = a.count[g];
-        const EdgeRec* row = a.recs + (size_t)g * a.cap;
         float part[CPT], ya[CPT], mba[CPT];
 #pragma unroll
         for (int c = 0; c < CPT; ++c) part[c] = 0.f;
@@ -257,9 +256,9 @@ k_edge(EdgeArgs a)
             float r = 0.f, fc = 0.f, fcp = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
             int jrow = g;
             if (valid) {
-                const float4 e0 = *reinterpret_cast<const float4*>(row + slot);
-                const float4 e1 = *(reinterpret_cast<const float4*>(row + slot) + 1);
-                r = e0.x; fc = e0.y; fcp = e0.z; ux = e0.w; uy = e1.x; uz = e1.y; jrow = __float_as_int(e1.z);
+                const float* e = a.recs + lsd_rec_index((size_t)g, a.cap, slot, 0);
+                r = e[LSD_REC_R * 16]; fc = e[LSD_REC_FC * 16]; jrow = __float_as_int(e[LSD_REC_JROW * 16]);
+                if (BWD) { fcp = e[LSD_REC_FCP * 16]; ux = e[LSD_REC_UX * 16]; uy = e[LSD_REC_UY * 16]; uz = e[LSD_REC_UZ * 16]; }
             }
             // --- radial basis rows (M1): lane k holds basis k; BWD interleaves value / r-derivative rows
 #pragma unroll

@@ -40,25 +40,25 @@ constexpr int kMaxGroups = kCH * (512 / kGE);   // rows hold at most 512 slots (
 
 template <int F, bool BWD> struct TcCfg {
     static constexpr int Q = 128 / F;                                   // edge sets
-    static constexpr int GPT = F == 32 ? (BWD ? 1 : 2) : (BWD ? 2 : 4);   // groups per tile and set
+    static constexpr int GPT = F == 128 ? (BWD ? 2 : 4) : (BWD ? 1 : 2);   // groups per tile and set
     static constexpr int NT = GPT * kGE;                                // edges per tile and set
     static constexpr int NCOLS = NT * (BWD ? 2 : 1);                    // MMA N (value [+ tangent] columns)
     static constexpr int ET = Q * NT;                                   // edges per tile
     static constexpr int ZROWS = 256 - F;                               // rows of the padded weight images
     static constexpr int W1Bytes = ZROWS * kR * 2;
     static constexpr int W2Bytes = ZROWS * F * 2;
-    static constexpr int B2Bytes = NCOLS * 128 * 2;                     // B1 (Q*32 x NCOLS) aliases its head
+    static constexpr int B2Bytes = NCOLS * 128 * 2;
+    static constexpr int B1Bytes = NCOLS * Q * kR * 2;
     static constexpr int StageBytes = ET * F * 2 * (BWD ? 2 : 1);
     static constexpr int OwnBytes = BWD ? Q * GPT * 2 * F * 2 : 0;
-    static constexpr int RecBytes = 2 * ET * 32;
-    static constexpr int ScalBytes = (BWD ? 5 : 1) * ET * 4;
+    static constexpr int RecBytes = 3 * ET * 32;                        // three tiles of record groups in flight
     static constexpr int PrefBytes = 272, CntBytes = kCH * 4;
     static constexpr int FpartBytes = BWD ? kCH * (F / 32) * 3 * 4 : 0;
-    static constexpr int TeamBytes = B2Bytes + StageBytes + OwnBytes + RecBytes + ScalBytes + PrefBytes + CntBytes + kMaxGroups + FpartBytes;
+    static constexpr int TeamBytes = B2Bytes + B1Bytes + StageBytes + OwnBytes + RecBytes + PrefBytes + CntBytes + kMaxGroups + FpartBytes;
     static constexpr int Smem = W1Bytes + W2Bytes + kTeams * TeamBytes;
-    static_assert(Smem <= 227 * 1024, "shared memory budget");
+    static_assert(Smem + 256 <= 227 * 1024, "shared memory budget");
     static_assert(TeamBytes % 16 == 0 && W1Bytes % 16 == 0 && W2Bytes % 16 == 0, "regions stay 16-byte aligned");
-    static_assert(NCOLS <= 64 && NCOLS % 16 == 0, "TMEM columns per team");
+    static_assert(NCOLS <= 64 && NCOLS % 16 == 0, "TMEM columns per team and accumulator");
 };
 
 constexpr float kLn2 = 0.69314718055994530942f;
@@ -143,9 +143,10 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
     constexpr int KPT = kR / TPE;                      // radial basis functions per staging thread
     constexpr int RCH = F / 8;                         // 16-byte chunks per bf16 feature row
     constexpr int NSW = F >= 64 ? 8 : 4;               // stage swizzle period
+    constexpr int RECF = ET * 8;                       // floats per tile of record groups
     static_assert(TPE >= 1 && TPE * ET == kTT, "staging roles");
-    extern __shared__ __align__(1024) uint8_t smem[];
-    __shared__ __align__(8) uint64_t mbar[kTeams];
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t mbar[2 * kTeams];
     __shared__ uint32_t tmem_base_s;
     __shared__ int next_chunk, s_chunk[kTeams];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, team = tid >> 7, tt = tid & (kTT - 1);
@@ -162,12 +163,12 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
         for (int i = tid; i < kTeams * C::TeamBytes / 16; i += kThreadsTC) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     if (tid == 0) {
-        for (int t = 0; t < kTeams; ++t) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar[t])));
+        for (int t = 0; t < 2 * kTeams; ++t) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar[t])));
         asm volatile("fence.mbarrier_init.release.cluster;");
         next_chunk = 0;
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(256));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     fence_async_smem();
@@ -176,24 +177,27 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
     tc_fence_after();
 
     uint8_t* const tb = smem + C::W1Bytes + C::W2Bytes + team * C::TeamBytes;
-    uint8_t* const Bop = tb;                                           // B2 [NCOLS][128 k] MN-major; B1 aliases its head
-    uint8_t* const stage = Bop + C::B2Bytes;
+    uint8_t* const B2 = tb;                                            // [NCOLS][128 k] MN-major
+    uint8_t* const B1 = B2 + C::B2Bytes;                               // [NCOLS][Q*32 k] K-major
+    uint8_t* const stage = B1 + C::B1Bytes;
     uint8_t* const own = stage + C::StageBytes;
-    uint8_t* const recs = own + C::OwnBytes;                           // [2][ET] EdgeRec
-    float* const scal = reinterpret_cast<float*>(recs + C::RecBytes);  // [5][ET]: fc (, fcp, ux, uy, uz)
-    int* const pref = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(scal) + C::ScalBytes);   // first group of every atom of the chunk
+    float* const recs = reinterpret_cast<float*>(own + C::OwnBytes);   // [3][ET/16 groups][8 fields][16 slots]
+    int* const pref = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(recs) + C::RecBytes);   // first group of every atom of the chunk
     int* const cnts = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(pref) + C::PrefBytes);
     uint8_t* const gatom = reinterpret_cast<uint8_t*>(cnts) + C::CntBytes;                      // group -> atom of the chunk
     float* const fpart = reinterpret_cast<float*>(gatom + kMaxGroups);
-    const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + C::W1Bytes), sB = smem_u32(Bop), bar = smem_u32(&mbar[team]);
+    const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + C::W1Bytes), sB1 = smem_u32(B1), sB2 = smem_u32(B2);
+    const uint32_t bar1 = smem_u32(&mbar[2 * team]), bar2 = smem_u32(&mbar[2 * team + 1]);
     const uint32_t sStage = smem_u32(stage), sOwn = smem_u32(own), sRecs = smem_u32(recs);
-    const uint32_t tmem = tmem_base_s + (uint32_t)(team * 64);
-    const uint32_t tlane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t tmem1 = tmem_base_s + (uint32_t)(team * 128), tmem2 = tmem1 + 64;             // D1, D2 accumulators
+    const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t tl1 = tmem1 + lane_sel, tl2 = tmem2 + lane_sel;
     const uint32_t idesc1 = make_idesc(128, NCOLS, 0), idesc2 = make_idesc(128, NCOLS, 1);
-    uint32_t phase = 0;
+    uint32_t phase1 = 0, phase2 = 0;
     const int n = a.n;
     const int se = tt / TPE, sp = tt % TPE;            // staging role: edge of the tile (set sq, column sn), part of its row
     const int sq = se / NT, sn = se % NT;
+    const int srec = (sq * GPT + sn / kGE) * LSD_REC_GROUP_FLOATS + (sn & (kGE - 1));   // this edge inside a tile of record groups
     const float c2 = -0.5f * kLog2e * a.inv_delta2;
     // gather stage rows are F/8 chunks of 16 B, chunk c of row e stored at c ^ swz(e) (conflict-free cp.async writes);
     // this thread's channel sits in chunk f/8: byte offset inside a row for each value of swz(e)
@@ -226,25 +230,75 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
         const int ntiles = (gmax + GPT - 1) / GPT;
         const int gbase = pref[q * AQ], Gq = pref[(q + 1) * AQ] - gbase;      // this thread's set: first group, group count
 
-        // asynchronous copy of the edge records of tile t into buffer t & 1 (zero records for padding slots)
+        // asynchronous copy of the record groups of tile t into buffer t % 3 (zeros for groups behind a set's end)
         auto fetch_records = [&](int t) {
             for (int idx = tt; idx < ET * 2; idx += kTT) {
-                const int e = idx >> 1, half = idx & 1;
-                const int eq = e / NT, en = e % NT;
-                const int gl = t * GPT + en / kGE;
+                const int gs = idx >> 5, chunk16 = idx & 31;           // gs = set * GPT + group of the tile
+                const int eq = gs / GPT, gl = t * GPT + gs % GPT;
                 const int gb = pref[eq * AQ];
-                const EdgeRec* src = a.recs;
+                const float* src = a.recs;
                 uint32_t bytes = 0;
                 if (gl < pref[(eq + 1) * AQ] - gb) {
                     const int at = gatom[gb + gl];
-                    const int slot = (gb + gl - pref[at]) * kGE + (en & (kGE - 1));
-                    if (slot < cnts[at]) { src = a.recs + (size_t)(g0 + at) * a.cap + slot; bytes = 16; }
+                    src = a.recs + lsd_rec_index((size_t)(g0 + at), a.cap, (gb + gl - pref[at]) * kGE, 0);
+                    bytes = 16;
                 }
-                cp_async16(sRecs + (uint32_t)(((t & 1) * ET + e) * 32 + half * 16), reinterpret_cast<const uint8_t*>(src) + half * 16, bytes);
+                cp_async16(sRecs + (uint32_t)(((t % 3) * RECF + gs * LSD_REC_GROUP_FLOATS) * 4 + chunk16 * 16),
+                           reinterpret_cast<const uint8_t*>(src) + chunk16 * 16, bytes);
             }
         };
-        if (ntiles > 0) fetch_records(0);
-        cp_async_commit();
+        // radial basis (M1) of tile t -> B1, K-major: (n, k) at (n/8)*Q*512 + (k/8)*128 + (n%8)*16 + (k%8)*2, k = sq*32 + basis index
+        auto stage_basis = [&](int t) {
+            const float r = recs[(t % 3) * RECF + srec + LSD_REC_R * 16];
+            uint32_t gv[KPT / 2], gt[KPT / 2];
+#pragma unroll
+            for (int k = 0; k < KPT; k += 2) {
+                const float x0 = r - (float)(sp * KPT + k) * a.delta, x1 = x0 - a.delta;
+                const float v0 = ex2f(c2 * x0 * x0), v1 = ex2f(c2 * x1 * x1);
+                gv[k >> 1] = pack_bf16(v0, v1);
+                if (BWD) gt[k >> 1] = pack_bf16(-v0 * x0 * a.inv_delta2, -v1 * x1 * a.inv_delta2);
+            }
+            uint8_t* dst = B1 + (sn >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
+#pragma unroll
+            for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dst + kc * 128) = make_uint4(gv[4 * kc], gv[4 * kc + 1], gv[4 * kc + 2], gv[4 * kc + 3]);
+            if (BWD) {
+                uint8_t* dt = B1 + ((NT + sn) >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
+#pragma unroll
+                for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dt + kc * 128) = make_uint4(gt[4 * kc], gt[4 * kc + 1], gt[4 * kc + 2], gt[4 * kc + 3]);
+            }
+        };
+        auto issue_mma1 = [&]() {                                      // one thread: D1 = sum over sets of window(W_f1) * B1
+            tc_fence_after();
+#pragma unroll
+            for (int k = 0; k < Q; ++k)
+#pragma unroll
+                for (int k16 = 0; k16 < kR / 16; ++k16)
+                    umma(tmem1, make_desc(sW1 + ((128 - F - k * F) / 8) * 512 + k16 * 256, 128, 512),
+                         make_desc(sB1 + (k * 4 + k16 * 2) * 128, 128, Q * 512), idesc1, (k | k16) > 0);
+            umma_commit(bar1);
+        };
+        // bf16 feature rows of tile t (y_j, mbar_j and the groups' own rows) -> gather stage
+        auto issue_gathers = [&](int t) {
+            const int jrow = __float_as_int(recs[(t % 3) * RECF + srec + LSD_REC_JROW * 16]);
+            const uint8_t* sy = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (F * 2);
+#pragma unroll
+            for (int i = 0; i < RCH / TPE; ++i)
+                cp_async16(sStage + (uint32_t)(se * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sy + (TPE * i + sp) * 16, 16);
+            if (BWD) {
+                const uint8_t* sm = reinterpret_cast<const uint8_t*>(a.mbar16) + (size_t)jrow * (F * 2);
+#pragma unroll
+                for (int i = 0; i < RCH / TPE; ++i)
+                    cp_async16(sStage + (uint32_t)((ET + se) * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sm + (TPE * i + sp) * 16, 16);
+                if (tt < Q * GPT * 2 * RCH) {                          // the groups' own rows (y_a, mbar_a)
+                    const int ch = tt % RCH, arr = (tt / RCH) & 1, gs = tt / (2 * RCH);     // gs = set * GPT + group
+                    const int oq = gs / GPT, gl = t * GPT + gs % GPT;
+                    const int gb = pref[oq * AQ], gq_n = pref[(oq + 1) * AQ] - gb;
+                    const size_t arow = (size_t)(g0 + (gq_n > 0 ? gatom[gb + min(gl, gq_n - 1)] : 0));
+                    const uint8_t* so = reinterpret_cast<const uint8_t*>(arr ? a.mbar16 : a.y16) + arow * (F * 2) + ch * 16;
+                    cp_async16(sOwn + (uint32_t)((gs * 2 + arr) * (2 * F) + ch * 16), so, 16);
+                }
+            }
+        };
 
         int cur = -1;
         float part = 0.f, ya = 0.f, mba = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
@@ -261,79 +315,30 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
             }
         };
 
-        for (int t = 0; t < ntiles; ++t) {
-            // ---- phase 1: records of this tile are in shared memory; start the gathers, build the radial basis operand
-            cp_async_wait_all();
-            team_bar(team);                                            // also: everybody is done with the previous tile's buffers
-            if (t + 1 < ntiles) fetch_records(t + 1);
-            const uint8_t* rec = recs + ((t & 1) * ET + se) * 32;
-            const float4 r0 = *reinterpret_cast<const float4*>(rec);   // r, fc, fcp, ux
-            const float4 r1 = *reinterpret_cast<const float4*>(rec + 16);   // uy, uz, jrow, pad
-            {
-                const int jrow = __float_as_int(r1.z);
-                const uint8_t* sy = reinterpret_cast<const uint8_t*>(a.y16) + (size_t)jrow * (F * 2);
-#pragma unroll
-                for (int i = 0; i < RCH / TPE; ++i)
-                    cp_async16(sStage + (uint32_t)(se * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sy + (TPE * i + sp) * 16, 16);
-                if (BWD) {
-                    const uint8_t* sm = reinterpret_cast<const uint8_t*>(a.mbar16) + (size_t)jrow * (F * 2);
-#pragma unroll
-                    for (int i = 0; i < RCH / TPE; ++i)
-                        cp_async16(sStage + (uint32_t)((ET + se) * (2 * F) + (((TPE * i + sp) ^ swz(se)) << 4)), sm + (TPE * i + sp) * 16, 16);
-                    if (tt < Q * GPT * 2 * RCH) {                      // the groups' own rows (y_a, mbar_a)
-                        const int ch = tt % RCH, arr = (tt / RCH) & 1, gs = tt / (2 * RCH);     // gs = set * GPT + group
-                        const int oq = gs / GPT, gl = t * GPT + gs % GPT;
-                        const int gb = pref[oq * AQ], gq_n = pref[(oq + 1) * AQ] - gb;
-                        const size_t arow = (size_t)(g0 + (gq_n > 0 ? gatom[gb + min(gl, gq_n - 1)] : 0));
-                        const uint8_t* so = reinterpret_cast<const uint8_t*>(arr ? a.mbar16 : a.y16) + arow * (F * 2) + ch * 16;
-                        cp_async16(sOwn + (uint32_t)((gs * 2 + arr) * (2 * F) + ch * 16), so, 16);
-                    }
-                }
-            }
-            cp_async_commit();
-            {   // radial basis (M1) -> B1, K-major: (n, k) at (n/8)*Q*512 + (k/8)*128 + (n%8)*16 + (k%8)*2, k = sq*32 + basis index
-                uint32_t gv[KPT / 2], gt[KPT / 2];
-#pragma unroll
-                for (int k = 0; k < KPT; k += 2) {
-                    const float x0 = r0.x - (float)(sp * KPT + k) * a.delta, x1 = x0 - a.delta;
-                    const float v0 = ex2f(c2 * x0 * x0), v1 = ex2f(c2 * x1 * x1);
-                    gv[k >> 1] = pack_bf16(v0, v1);
-                    if (BWD) gt[k >> 1] = pack_bf16(-v0 * x0 * a.inv_delta2, -v1 * x1 * a.inv_delta2);
-                }
-                uint8_t* dst = Bop + (sn >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
-#pragma unroll
-                for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dst + kc * 128) = make_uint4(gv[4 * kc], gv[4 * kc + 1], gv[4 * kc + 2], gv[4 * kc + 3]);
-                if (BWD) {
-                    uint8_t* dt = Bop + ((NT + sn) >> 3) * (Q * 512) + (sn & 7) * 16 + (sq * 4 + sp * (KPT / 8)) * 128;
-#pragma unroll
-                    for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dt + kc * 128) = make_uint4(gt[4 * kc], gt[4 * kc + 1], gt[4 * kc + 2], gt[4 * kc + 3]);
-                }
-                if (sp == 0) {
-                    scal[se] = r0.y;
-                    if (BWD) { scal[ET + se] = r0.z; scal[2 * ET + se] = r0.w; scal[3 * ET + se] = r1.x; scal[4 * ET + se] = r1.y; }
-                }
-            }
+        // ---- prologue: records of tiles 0 and 1, radial basis and MMA1 of tile 0
+        if (ntiles > 0) fetch_records(0);
+        if (ntiles > 1) fetch_records(1);
+        cp_async_commit();
+        cp_async_wait_all();
+        team_bar(team);
+        if (ntiles > 0) {
+            stage_basis(0);
             fence_async_smem();
             team_bar(team);
-            if (tt == 0) {
-                tc_fence_after();
-#pragma unroll
-                for (int k = 0; k < Q; ++k)
-#pragma unroll
-                    for (int k16 = 0; k16 < kR / 16; ++k16)
-                        umma(tmem, make_desc(sW1 + ((128 - F - k * F) / 8) * 512 + k16 * 256, 128, 512),
-                             make_desc(sB + (k * 4 + k16 * 2) * 128, 128, Q * 512), idesc1, (k | k16) > 0);
-                umma_commit(bar);
-            }
+            if (tt == 0) issue_mma1();
+        }
+
+        for (int t = 0; t < ntiles; ++t) {
             const int ng = max(0, min(GPT, Gq - t * GPT));             // groups of this tile in this thread's set
-            mbar_wait(bar, phase); phase ^= 1u;
+            const float* rt = recs + (t % 3) * RECF + (q * GPT) * LSD_REC_GROUP_FLOATS;   // this set's record groups of the tile
+            // ---- activation (M3) of tile t: D1 -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's row
+            mbar_wait(bar1, phase1); phase1 ^= 1u;
             tc_fence_after();
-            // ---- phase 2: activation (M3) -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's row
             for (int gq = 0; gq < ng; ++gq) {
                 const int c0 = gq * kGE;
                 uint32_t v[16], vp[16];
-                tmem_ld16(tlane + c0, v);
-                if (BWD) tmem_ld16(tlane + NT + c0, vp);
+                tmem_ld16(tl1 + c0, v);
+                if (BWD) tmem_ld16(tl1 + NT + c0, vp);
                 tmem_wait_ld();
                 uint32_t pa[8], pt[8];
 #pragma unroll
@@ -351,39 +356,49 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
                     pa[c >> 1] = pack_bf16(s[0], s[1]);
                     if (BWD) pt[c >> 1] = pack_bf16(d[0], d[1]);
                 }
-                uint8_t* d0 = Bop + (c0 >> 3) * 2048 + tt * 16;
+                uint8_t* d0 = B2 + (c0 >> 3) * 2048 + tt * 16;
                 *reinterpret_cast<uint4*>(d0) = make_uint4(pa[0], pa[1], pa[2], pa[3]);
                 *reinterpret_cast<uint4*>(d0 + 2048) = make_uint4(pa[4], pa[5], pa[6], pa[7]);
                 if (BWD) {
-                    uint8_t* d1 = Bop + ((NT + c0) >> 3) * 2048 + tt * 16;
+                    uint8_t* d1 = B2 + ((NT + c0) >> 3) * 2048 + tt * 16;
                     *reinterpret_cast<uint4*>(d1) = make_uint4(pt[0], pt[1], pt[2], pt[3]);
                     *reinterpret_cast<uint4*>(d1 + 2048) = make_uint4(pt[4], pt[5], pt[6], pt[7]);
                 }
             }
             tc_fence_before();
             fence_async_smem();
-            team_bar(team);
+            team_bar(team);                                            // B2 complete; everybody is done with tile t-1's stage, D2 and records
             if (tt == 0) {
                 tc_fence_after();
 #pragma unroll
                 for (int k = 0; k < Q; ++k)
 #pragma unroll
                     for (int k16 = 0; k16 < F / 16; ++k16)
-                        umma(tmem, make_desc(sW2 + ((128 - F - k * F) / 8) * (F / 8) * 128 + k16 * 256, 128, (F / 8) * 128),
-                             make_desc(sB + (k * (F / 16) + k16) * 256, 128, 2048), idesc2, (k | k16) > 0);
-                umma_commit(bar);
+                        umma(tmem2, make_desc(sW2 + ((128 - F - k * F) / 8) * (F / 8) * 128 + k16 * 256, 128, (F / 8) * 128),
+                             make_desc(sB2 + (k * (F / 16) + k16) * 256, 128, 2048), idesc2, (k | k16) > 0);
+                umma_commit(bar2);
             }
-            cp_async_wait_all();                                       // this thread's gathers (and next tile's records) have landed
-            mbar_wait(bar, phase); phase ^= 1u;
+            issue_gathers(t);                                          // land under MMA2(t) and the staging of tile t+1
+            if (t + 2 < ntiles) fetch_records(t + 2);
+            cp_async_commit();
+            // ---- radial basis and MMA1 of tile t+1 (its records arrived an iteration ago) while MMA2(t) runs
+            if (t + 1 < ntiles) {
+                stage_basis(t + 1);
+                fence_async_smem();
+                team_bar(team);
+                if (tt == 0) issue_mma1();
+            }
+            // ---- epilogue of tile t: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
+            cp_async_wait_all();                                       // this thread's gathers (and tile t+2's records) have landed
+            mbar_wait(bar2, phase2); phase2 ^= 1u;
             tc_fence_after();
             team_bar(team);                                            // everybody's gathers are visible
-            // ---- phase 3: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
             for (int gq = 0; gq < ng; ++gq) {
                 const int c0 = gq * kGE;
                 const int at = gatom[gbase + t * GPT + gq];
                 uint32_t v[16], vp[16];
-                tmem_ld16(tlane + c0, v);
-                if (BWD) tmem_ld16(tlane + NT + c0, vp);
+                tmem_ld16(tl2 + c0, v);
+                if (BWD) tmem_ld16(tl2 + NT + c0, vp);
                 if (at != cur) {
                     flush(); cur = at; part = 0.f;
                     if (BWD) {
@@ -392,11 +407,11 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
                     }
                 }
                 tmem_wait_ld();
-                const int e0 = q * NT + c0;                            // stage row / scalar index of the group's first edge
-                const uint8_t* sy = stage + e0 * (2 * F);
+                const float* rg = rt + gq * LSD_REC_GROUP_FLOATS;      // fields x 16 slots of this group
+                const uint8_t* sy = stage + (q * NT + c0) * (2 * F);
 #pragma unroll
                 for (int c4 = 0; c4 < 16; c4 += 4) {
-                    const float4 fc4 = *reinterpret_cast<const float4*>(scal + e0 + c4);
+                    const float4 fc4 = *reinterpret_cast<const float4*>(rg + LSD_REC_FC * 16 + c4);
                     const float fcs[4] = {fc4.x, fc4.y, fc4.z, fc4.w};
                     if (!BWD) {
 #pragma unroll
@@ -405,10 +420,10 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
                             part = fmaf(yj, __uint_as_float(v[c4 + c]) * fcs[c], part);
                         }
                     } else {
-                        const float4 fp4 = *reinterpret_cast<const float4*>(scal + ET + e0 + c4);
-                        const float4 ux4 = *reinterpret_cast<const float4*>(scal + 2 * ET + e0 + c4);
-                        const float4 uy4 = *reinterpret_cast<const float4*>(scal + 3 * ET + e0 + c4);
-                        const float4 uz4 = *reinterpret_cast<const float4*>(scal + 4 * ET + e0 + c4);
+                        const float4 fp4 = *reinterpret_cast<const float4*>(rg + LSD_REC_FCP * 16 + c4);
+                        const float4 ux4 = *reinterpret_cast<const float4*>(rg + LSD_REC_UX * 16 + c4);
+                        const float4 uy4 = *reinterpret_cast<const float4*>(rg + LSD_REC_UY * 16 + c4);
+                        const float4 uz4 = *reinterpret_cast<const float4*>(rg + LSD_REC_UZ * 16 + c4);
                         const float fps[4] = {fp4.x, fp4.y, fp4.z, fp4.w}, uxs[4] = {ux4.x, ux4.y, ux4.z, ux4.w};
                         const float uys[4] = {uy4.x, uy4.y, uy4.z, uy4.w}, uzs[4] = {uz4.x, uz4.y, uz4.z, uz4.w};
 #pragma unroll
@@ -442,7 +457,7 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(256));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
 int tc_num_sms()

@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256)
 k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __restrict__ img, const int* __restrict__ species, int ns,
           const int* __restrict__ vcount, const uint32_t* __restrict__ vkeys, int vcap, double rc2_single,
           const double* __restrict__ pair_rc2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags,
-          EdgeRec* __restrict__ recs, float inv_rc)
+          float* __restrict__ recs, float inv_rc)
 {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= n * B) return;
@@ -217,16 +217,17 @@ k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __res
                 out[pos] = key;
                 if (recs) {                                                 // fp64 geometry rounded once to fp32
                     const double rd = sqrt(r2);
-                    EdgeRec o;
-                    o.r = (float)rd; o.ux = (float)(d[0] / rd); o.uy = (float)(d[1] / rd); o.uz = (float)(d[2] / rd);
-                    o.fc = 0.f; o.fcp = 0.f;
-                    const float t = o.r * inv_rc;
+                    const float rf = (float)rd;
+                    float fc = 0.f, fcp = 0.f;
+                    const float t = rf * inv_rc;
                     if (t < 1.f) {                                          // M2
                         float sn, cs; sincospif(t, &sn, &cs);
-                        o.fc = 0.5f * (cs + 1.f); o.fcp = -0.5f * 3.14159265358979323846f * inv_rc * sn;
+                        fc = 0.5f * (cs + 1.f); fcp = -0.5f * 3.14159265358979323846f * inv_rc * sn;
                     }
-                    o.jrow = b * n + j; o.pad = 0;
-                    recs[(size_t)warp * cap + pos] = o;
+                    float* o = recs + lsd_rec_index((size_t)warp, cap, pos, 0);
+                    o[LSD_REC_R * 16] = rf; o[LSD_REC_FC * 16] = fc; o[LSD_REC_FCP * 16] = fcp;
+                    o[LSD_REC_UX * 16] = (float)(d[0] / rd); o[LSD_REC_UY * 16] = (float)(d[1] / rd); o[LSD_REC_UZ * 16] = (float)(d[2] / rd);
+                    o[LSD_REC_JROW * 16] = __int_as_float(b * n + j);
                 }
             }
         }
@@ -234,6 +235,15 @@ k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __res
     }
     if (cnt > cap) { if (lane == 0) atomicOr(flags, LSD_FLAG_OVERFLOW); cnt = cap; }
     for (int e = cnt + lane; e < cap; e += 32) out[e] = 0xFFFFFFFFu;
+    if (recs) {                                                             // zero records behind the count, to the end of the last group
+        const int e = cnt + lane;
+        if (lane < 16 && e < ((cnt + 15) & ~15) && e < cap) {
+            float* o = recs + lsd_rec_index((size_t)warp, cap, e, 0);
+#pragma unroll
+            for (int fld = 0; fld < 6; ++fld) o[fld * 16] = 0.f;
+            o[LSD_REC_JROW * 16] = __int_as_float(warp);
+        }
+    }
     if (lane == 0) count[warp] = cnt;
 }
 
