@@ -255,7 +255,7 @@ def main():
                         kernel="k_edge<F,true> (MLIP edge backward)", avg_launch_ms=avg_ms, launches=eb["launches"],
                         algorithmic_flops_per_launch=flops_per_launch, directed_edges_per_window=edges, peak_note=peak_note,
                         share_of_step=eb["ms"] / ms if ms > 0 else None,
-                        a2_strict_tflops=edges * T * (2 * R * F + 2 * F * F + 8 * F) / (mlip_ms * 1e-3) / 1e12 if mlip_ms > 0 else None,
+                        a2_strict_tflops=args.steps * edges * T * (2 * R * F + 2 * F * F + 8 * F) / (mlip_ms * 1e-3) / 1e12 if mlip_ms > 0 else None,
                         stage_ms_per_step={k: v["ms"] / args.steps for k, v in prof.items() if v["launches"]})
 
     if rank == 0:

@@ -104,6 +104,7 @@ struct MlipWork {                    // activations of one batched evaluation (k
     std::vector<float*> y, h;        // [T] each [bmax*n][F]
     std::vector<uint16_t*> y16;      // [T] bf16 copies of y gathered by the tcgen05 edge kernels (LSD_BF16_TC only)
     uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
+    uint32_t* ym16 = nullptr;        // width 128 only: rows of (y, mbar) bf16 pairs gathered by the backward tcgen05 kernel
     double* e_atom = nullptr;        // [bmax*n]
 };
 
@@ -176,6 +177,7 @@ struct EdgeArgs {
     const void *Wf1_tc = nullptr, *Wf2_tc = nullptr;   // bf16, UMMA canonical K-major layouts (mlip_tc.cu)
     const float* y;                   // [total][F]
     const uint16_t *y16 = nullptr, *mbar16 = nullptr;   // bf16 rows gathered by the tcgen05 kernels
+    const uint32_t* ym16 = nullptr;   // [total][F] (y | mbar << 16) bf16 pairs, width-128 backward kernel
     float* m_out;                     // FWD: m
     const float* mbar; float* ybar;   // BWD
     double* Fout;                     // BWD: [B][3][n], accumulated
@@ -189,6 +191,7 @@ size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
 // ---- mlip_tc.cu (bf16 tcgen05 filter path)
 bool mlip_tc_supported(const MlipDev& net);
 void launch_edge_tc(Launcher L, const EdgeArgs& a, int F, bool backward);
+void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_tc128.cu: width 128
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,

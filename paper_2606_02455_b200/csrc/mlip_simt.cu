@@ -103,7 +103,8 @@ enum DenseMode { DENSE_IN = 0, DENSE_OUT = 1, BWD_OUT = 2, BWD_IN = 3 };
 template <int F, int MODE>
 __global__ void __launch_bounds__(kThreads, 1)
 k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, const float* __restrict__ W1,
-        float* __restrict__ aux, float* __restrict__ out, uint16_t* __restrict__ out16)
+        float* __restrict__ aux, float* __restrict__ out, uint16_t* __restrict__ out16,
+        const uint16_t* __restrict__ pair16 = nullptr, uint32_t* __restrict__ outpair = nullptr)
 {
     constexpr int CPT = F / 32, LDA = F + 4;
     constexpr bool TWO = (MODE == DENSE_OUT || MODE == BWD_OUT);
@@ -177,6 +178,14 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
                 } else {
                     stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
                     if (out16) st16(out16 + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
+                    if (outpair) {                                         // (y, mbar) bf16 pairs for the width-128 backward edge kernel
+                        const size_t o = (size_t)(g0 + r) * F + lane * CPT;
+#pragma unroll
+                        for (int c = 0; c < CPT; ++c) {
+                            const __nv_bfloat16 hb = __float2bfloat16_rn(acc2[r][c]);
+                            outpair[o + c] = (uint32_t)pair16[o + c] | ((uint32_t)*reinterpret_cast<const uint16_t*>(&hb) << 16);
+                        }
+                    }
                 }
             }
         }
@@ -371,7 +380,10 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; launch_edge_tc(L, ea, F, false); }
+        if (use_tc) {
+            ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t];
+            if (F == 128) launch_edge_tc128(L, ea, false); else launch_edge_tc(L, ea, F, false);
+        }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         pid = prof_begin(L, PROF_DENSE);
@@ -383,11 +395,16 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     prof_end(L, pidr);
     for (int t = net.T - 1; t >= 0; --t) {
         int pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc ? w.mbar16 : nullptr); LSD_COUNT(L);
+        const bool pairs = use_tc && F == 128;
+        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc && !pairs ? w.mbar16 : nullptr,
+                                                                                 pairs ? w.y16[t] : nullptr, pairs ? w.ym16 : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        if (use_tc) { ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; launch_edge_tc(L, ea, F, true); }
+        if (use_tc) {
+            ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; ea.ym16 = w.ym16;
+            if (F == 128) launch_edge_tc128(L, ea, true); else launch_edge_tc(L, ea, F, true);
+        }
         else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar, nullptr); LSD_COUNT(L); prof_end(L, pid); }
