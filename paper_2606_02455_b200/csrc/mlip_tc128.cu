@@ -25,11 +25,12 @@ constexpr int kF = 128;
 constexpr int kR = LSD_NRBF;
 constexpr int kTeams = 4;
 constexpr int kTT = 128;                // threads per team = accumulator rows
-constexpr int kThreads = kTeams * kTT;
+constexpr int kThreads = kTeams * kTT + kTeams * 32;   // + one MMA-issuing warp per team
 constexpr int kCH = 64;                 // atoms per chunk
 constexpr int kGE = 16;                 // edge slots per group
 constexpr int kMaxGroups = kCH * (512 / kGE);
 constexpr int kRecBufs = 4;             // tiles of record groups in flight
+constexpr int kBars = 4 + kRecBufs;     // mbarriers per team
 
 template <bool BWD> struct Cfg {
     static constexpr int NT = BWD ? 32 : 64;                // edges per tile
@@ -64,9 +65,10 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     constexpr int GPT = C::GPT, NT = C::NT, NCOLS = C::NCOLS, SEG = C::SEG, RECF = C::RecFloats;
     constexpr int KPT = BWD ? 8 : 16;                  // radial basis functions per staging thread
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t mbar[4 * kTeams];
+    __shared__ __align__(8) uint64_t mbar[kBars * kTeams];
     __shared__ uint32_t tmem_base_s;
     __shared__ int next_chunk, s_chunk[kTeams];
+    __shared__ volatile int s_done[kTeams];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, team = tid >> 7, tt = tid & (kTT - 1), wq = warp & 3;
 
     {   // resident A operand images (canonical K-major layout); every other operand buffer starts as zeros
@@ -81,11 +83,13 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     }
     if (tid == 0) {
         for (int t = 0; t < kTeams; ++t) {
-            mbar_init(smem_u32(&mbar[4 * t]), 1); mbar_init(smem_u32(&mbar[4 * t + 1]), 1);           // MMA1 / MMA2 complete
-            mbar_init(smem_u32(&mbar[4 * t + 2]), kTT); mbar_init(smem_u32(&mbar[4 * t + 3]), kTT);   // B1 / B2 written by everyone
+            mbar_init(smem_u32(&mbar[kBars * t]), 1); mbar_init(smem_u32(&mbar[kBars * t + 1]), 1);           // MMA1 / MMA2 complete
+            mbar_init(smem_u32(&mbar[kBars * t + 2]), kTT); mbar_init(smem_u32(&mbar[kBars * t + 3]), kTT);   // B1 / B2 written by everyone
+            for (int r = 0; r < kRecBufs; ++r) mbar_init(smem_u32(&mbar[kBars * t + 4 + r]), NT * 2);         // record copies landed
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
         next_chunk = 0;
+        for (int t = 0; t < kTeams; ++t) s_done[t] = 0;
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
@@ -96,6 +100,35 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     __syncthreads();
     tc_fence_after();
 
+    if (warp >= kTeams * 4) {
+        // ---- MMA warps: warp 16 + k issues the contractions of team k.  A team's requests strictly alternate
+        // (D1 = W_f1 B1, D2 = W_f2 B2, D1, ...); "done" arrives as a D1 request with the team's flag set.
+        if (lane == 0) {
+            const int tm = warp - kTeams * 4;
+            const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + C::W1Bytes);
+            const uint32_t sB2 = smem_u32(smem + C::W1Bytes + C::W2Bytes + tm * C::TeamBytes), sB1 = sB2 + C::B2Bytes;
+            const uint32_t bar1 = smem_u32(&mbar[kBars * tm]), bar2 = bar1 + 8, rdy1 = bar1 + 16, rdy2 = bar1 + 24;
+            const uint32_t tmem1 = tmem_base_s + (uint32_t)(tm * 128), tmem2 = tmem1 + 64;
+            const uint32_t idesc1 = make_idesc(128, NCOLS, 0), idesc2 = make_idesc(128, NCOLS, 1);
+            uint32_t ph = 0;
+            for (;;) {
+                mbar_wait(rdy1, ph);
+                if (s_done[tm]) break;
+                tc_fence_after();
+#pragma unroll
+                for (int k16 = 0; k16 < kR / 16; ++k16)
+                    umma(tmem1, make_desc(sW1 + k16 * 256, 128, 512), make_desc(sB1 + k16 * 256, 128, 512), idesc1, k16 > 0);
+                umma_commit(bar1);
+                mbar_wait(rdy2, ph);
+                tc_fence_after();
+#pragma unroll
+                for (int k16 = 0; k16 < kF / 16; ++k16)
+                    umma(tmem2, make_desc(sW2 + k16 * 256, 128, 2048), make_desc(sB2 + k16 * 256, 128, 2048), idesc2, k16 > 0);
+                umma_commit(bar2);
+                ph ^= 1u;
+            }
+        }
+    } else {
     uint8_t* const tb = smem + C::W1Bytes + C::W2Bytes + team * C::TeamBytes;
     uint8_t* const B2 = tb;                                            // [NCOLS][128 k] MN-major
     uint8_t* const B1 = B2 + C::B2Bytes;                               // [NCOLS][32 k] K-major
@@ -108,14 +141,13 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     float* const fpart = reinterpret_cast<float*>(gatom + kMaxGroups);
     uint8_t* const stage_w = stage + wq * (NT * SEG);
     uint8_t* const own_w = own + wq * (GPT * 128);
-    const uint32_t sW1 = smem_u32(smem), sW2 = smem_u32(smem + C::W1Bytes), sB1 = smem_u32(B1), sB2 = smem_u32(B2);
-    const uint32_t bar1 = smem_u32(&mbar[4 * team]), bar2 = bar1 + 8, rdy1 = bar1 + 16, rdy2 = bar1 + 24;
+    const uint32_t bar1 = smem_u32(&mbar[kBars * team]), bar2 = bar1 + 8, rdy1 = bar1 + 16, rdy2 = bar1 + 24, recf = bar1 + 32;
     const uint32_t sStageW = smem_u32(stage_w), sOwnW = smem_u32(own_w), sRecs = smem_u32(recs);
     const uint32_t tmem1 = tmem_base_s + (uint32_t)(team * 128), tmem2 = tmem1 + 64;             // D1, D2 accumulators
     const uint32_t lane_sel = (uint32_t)(wq * 32) << 16;
     const uint32_t tl1 = tmem1 + lane_sel, tl2 = tmem2 + lane_sel;
-    const uint32_t idesc1 = make_idesc(128, NCOLS, 0), idesc2 = make_idesc(128, NCOLS, 1);
-    uint32_t phase1 = 0, phase2 = 0, phr1 = 0, phr2 = 0;
+    uint32_t phase1 = 0, phase2 = 0;
+    uint32_t gt0 = 0;                                  // tiles this team has processed (record buffers and their mbarrier phases follow it)
     const int n = a.n;
     // staging role: edge sn of the tile, basis functions k0 .. k0 + KPT - 1; the 8 lanes of a quarter warp own 8 consecutive edges
     const int sn = BWD ? 8 * wq + (lane & 7) : 16 * wq + (lane & 7) + 8 * ((lane >> 3) & 1);
@@ -129,7 +161,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         if (tt == 0) s_chunk[team] = atomicAdd(&next_chunk, 1);
         team_bar(team);
         const int chunk = blockIdx.x + s_chunk[team] * gridDim.x;
-        if (chunk >= nchunks) break;
+        if (chunk >= nchunks) { if (tt == 0) s_done[team] = 1; mbar_arrive(rdy1); break; }
         const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
         const int g0 = b * n + ci * kCH;                               // first feature row of the chunk
         const int natoms = min(kCH, n - ci * kCH);
@@ -146,11 +178,13 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         const int G = pref[kCH];                                       // groups of the chunk
         const int ntiles = (G + GPT - 1) / GPT;
 
-        // asynchronous copy of the record groups of tile t into buffer t % kRecBufs (zeros for groups behind the chunk's end)
+        // asynchronous copy of the record groups of tile t into buffer (gt0 + t) % kRecBufs (zeros for groups behind the
+        // chunk's end); the buffer's mbarrier completes when every copying thread's piece has landed
         auto fetch_records = [&](int t) {
             if (tt < NT * 2) {
                 const int gs = tt >> 5, chunk16 = tt & 31;             // group of the tile, 16-byte piece of its 512-byte block
                 const int gl = t * GPT + gs;
+                const uint32_t buf = (gt0 + (uint32_t)t) & (kRecBufs - 1);
                 const float* src = a.recs;
                 uint32_t bytes = 0;
                 if (gl < G) {
@@ -158,13 +192,18 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
                     src = a.recs + lsd_rec_index((size_t)(g0 + at), a.cap, (gl - pref[at]) * kGE, 0);
                     bytes = 16;
                 }
-                cp_async16(sRecs + (uint32_t)(((t & (kRecBufs - 1)) * RECF + gs * LSD_REC_GROUP_FLOATS) * 4 + chunk16 * 16),
+                cp_async16(sRecs + (uint32_t)((buf * RECF + gs * LSD_REC_GROUP_FLOATS) * 4 + chunk16 * 16),
                            reinterpret_cast<const uint8_t*>(src) + chunk16 * 16, bytes);
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(recf + buf * 8) : "memory");
             }
+        };
+        auto wait_records = [&](int t) {                               // records of tile t are in shared memory
+            const uint32_t g = gt0 + (uint32_t)t;
+            mbar_wait(recf + (g & (kRecBufs - 1)) * 8, (g / kRecBufs) & 1u);
         };
         // radial basis (M1) of tile t -> B1, K-major: (n, k) at (n/8)*512 + (k/8)*128 + (n%8)*16 + (k%8)*2
         auto stage_basis = [&](int t) {
-            const float r = recs[(t & (kRecBufs - 1)) * RECF + srec + LSD_REC_R * 16];
+            const float r = recs[((gt0 + t) & (kRecBufs - 1)) * RECF + srec + LSD_REC_R * 16];
             uint32_t gv[KPT / 2], gt[KPT / 2];
             const f32x2 c22 = pk2(c2, c2), nid = pk2(-a.inv_delta2, -a.inv_delta2);
 #pragma unroll
@@ -186,24 +225,15 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
                 for (int kc = 0; kc < KPT / 8; ++kc) *reinterpret_cast<uint4*>(dt + kc * 128) = make_uint4(gt[4 * kc], gt[4 * kc + 1], gt[4 * kc + 2], gt[4 * kc + 3]);
             }
         };
-        // everybody: "my part of B1 is written and I am done reading D1"; the issuing thread waits for all and issues D1 = W_f1 B1
+        // everybody: "my part of B1 is written and I am done reading D1"; the MMA warp waits for all and issues D1 = W_f1 B1
         auto publish_b1_and_mma1 = [&]() {
             tc_fence_before();
             fence_async_smem();
             mbar_arrive(rdy1);
-            if (tt == 0) {
-                mbar_wait(rdy1, phr1);
-                tc_fence_after();
-#pragma unroll
-                for (int k16 = 0; k16 < kR / 16; ++k16)
-                    umma(tmem1, make_desc(sW1 + k16 * 256, 128, 512), make_desc(sB1 + k16 * 256, 128, 512), idesc1, k16 > 0);
-                umma_commit(bar1);
-            }
-            phr1 ^= 1u;
         };
         // this warp's 32-channel segment of the bf16 feature rows of tile t (and of the groups' own rows) -> gather stage
         auto issue_gathers = [&](int t) {
-            const float* rj = recs + (t & (kRecBufs - 1)) * RECF + LSD_REC_JROW * 16;
+            const float* rj = recs + ((gt0 + t) & (kRecBufs - 1)) * RECF + LSD_REC_JROW * 16;
             if (BWD) {
 #pragma unroll
                 for (int i = 0; i < NT / 4; ++i) {
@@ -250,12 +280,18 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         if (ntiles > 0) fetch_records(0);
         if (ntiles > 1) fetch_records(1);
         cp_async_commit();
-        cp_async_wait_all();
-        team_bar(team);
-        if (ntiles > 0) { stage_basis(0); publish_b1_and_mma1(); }
+        if (ntiles > 0) { wait_records(0); stage_basis(0); publish_b1_and_mma1(); }
 
         for (int t = 0; t < ntiles; ++t) {
             const int ng = min(GPT, G - t * GPT);                      // groups of this tile
+            // This warp is done with the epilogue of tile t-1, so its gather stage is free.  Record buffer (t+2) % 4 was last
+            // read by the epilogue of tile t-2, which every warp of the team finished before it signalled B2(t-1) ready, i.e.
+            // before MMA2(t-1) completed, which this warp has waited for.
+            wait_records(t);
+            issue_gathers(t);                                          // land under the activation, MMA2(t) and the staging of tile t+1
+            cp_async_commit();
+            if (t + 2 < ntiles) fetch_records(t + 2);
+            cp_async_commit();                                         // (possibly empty) most recent group: not waited for below
             // ---- activation (M3) of tile t: D1 -> B2, MN-major: (n, k) at (n/8)*2048 + (k/8)*128 + (k%8)*16 + (n%8)*2, k = this thread's row
             mbar_wait(bar1, phase1); phase1 ^= 1u;
             tc_fence_after();
@@ -294,26 +330,14 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
             tc_fence_before();
             fence_async_smem();
             mbar_arrive(rdy2);                                         // my rows of B2 are written, I am done with D1 (and, earlier, with D2 of tile t-1)
-            if (tt == 0) {
-                mbar_wait(rdy2, phr2);
-                tc_fence_after();
-#pragma unroll
-                for (int k16 = 0; k16 < kF / 16; ++k16)
-                    umma(tmem2, make_desc(sW2 + k16 * 256, 128, 2048), make_desc(sB2 + k16 * 256, 128, 2048), idesc2, k16 > 0);
-                umma_commit(bar2);
-            }
-            phr2 ^= 1u;
-            issue_gathers(t);                                          // land under MMA2(t) and the staging of tile t+1
-            if (t + 2 < ntiles) fetch_records(t + 2);                  // buffer (t+2) % 4 was last read by the epilogue of tile t-2
-            cp_async_commit();
             // ---- radial basis and MMA1 of tile t+1 (its records arrived an iteration ago) while MMA2(t) runs
-            if (t + 1 < ntiles) { stage_basis(t + 1); publish_b1_and_mma1(); }
+            if (t + 1 < ntiles) { wait_records(t + 1); stage_basis(t + 1); publish_b1_and_mma1(); }
             // ---- epilogue of tile t: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
-            cp_async_wait_all();
-            team_bar(team);                                            // the team's copies (gathered rows, records of tile t+2) are visible
+            asm volatile("cp.async.wait_group 1;" ::: "memory");        // this thread's gathers of tile t have landed
+            __syncwarp();                                              // ... and the rest of the warp's (a warp gathers only what it reads)
             mbar_wait(bar2, phase2); phase2 ^= 1u;
             tc_fence_after();
-            const float* rt = recs + (t & (kRecBufs - 1)) * RECF;
+            const float* rt = recs + ((gt0 + t) & (kRecBufs - 1)) * RECF;
             for (int gq = 0; gq < ng; ++gq) {
                 const int c0 = gq * kGE;
                 const int at = gatom[t * GPT + gq];
@@ -366,6 +390,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
             tc_fence_before();
         }
         flush();
+        gt0 += (uint32_t)ntiles;
         if (BWD) {
             team_bar(team);
             if (tt < natoms && cnts[tt] > 0) {
@@ -378,6 +403,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
                 Fb[i] += sx; Fb[n + i] += sy; Fb[2 * n + i] += sz;
             }
         }
+    }
     }
     tc_fence_before();
     __syncthreads();
