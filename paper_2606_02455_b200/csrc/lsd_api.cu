@@ -127,6 +127,22 @@ lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
             TRY(upload(ctx, &a, p1.data(), p1.size())); TRY(upload(ctx, &b2, p2.data(), p2.size()));
             d.Wf1_bf16[t] = a; d.Wf2_bf16[t] = b2;
         }
+        if (F == 128) {                                                  // atom-wise layers on the tensor cores
+            d.Win_tc.resize(T); d.WinT_tc.resize(T); d.Wo1_tc.resize(T); d.Wo1T_tc.resize(T); d.Wo2_tc.resize(T); d.Wo2T_tc.resize(T);
+            auto upk = [&](const double* W, bool tr, void** out) -> lsd_status {
+                tc_pack_square128(W, tr, p1);
+                uint16_t* dev = nullptr;
+                TRY(upload(ctx, &dev, p1.data(), p1.size()));
+                *out = dev;
+                return LSD_OK;
+            };
+            for (int t = 0; t < T; ++t) {
+                const double* Win = blk + t * per_block; const double* Wo1 = Win + (size_t)2 * F * F + (size_t)F * R; const double* Wo2 = Wo1 + (size_t)F * F;
+                TRY(upk(Win, false, &d.Win_tc[t])); TRY(upk(Win, true, &d.WinT_tc[t]));
+                TRY(upk(Wo1, false, &d.Wo1_tc[t])); TRY(upk(Wo1, true, &d.Wo1T_tc[t]));
+                TRY(upk(Wo2, false, &d.Wo2_tc[t])); TRY(upk(Wo2, true, &d.Wo2T_tc[t]));
+            }
+        }
     }
     const double* Wr1 = blk + (size_t)T * per_block;
     TRY(up(Wr1, F / 2, F, false, &d.Wr1));
@@ -183,7 +199,7 @@ lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
         w.y16.resize(net.T);
         for (int t = 0; t < net.T; ++t) TRY(dalloc(ctx, &w.y16[t], e));
         TRY(dalloc(ctx, &w.mbar16, e));
-        if (net.F == 128) TRY(dalloc(ctx, &w.ym16, e));
+        if (net.F == 128) { TRY(dalloc(ctx, &w.ym16, e)); TRY(dalloc(ctx, &w.ytab, (size_t)net.ns * net.F)); }
     }
     return LSD_OK;
 }

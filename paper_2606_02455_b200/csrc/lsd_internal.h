@@ -42,6 +42,8 @@ struct MlipDev {
     float* wr2 = nullptr;                       // [F/2]
     // bf16 copies for the tcgen05 path (K-major operands), filled when precision == LSD_BF16_TC
     std::vector<void*> Wf1_bf16, Wf2_bf16;
+    // width 128: bf16 A operand images of the atom-wise layers and their transposes (mlip_atom_tc128.cu)
+    std::vector<void*> Win_tc, WinT_tc, Wo1_tc, Wo1T_tc, Wo2_tc, Wo2T_tc;
 };
 
 struct PotDev {
@@ -105,6 +107,7 @@ struct MlipWork {                    // activations of one batched evaluation (k
     std::vector<uint16_t*> y16;      // [T] bf16 copies of y gathered by the tcgen05 edge kernels (LSD_BF16_TC only)
     uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
     uint32_t* ym16 = nullptr;        // width 128 only: rows of (y, mbar) bf16 pairs gathered by the backward tcgen05 kernel
+    float* ytab = nullptr;           // width 128: [ns][F] y of the first block per species
     double* e_atom = nullptr;        // [bmax*n]
 };
 
@@ -179,6 +182,8 @@ struct EdgeArgs {
     const uint16_t *y16 = nullptr, *mbar16 = nullptr;   // bf16 rows gathered by the tcgen05 kernels
     const uint32_t* ym16 = nullptr;   // [total][F] (y | mbar << 16) bf16 pairs, width-128 backward kernel
     float* m_out;                     // FWD: m
+    uint16_t* m16_out = nullptr;      // FWD, width 128: m as bf16 rows instead of m_out
+    uint16_t* ybar16_out = nullptr;   // BWD, width 128: ybar as bf16 rows instead of ybar
     const float* mbar; float* ybar;   // BWD
     double* Fout;                     // BWD: [B][3][n], accumulated
 };
@@ -187,6 +192,8 @@ struct EdgeArgs {
 void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                 const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);
 size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
+void launch_readout(Launcher L, int F, int total, float alpha, const float* x, const float* Wr1, const float* wr2, float* xbar,
+                    uint16_t* xbar16 /*optional bf16 copy*/, double* e_atom);
 
 // ---- mlip_tc.cu (bf16 tcgen05 filter path)
 bool mlip_tc_supported(const MlipDev& net);
@@ -196,3 +203,8 @@ void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // ml
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                   const int* img, const CompactList& cl, double* F, double* e_atom);
+
+// ---- mlip_atom_tc128.cu (width 128: atom-wise layers on the tensor cores, whole bf16 network driver)
+void tc_pack_square128(const double* W, bool transpose, std::vector<uint16_t>& out);
+void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                 const int* img, const CompactList& cl, double* F, double* e_atom);

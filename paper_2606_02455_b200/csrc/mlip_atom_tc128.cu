@@ -1,0 +1,376 @@
+// Atom-wise layers of the width-128 network on the tensor cores (bf16 operands, fp32 accumulation in TMEM), fused into one
+// chain kernel per interaction block and direction (M5, M9):
+//
+//   forward  block t : h = W_o1 m ;  x += W_o2 ssp(h) ;  y' = W_in(t+1) x                       (k_atom_tc128<FWD3 / FWD2>)
+//   backward block t : xbar += W_in(t+1)^T ybar ;  hbar = logistic(h) . W_o2^T xbar ;  mbar = W_o1^T hbar
+//                                                                                             (k_atom_tc128<BWD3 / BWD2>)
+//
+// "Channels are rows", as in the edge kernels: D[128 channels x NT atoms] = W[128 x 128] B[128 x NT]; TMEM lane = channel =
+// thread, TMEM column = atom, so every global access of an epilogue is one coalesced 128-byte (fp32) or 64-byte (bf16)
+// run per warp and atom.  The B operand of the first contraction is the bf16 row block of NT atoms, copied by cp.async
+// straight into the K-major core-matrix layout (a 16-byte piece = 8 channels of one atom = one core-matrix row); the B
+// operands of the following contractions are written by the epilogue threads in the MN-major layout (8 atoms = 16 bytes
+// per thread).  These layers are HBM-bound (2 KB of traffic per atom against 3 x 32 kflop): the design goal is memory
+// concurrency -- 4 teams per SM, a 3-deep cp.async ring per team, fp32 residual rows pre-loaded before the wait on the
+// contraction they are added to.
+#include <algorithm>
+#include <vector>
+#include "lsd_internal.h"
+#include "tc_ptx.cuh"
+
+namespace {
+using namespace tcp;
+
+constexpr int kF = 128;
+constexpr int kTeams = 4;
+constexpr int kTT = 128;                               // threads per team = channels
+constexpr int kThreads = kTeams * kTT + kTeams * 32;   // + one MMA-issuing warp per team
+constexpr int kNT = 32;                                // atoms per tile
+constexpr int kRing = 3;                               // tiles of the first operand in flight per team
+constexpr int kWBytes = kF * kF * 2;
+constexpr int kBBytes = kNT * kF * 2;
+constexpr int kTeamBytes = (kRing + 1) * kBBytes;
+constexpr int kSmem = 3 * kWBytes + kTeams * kTeamBytes;
+constexpr int kBars = 5 + kRing;                       // per team: 3 x "contraction complete", 2 x "operand written", ring slots
+static_assert(kSmem + 1024 <= 227 * 1024, "shared memory budget");
+
+enum AtomMode { FWD3 = 0, FWD2 = 1, BWD3 = 2, BWD2 = 3 };
+
+struct AtomArgs {
+    int total;                    // rows (states x atoms)
+    const uint16_t* in16;         // [total][128] bf16: m (forward), ybar (BWD3), xbar (BWD2)
+    const void* W[3];             // A operand images of the (up to) three contractions
+    float* h;                     // forward: written; backward: read
+    float* x;                     // forward: x, read and written; BWD3: xbar, read and written
+    uint16_t* y16_out;            // FWD3: y of the next block
+    const uint16_t* y16;          // backward: y of the block
+    uint32_t* ym16;               // backward: (y, mbar) bf16 pairs gathered by the backward edge kernel
+};
+
+constexpr float kLn2 = 0.69314718055994530942f;
+__device__ __forceinline__ float ssp_f(float x) { return fmaxf(x, 0.f) + __logf(1.f + __expf(-fabsf(x))) - kLn2; }
+__device__ __forceinline__ float logistic_f(float x) { return __fdividef(1.f, 1.f + __expf(-x)); }
+
+template <int MODE>
+__global__ void __launch_bounds__(kThreads, 1)
+k_atom_tc128(AtomArgs a)
+{
+    constexpr bool FWD = MODE == FWD3 || MODE == FWD2;
+    constexpr bool HAS0 = MODE != BWD2, HAS2 = MODE != FWD2;
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t mbar[kBars * kTeams];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    for (int s = 0; s < 3; ++s) {
+        if (a.W[s] == nullptr) continue;
+        const uint4* src = reinterpret_cast<const uint4*>(a.W[s]);
+        uint4* dst = reinterpret_cast<uint4*>(smem + s * kWBytes);
+        for (int i = tid; i < kWBytes / 16; i += kThreads) dst[i] = src[i];
+    }
+    if (tid == 0) {
+        for (int t = 0; t < kTeams; ++t) {
+            for (int b = 0; b < 3; ++b) mbar_init(smem_u32(&mbar[kBars * t + b]), 1);
+            for (int b = 3; b < kBars; ++b) mbar_init(smem_u32(&mbar[kBars * t + b]), kTT);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+
+    const int team = warp >= kTeams * 4 ? warp - kTeams * 4 : warp >> 2;
+    const int ntiles = (a.total + kNT - 1) / kNT;
+    const int first = blockIdx.x * kTeams + team, stride = gridDim.x * kTeams;
+    const int cnt = first < ntiles ? (ntiles - first + stride - 1) / stride : 0;
+    const uint32_t sW = smem_u32(smem);
+    const uint32_t sRing = smem_u32(smem + 3 * kWBytes + team * kTeamBytes), sB2 = sRing + kRing * kBBytes;
+    const uint32_t bar0 = smem_u32(&mbar[kBars * team]), rdy1 = bar0 + 24, rdy2 = bar0 + 32, full = bar0 + 40;
+    const uint32_t tD = tmem_base_s + (uint32_t)(team * 128);                  // D0, D1, D2 at columns +0, +32, +64
+
+    if (warp >= kTeams * 4) {
+        // ---- MMA warp of the team: contractions in order, each as soon as its B operand is published
+        if (lane == 0) {
+            const uint32_t idK = make_idesc(128, kNT, 0), idMN = make_idesc(128, kNT, 1);
+            uint32_t ph = 0;
+            for (int i = 0; i < cnt; ++i) {
+                const uint32_t sB1 = sRing + (uint32_t)(i % kRing) * kBBytes;
+                mbar_wait(full + (uint32_t)(i % kRing) * 8, (uint32_t)(i / kRing) & 1u);
+                tc_fence_after();
+                if (HAS0) {
+#pragma unroll
+                    for (int k16 = 0; k16 < kF / 16; ++k16)
+                        umma(tD, make_desc(sW + k16 * 256, 128, 2048), make_desc(sB1 + k16 * 256, 128, 2048), idK, k16 > 0);
+                    umma_commit(bar0);
+                    mbar_wait(rdy1, ph);
+                    tc_fence_after();
+#pragma unroll
+                    for (int k16 = 0; k16 < kF / 16; ++k16)
+                        umma(tD + 32, make_desc(sW + kWBytes + k16 * 256, 128, 2048), make_desc(sB2 + k16 * 256, 128, 2048), idMN, k16 > 0);
+                    umma_commit(bar0 + 8);
+                } else {
+#pragma unroll
+                    for (int k16 = 0; k16 < kF / 16; ++k16)
+                        umma(tD + 32, make_desc(sW + kWBytes + k16 * 256, 128, 2048), make_desc(sB1 + k16 * 256, 128, 2048), idK, k16 > 0);
+                    umma_commit(bar0 + 8);
+                }
+                if (HAS2) {
+                    mbar_wait(rdy2, ph);
+                    tc_fence_after();
+#pragma unroll
+                    for (int k16 = 0; k16 < kF / 16; ++k16)
+                        umma(tD + 64, make_desc(sW + 2 * kWBytes + k16 * 256, 128, 2048), make_desc(sB2 + k16 * 256, 128, 2048), idMN, k16 > 0);
+                    umma_commit(bar0 + 16);
+                }
+                ph ^= 1u;
+            }
+        }
+    } else {
+        const int tt = tid & (kTT - 1), wq = warp & 3;
+        uint8_t* const B2 = smem + 3 * kWBytes + team * kTeamBytes + kRing * kBBytes;
+        const uint32_t tl = tD + ((uint32_t)(wq * 32) << 16);
+        // cp.async piece of this thread in iteration i: atom 8 i + (lane & 7), channels 8 kc .. 8 kc + 7, kc = 4 wq + (lane >> 3):
+        // a warp instruction covers 8 atoms x 64 bytes (full 32-byte sectors) and 8 distinct 16-byte bank groups
+        const int pn = lane & 7, kc = 4 * wq + (lane >> 3);
+        auto fetch = [&](int i) {
+            if (i < cnt) {
+                const int row0 = (first + i * stride) * kNT;
+                const uint32_t dst = sRing + (uint32_t)(i % kRing) * kBBytes + (uint32_t)(kc * 128 + pn * 16);
+#pragma unroll
+                for (int g = 0; g < kNT / 8; ++g) {
+                    const int row = row0 + 8 * g + pn;
+                    const bool ok = row < a.total;
+                    cp_async16(dst + g * 2048, a.in16 + (size_t)(ok ? row : 0) * kF + kc * 8, ok ? 16u : 0u);
+                }
+            }
+            cp_async_commit();
+        };
+        fetch(0);
+        fetch(1);
+        uint32_t ph = 0;
+        for (int i = 0; i < cnt; ++i) {
+            const int row0 = (first + i * stride) * kNT;
+            const size_t base = (size_t)row0 * kF + tt;
+            const int nrow = min(kNT, a.total - row0);
+            fetch(i + 2);
+            float pre[kNT];                                    // fp32 rows added to / multiplied with the next accumulator
+            if (MODE == BWD3) {
+#pragma unroll
+                for (int c = 0; c < kNT; ++c) pre[c] = c < nrow ? a.x[base + (size_t)c * kF] : 0.f;
+            }
+            asm volatile("cp.async.wait_group 2;" ::: "memory");    // this thread's pieces of tile i have landed
+            fence_async_smem();
+            tc_fence_before();
+            mbar_arrive(full + (uint32_t)(i % kRing) * 8);
+
+            if (HAS0) {   // ---- epilogue of the first contraction
+                mbar_wait(bar0, ph);
+                tc_fence_after();
+#pragma unroll
+                for (int c0 = 0; c0 < kNT; c0 += 16) {
+                    uint32_t v[16], pk[8];
+                    tmem_ld16(tl + c0, v);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 16; c += 2) {
+                        float o0, o1;
+                        if (FWD) {             // h kept for the backward; operand = ssp(h)
+                            const float h0 = __uint_as_float(v[c]), h1 = __uint_as_float(v[c + 1]);
+                            if (c0 + c < nrow) a.h[base + (size_t)(c0 + c) * kF] = h0;
+                            if (c0 + c + 1 < nrow) a.h[base + (size_t)(c0 + c + 1) * kF] = h1;
+                            o0 = ssp_f(h0); o1 = ssp_f(h1);
+                        } else {               // xbar += W_in^T ybar; operand = xbar
+                            o0 = pre[c0 + c] + __uint_as_float(v[c]); o1 = pre[c0 + c + 1] + __uint_as_float(v[c + 1]);
+                            if (c0 + c < nrow) a.x[base + (size_t)(c0 + c) * kF] = o0;
+                            if (c0 + c + 1 < nrow) a.x[base + (size_t)(c0 + c + 1) * kF] = o1;
+                        }
+                        pk[c >> 1] = pack_bf16(o0, o1);
+                    }
+                    uint8_t* d = B2 + (c0 >> 3) * 2048 + tt * 16;
+                    *reinterpret_cast<uint4*>(d) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                    *reinterpret_cast<uint4*>(d + 2048) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+                }
+                tc_fence_before();
+                fence_async_smem();
+                mbar_arrive(rdy1);
+            }
+            {   // ---- epilogue of the second contraction
+                const float* src = FWD ? a.x : a.h;
+#pragma unroll
+                for (int c = 0; c < kNT; ++c) pre[c] = c < nrow ? src[base + (size_t)c * kF] : 0.f;
+                mbar_wait(bar0 + 8, ph);
+                tc_fence_after();
+#pragma unroll
+                for (int c0 = 0; c0 < kNT; c0 += 16) {
+                    uint32_t v[16], pk[8];
+                    tmem_ld16(tl + 32 + c0, v);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 16; c += 2) {
+                        float o0, o1;
+                        if (FWD) {             // x += W_o2 ssp(h)
+                            o0 = pre[c0 + c] + __uint_as_float(v[c]); o1 = pre[c0 + c + 1] + __uint_as_float(v[c + 1]);
+                            if (c0 + c < nrow) a.x[base + (size_t)(c0 + c) * kF] = o0;
+                            if (c0 + c + 1 < nrow) a.x[base + (size_t)(c0 + c + 1) * kF] = o1;
+                        } else {               // hbar = logistic(h) . W_o2^T xbar
+                            o0 = logistic_f(pre[c0 + c]) * __uint_as_float(v[c]); o1 = logistic_f(pre[c0 + c + 1]) * __uint_as_float(v[c + 1]);
+                        }
+                        pk[c >> 1] = pack_bf16(o0, o1);
+                    }
+                    if (HAS2) {
+                        uint8_t* d = B2 + (c0 >> 3) * 2048 + tt * 16;
+                        *reinterpret_cast<uint4*>(d) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                        *reinterpret_cast<uint4*>(d + 2048) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+                    }
+                }
+                tc_fence_before();
+                if (HAS2) { fence_async_smem(); mbar_arrive(rdy2); }
+            }
+            if (HAS2) {   // ---- epilogue of the third contraction
+                uint16_t yv[kNT];
+                if (!FWD) {
+#pragma unroll
+                    for (int c = 0; c < kNT; ++c) yv[c] = c < nrow ? a.y16[base + (size_t)c * kF] : (uint16_t)0;
+                }
+                mbar_wait(bar0 + 16, ph);
+                tc_fence_after();
+#pragma unroll
+                for (int c0 = 0; c0 < kNT; c0 += 16) {
+                    uint32_t v[16];
+                    tmem_ld16(tl + 64 + c0, v);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        if (c0 + c < nrow) {
+                            const __nv_bfloat16 b = __float2bfloat16_rn(__uint_as_float(v[c]));
+                            const uint16_t bits = *reinterpret_cast<const uint16_t*>(&b);
+                            if (FWD) a.y16_out[base + (size_t)(c0 + c) * kF] = bits;
+                            else a.ym16[base + (size_t)(c0 + c) * kF] = (uint32_t)yv[c0 + c] | ((uint32_t)bits << 16);
+                        }
+                    }
+                }
+                tc_fence_before();
+            }
+            ph ^= 1u;
+        }
+        cp_async_wait_all();
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
+}
+
+// y table of the first block: W_in(0) Emb[s] for every species (x(0) = Emb[s] does not depend on the positions)
+__global__ void k_ytab(int F, const float* __restrict__ emb, const float* __restrict__ WinT, float* __restrict__ ytab)
+{
+    const int s = blockIdx.x, c = threadIdx.x;
+    float acc = 0.f;
+    for (int k = 0; k < F; ++k) acc = fmaf(emb[s * F + k], WinT[k * F + c], acc);
+    ytab[s * F + c] = acc;
+}
+// x = Emb[s] (fp32) and y16 = bf16(W_in(0) Emb[s]); 4 channels per thread
+__global__ void k_embed_tc(int total, int n, const int* __restrict__ species, const float* __restrict__ emb, const float* __restrict__ ytab,
+                           float* __restrict__ x, uint16_t* __restrict__ y16)
+{
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (size_t)total * (kF / 4)) return;
+    const int g = (int)(t / (kF / 4)), f = (int)(t % (kF / 4)) * 4;
+    const int s = species[g % n];
+    const float4 e = *reinterpret_cast<const float4*>(emb + s * kF + f);
+    const float4 y = *reinterpret_cast<const float4*>(ytab + s * kF + f);
+    *reinterpret_cast<float4*>(x + (size_t)g * kF + f) = e;
+    *reinterpret_cast<uint2*>(y16 + (size_t)g * kF + f) = make_uint2(pack_bf16(y.x, y.y), pack_bf16(y.z, y.w));
+}
+
+int sm_count()
+{
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
+    return sms;
+}
+
+template <int MODE> void launch_atom(Launcher L, const AtomArgs& a)
+{
+    static bool configured = false;
+    if (!configured) { cudaFuncSetAttribute(k_atom_tc128<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem); configured = true; }
+    const int ntiles = (a.total + kNT - 1) / kNT;
+    const int grid = std::max(1, std::min(sm_count(), (ntiles + kTeams - 1) / kTeams));
+    const int pid = prof_begin(L, PROF_DENSE);
+    k_atom_tc128<MODE><<<grid, kThreads, kSmem, L.s>>>(a);
+    LSD_COUNT(L);
+    prof_end(L, pid);
+}
+
+uint16_t bf16_bits(double v)
+{
+    const __nv_bfloat16 b = __float2bfloat16_rn((float)v);
+    return *reinterpret_cast<const uint16_t*>(&b);
+}
+
+}  // namespace
+
+// host: A operand image of a 128 x 128 matrix W [out][in] (row-major fp64), or of its transpose:
+// (m, k) at byte (m/8)*2048 + (k/8)*128 + (m%8)*16 + (k%8)*2
+void tc_pack_square128(const double* W, bool transpose, std::vector<uint16_t>& out)
+{
+    out.assign((size_t)kF * kF, 0);
+    for (int m = 0; m < kF; ++m)
+        for (int k = 0; k < kF; ++k)
+            out[((size_t)(m / 8) * 2048 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_bits(transpose ? W[(size_t)k * kF + m] : W[(size_t)m * kF + k]);
+}
+
+// Width-128 bf16 tensor-core network: edge kernels of mlip_tc128.cu + the chain kernels above.  bf16 aliases of fp32 work
+// buffers that this path does not need: m16 in w.m, ybar16 in w.ybar, xbar16 in w.mbar.
+void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
+                                 const int* img, const CompactList& cl, double* Fout, double* e_atom)
+{
+    (void)q; (void)img;
+    const int total = B * sys.n, T = net.T;
+    uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
+    uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
+    uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
+    int pid = prof_begin(L, PROF_DENSE);
+    k_ytab<<<net.ns, kF, 0, L.s>>>(kF, net.emb, net.WinT[0], w.ytab); LSD_COUNT(L);
+    k_embed_tc<<<(int)(((size_t)total * (kF / 4) + 255) / 256), 256, 0, L.s>>>(total, sys.n, sys.species, net.emb, w.ytab, w.x, w.y16[0]); LSD_COUNT(L);
+    prof_end(L, pid);
+    EdgeArgs ea{};
+    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs;
+    ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
+    for (int t = 0; t < T; ++t) {
+        ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
+        pid = prof_begin(L, PROF_EDGE_FWD);
+        launch_edge_tc128(L, ea, false);
+        prof_end(L, pid);
+        AtomArgs aa{};
+        aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;
+        aa.W[0] = net.Wo1_tc[t]; aa.W[1] = net.Wo2_tc[t];
+        if (t + 1 < T) { aa.W[2] = net.Win_tc[t + 1]; aa.y16_out = w.y16[t + 1]; launch_atom<FWD3>(L, aa); }
+        else launch_atom<FWD2>(L, aa);
+    }
+    launch_readout(L, kF, total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, xbar16, e_atom);
+    ea.m16_out = nullptr;
+    for (int t = T - 1; t >= 0; --t) {
+        if (t == T - 1) {
+            AtomArgs aa{};
+            aa.total = total; aa.in16 = xbar16; aa.h = w.h[t]; aa.y16 = w.y16[t]; aa.ym16 = w.ym16;
+            aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t];
+            launch_atom<BWD2>(L, aa);
+        }
+        ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.ym16 = w.ym16;
+        ea.ybar16_out = t > 0 ? ybar16 : nullptr; ea.ybar = nullptr; ea.Fout = Fout;
+        pid = prof_begin(L, PROF_EDGE_BWD);
+        launch_edge_tc128(L, ea, true);
+        prof_end(L, pid);
+        if (t > 0) {
+            AtomArgs aa{};
+            aa.total = total; aa.in16 = ybar16; aa.x = w.xbar; aa.h = w.h[t - 1]; aa.y16 = w.y16[t - 1]; aa.ym16 = w.ym16;
+            aa.W[0] = net.WinT_tc[t]; aa.W[1] = net.Wo2T_tc[t - 1]; aa.W[2] = net.Wo1T_tc[t - 1];
+            launch_atom<BWD3>(L, aa);
+        }
+    }
+}

@@ -172,7 +172,9 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         if (tt < kCH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
         {   // atoms without neighbours: their sums are empty
             float* out = BWD ? a.ybar : a.m_out;
-            if (out) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * kF + tt] = 0.f;
+            uint16_t* out16 = BWD ? a.ybar16_out : a.m16_out;
+            if (out16) { for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out16[(size_t)(g0 + i) * kF + tt] = 0; }
+            else if (out) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * kF + tt] = 0.f;
         }
         team_bar(team);
         const int G = pref[kCH];                                       // groups of the chunk
@@ -263,9 +265,13 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
             float lo, hi;
             un2(part2, lo, hi);
             const float part = lo + hi;
-            if (!BWD) a.m_out[(size_t)(g0 + cur) * kF + tt] = part;
-            else {
-                if (a.ybar) a.ybar[(size_t)(g0 + cur) * kF + tt] = part;
+            const __nv_bfloat16 pb = __float2bfloat16_rn(part);
+            if (!BWD) {
+                if (a.m16_out) a.m16_out[(size_t)(g0 + cur) * kF + tt] = *reinterpret_cast<const uint16_t*>(&pb);
+                else a.m_out[(size_t)(g0 + cur) * kF + tt] = part;
+            } else {
+                if (a.ybar16_out) a.ybar16_out[(size_t)(g0 + cur) * kF + tt] = *reinterpret_cast<const uint16_t*>(&pb);
+                else if (a.ybar) a.ybar[(size_t)(g0 + cur) * kF + tt] = part;
                 float fx, fy, fz;
                 un2(fx2, lo, hi); fx = lo + hi; un2(fy2, lo, hi); fy = lo + hi; un2(fz2, lo, hi); fz = lo + hi;
 #pragma unroll
