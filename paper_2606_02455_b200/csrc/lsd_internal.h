@@ -199,6 +199,7 @@ void launch_readout(Launcher L, int F, int total, float alpha, const float* x, c
 bool mlip_tc_supported(const MlipDev& net);
 void launch_edge_tc(Launcher L, const EdgeArgs& a, int F, bool backward);
 void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_tc128.cu: width 128
+void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,

@@ -14,6 +14,7 @@
 // concurrency -- 4 teams per SM, a 3-deep cp.async ring per team, fp32 residual rows pre-loaded before the wait on the
 // contraction they are added to.
 #include <algorithm>
+#include <cstdlib>
 #include <vector>
 #include "lsd_internal.h"
 #include "tc_ptx.cuh"
@@ -331,6 +332,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
 {
     (void)q; (void)img;
     const int total = B * sys.n, T = net.T;
+    static const bool use_er = [] { const char* v = getenv("LSD_EDGE_ER"); return v == nullptr || v[0] != '0'; }();
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
@@ -344,7 +346,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        launch_edge_tc128(L, ea, false);
+        if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
         prof_end(L, pid);
         AtomArgs aa{};
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;
