@@ -184,7 +184,12 @@ lsd_status alloc_compact(lsd_ctx* ctx, CompactList& cl, int cap, int bmax, bool 
     cl.cap = cap; cl.bmax = bmax;
     TRY(dalloc(ctx, &cl.count, (size_t)ctx->sys.n * bmax));
     TRY(dalloc(ctx, &cl.keys, (size_t)ctx->sys.n * bmax * cap));
-    if (records) TRY(dalloc(ctx, &cl.recs, (size_t)ctx->sys.n * bmax * cap * 8));
+    if (records) {                                                     // + one zero group behind the last row (padding tiles of the tcgen05 kernels)
+        const size_t nrec = (size_t)ctx->sys.n * bmax * cap * 8;
+        TRY(dalloc(ctx, &cl.recs, nrec + LSD_REC_GROUP_FLOATS));
+        CK(cudaMemset(cl.recs + nrec, 0, LSD_REC_GROUP_FLOATS * sizeof(float)));
+        cl.rec_zero = cl.recs + nrec;
+    }
     return LSD_OK;
 }
 lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)

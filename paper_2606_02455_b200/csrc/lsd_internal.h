@@ -87,6 +87,7 @@ struct CompactList {                 // per-state exact list (r < rc), rows padd
     int* count = nullptr;            // [bmax*n]
     uint32_t* keys = nullptr;        // [bmax*n][cap]
     float* recs = nullptr;           // [bmax*n][cap/16][8][16], MLIP lists only (cap is a multiple of 16)
+    const float* rec_zero = nullptr; // one zero group behind the records
 };
 
 struct CellGrid {
@@ -175,6 +176,7 @@ void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B
 struct EdgeArgs {
     int total, n, cap;
     const int* count; const uint32_t* keys; const float* recs;
+    const float* rec_zero = nullptr;  // one all-zero record group (512 bytes) behind the records
     float rc, inv_rc, delta, inv_delta2;
     const float *Wf1, *Wf2;           // [R][F], [F][F] (k-major), fp32 path
     const void *Wf1_tc = nullptr, *Wf2_tc = nullptr;   // bf16, UMMA canonical K-major layouts (mlip_tc.cu)

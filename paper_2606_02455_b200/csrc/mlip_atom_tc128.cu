@@ -341,7 +341,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     k_embed_tc<<<(int)(((size_t)total * (kF / 4) + 255) / 256), 256, 0, L.s>>>(total, sys.n, sys.species, net.emb, w.ytab, w.x, w.y16[0]); LSD_COUNT(L);
     prof_end(L, pid);
     EdgeArgs ea{};
-    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs;
+    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs; ea.rec_zero = cl.rec_zero;
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;

@@ -94,7 +94,7 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
     if (tid == 0) {
         for (int t = 0; t < kTeams; ++t) {
             for (int b = 0; b < 3; ++b) mbar_init(smem_u32(&mbar[kBars * t + b]), 1);
-            for (int b = 3; b < kBars; ++b) mbar_init(smem_u32(&mbar[kBars * t + b]), kTeamThreads);
+            for (int b = 3; b < kBars; ++b) mbar_init(smem_u32(&mbar[kBars * t + b]), kTeamThreads / 32);   // one arrival per warp
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
     }
@@ -216,7 +216,7 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
 #pragma unroll
                 for (int kc = 0; kc < KH / 8; ++kc) *reinterpret_cast<uint4*>(a1row + (half * (KH / 8) + kc) * 128) = make_uint4(gv[4 * kc], gv[4 * kc + 1], gv[4 * kc + 2], gv[4 * kc + 3]);
                 fence_async_smem();
-                mbar_arrive(rdyA1);
+                warp_arrive(rdyA1, lane);
             };
 
             load_record(0);
@@ -261,7 +261,7 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
                 }
                 tc_fence_before();
                 fence_async_smem();
-                mbar_arrive(rdyA2);
+                warp_arrive(rdyA2, lane);
                 // ---- radial basis of tile t+1 while GEMM2 runs (A1 is free: GEMM1 of tile t is complete)
                 if (t + 1 < ntiles) stage_basis(r_n);
                 // ---- epilogue: P = bf16(w fc) . y_j, MN-major (8 channels of this edge = 16 bytes)
@@ -293,7 +293,7 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
                 at_prev = at;
                 tc_fence_before();
                 fence_async_smem();
-                mbar_arrive(rdyP);
+                warp_arrive(rdyP, lane);
                 ph ^= 1u;
             }
             // ---- sums of the chunk: D3[channel][atom] -> m (bf16 rows)
@@ -316,7 +316,7 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
         }
         if (e == 0 && half == 0) s_nt[team] = -1;
         team_bar(team);
-        mbar_arrive(rdyA1);
+        warp_arrive(rdyA1, lane);
     }
     tc_fence_before();
     __syncthreads();

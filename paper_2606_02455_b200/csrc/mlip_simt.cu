@@ -373,7 +373,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
     k_embed<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, w.x); LSD_COUNT(L);
     EdgeArgs ea{};
-    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs;
+    ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs; ea.rec_zero = cl.rec_zero;
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
     for (int t = 0; t < net.T; ++t) {
         int pid = prof_begin(L, PROF_DENSE);

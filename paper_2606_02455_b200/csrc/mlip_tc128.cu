@@ -84,8 +84,8 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     if (tid == 0) {
         for (int t = 0; t < kTeams; ++t) {
             mbar_init(smem_u32(&mbar[kBars * t]), 1); mbar_init(smem_u32(&mbar[kBars * t + 1]), 1);           // MMA1 / MMA2 complete
-            mbar_init(smem_u32(&mbar[kBars * t + 2]), kTT); mbar_init(smem_u32(&mbar[kBars * t + 3]), kTT);   // B1 / B2 written by everyone
-            for (int r = 0; r < kRecBufs; ++r) mbar_init(smem_u32(&mbar[kBars * t + 4 + r]), NT * 2);         // record copies landed
+            mbar_init(smem_u32(&mbar[kBars * t + 2]), kTT / 32); mbar_init(smem_u32(&mbar[kBars * t + 3]), kTT / 32);   // B1 / B2 written by every warp
+            for (int r = 0; r < kRecBufs; ++r) mbar_init(smem_u32(&mbar[kBars * t + 4 + r]), 1);              // record copies landed (byte count)
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
         next_chunk = 0;
@@ -161,7 +161,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         if (tt == 0) s_chunk[team] = atomicAdd(&next_chunk, 1);
         team_bar(team);
         const int chunk = blockIdx.x + s_chunk[team] * gridDim.x;
-        if (chunk >= nchunks) { if (tt == 0) s_done[team] = 1; mbar_arrive(rdy1); break; }
+        if (chunk >= nchunks) { if (tt == 0) s_done[team] = 1; team_bar(team); warp_arrive(rdy1, lane); break; }
         const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
         const int g0 = b * n + ci * kCH;                               // first feature row of the chunk
         const int natoms = min(kCH, n - ci * kCH);
@@ -180,23 +180,22 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         const int G = pref[kCH];                                       // groups of the chunk
         const int ntiles = (G + GPT - 1) / GPT;
 
-        // asynchronous copy of the record groups of tile t into buffer (gt0 + t) % kRecBufs (zeros for groups behind the
-        // chunk's end); the buffer's mbarrier completes when every copying thread's piece has landed
+        // bulk asynchronous copy of the record groups (512 bytes each) of tile t into buffer (gt0 + t) % kRecBufs, issued by one
+        // thread (a zero group for groups behind the chunk's end); the buffer's mbarrier completes on the byte count
         auto fetch_records = [&](int t) {
-            if (tt < NT * 2) {
-                const int gs = tt >> 5, chunk16 = tt & 31;             // group of the tile, 16-byte piece of its 512-byte block
-                const int gl = t * GPT + gs;
+            if (tt == 0) {
                 const uint32_t buf = (gt0 + (uint32_t)t) & (kRecBufs - 1);
-                const float* src = a.recs;
-                uint32_t bytes = 0;
-                if (gl < G) {
-                    const int at = gatom[gl];
-                    src = a.recs + lsd_rec_index((size_t)(g0 + at), a.cap, (gl - pref[at]) * kGE, 0);
-                    bytes = 16;
+                mbar_expect_tx(recf + buf * 8, GPT * LSD_REC_GROUP_FLOATS * 4);
+#pragma unroll
+                for (int gs = 0; gs < GPT; ++gs) {
+                    const int gl = t * GPT + gs;
+                    const float* src = a.rec_zero;
+                    if (gl < G) {
+                        const int at = gatom[gl];
+                        src = a.recs + lsd_rec_index((size_t)(g0 + at), a.cap, (gl - pref[at]) * kGE, 0);
+                    }
+                    bulk_g2s(sRecs + (uint32_t)((buf * RECF + gs * LSD_REC_GROUP_FLOATS) * 4), src, LSD_REC_GROUP_FLOATS * 4, recf + buf * 8);
                 }
-                cp_async16(sRecs + (uint32_t)((buf * RECF + gs * LSD_REC_GROUP_FLOATS) * 4 + chunk16 * 16),
-                           reinterpret_cast<const uint8_t*>(src) + chunk16 * 16, bytes);
-                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(recf + buf * 8) : "memory");
             }
         };
         auto wait_records = [&](int t) {                               // records of tile t are in shared memory
@@ -231,7 +230,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         auto publish_b1_and_mma1 = [&]() {
             tc_fence_before();
             fence_async_smem();
-            mbar_arrive(rdy1);
+            warp_arrive(rdy1, lane);
         };
         // this warp's 32-channel segment of the bf16 feature rows of tile t (and of the groups' own rows) -> gather stage
         auto issue_gathers = [&](int t) {
@@ -335,7 +334,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
             }
             tc_fence_before();
             fence_async_smem();
-            mbar_arrive(rdy2);                                         // my rows of B2 are written, I am done with D1 (and, earlier, with D2 of tile t-1)
+            warp_arrive(rdy2, lane);                                   // my rows of B2 are written, I am done with D1 (and, earlier, with D2 of tile t-1)
             // ---- radial basis and MMA1 of tile t+1 (its records arrived an iteration ago) while MMA2(t) runs
             if (t + 1 < ntiles) { wait_records(t + 1); stage_basis(t + 1); publish_b1_and_mma1(); }
             // ---- epilogue of tile t: cutoff, cfconv products and their adjoints; per-atom sums stay in this thread's registers
