@@ -29,6 +29,10 @@ sys.path.insert(0, ROOT)
 METRIC = "batched force-eval atom-steps/s (whole verified window; accepted target-exact MD steps/s beside it)"
 UNIT = "atom-steps/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from one `ncu --set full` capture of this
+# command (per workload and arithmetic type; null where no capture is committed): profiles/r1_edge_bwd_tc128_cfg5.md
+NCU_TRAFFIC = {("cfg5", "bf16"): 1.706460e9 + 0.144098e9}
+
 # bounded oracle samples: same per-atom cost as the full workload, sized for ~10-30 s of CPU work
 CPU_SAMPLES = {
     "cfg1": dict(kw={}, K=4, windows=4000),
@@ -173,33 +177,41 @@ def main():
             return None
         return ctx.window(K, stream)
 
+    def timed_pass():
+        """K timed windows, CUDA events on the launching stream around every window (L2 flush outside the events)."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for s in range(args.steps):
+            if need_flush:
+                with torch.cuda.stream(stream):
+                    flush.fill_(s & 0xFF)
+            ev[s][0].record(stream)
+            one_window()
+            ev[s][1].record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev)
+
     for _ in range(args.warmup):
         one_window()
     torch.cuda.synchronize()
     steps_before = P.lsd_get_stats(ctx.h)["committed_steps"]
     launches_before = P.lsd_launch_count(ctx.h)
-    P.lsd_profile(ctx.h, True)
     sampler = ClockSampler(local)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for s in range(args.steps):
-        if need_flush:
-            flush.fill_(s & 0xFF)
-        ev[s][0].record(stream)
-        one_window()
-        ev[s][1].record(stream)
-    torch.cuda.synchronize()
+    ms = timed_pass()                                   # the reported value: no per-kernel events, CUDA graphs replayed
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop()
-    ms = sum(a.elapsed_time(b) for a, b in ev)
-    prof = P.lsd_get_profile(ctx.h)
-    P.lsd_profile(ctx.h, False)
     launches = P.lsd_launch_count(ctx.h) - launches_before
     committed = P.lsd_get_stats(ctx.h)["committed_steps"] - steps_before
+    # second, identically configured pass of K windows with the library's per-kernel CUDA events on (they bypass graph
+    # replay and cost ~2 us per launch, which is why the value above is not taken from this pass): stage times, roofline
+    P.lsd_profile(ctx.h, True)
+    ms_prof = timed_pass()
+    clocks = sampler.stop()
+    prof = P.lsd_get_profile(ctx.h)
+    P.lsd_profile(ctx.h, False)
     edges = P.lsd_get_edge_count(ctx.h, P.LSD_TARGET, 0, K) if tgt is not None else 0
     if world > 1:
         t = torch.tensor([ms], device="cuda", dtype=torch.float64)
@@ -251,11 +263,13 @@ def main():
             peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12         # fp32 FMA lanes x 2 flop x max SM clock
             peak_note = "fp32 FMA pipe: 148 SMs x 128 lanes x 2 flop x clocks.max.sm (derived, DESIGN.md)"
         mlip_ms = prof["mlip_edge_bwd"]["ms"] + prof["mlip_edge_fwd"]["ms"] + prof["mlip_dense"]["ms"]
-        roofline = dict(bound=bound, achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak, traffic=None,
-                        kernel="k_edge<F,true> (MLIP edge backward)", avg_launch_ms=avg_ms, launches=eb["launches"],
+        roofline = dict(bound=bound, achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak, traffic=NCU_TRAFFIC.get((args.workload, dtype)),
+                        kernel=("k_edge_tc128<bwd>" if use_tc and F == 128 else "k_edge_tc<F,bwd>" if use_tc else "k_edge<F,bwd>") + " (MLIP edge backward: filter value + tangent, cfconv adjoints)", avg_launch_ms=avg_ms, launches=eb["launches"],
                         algorithmic_flops_per_launch=flops_per_launch, directed_edges_per_window=edges, peak_note=peak_note,
-                        share_of_step=eb["ms"] / ms if ms > 0 else None,
+                        share_of_step=eb["ms"] / ms_prof if ms_prof > 0 else None, profiled_ms_per_step=ms_prof / args.steps,
                         a2_strict_tflops=args.steps * edges * T * (2 * R * F + 2 * F * F + 8 * F) / (mlip_ms * 1e-3) / 1e12 if mlip_ms > 0 else None,
+                        a2_directed_tflops=args.steps * edges * T * (2 * (2 * R * F + 2 * F * F) + 8 * F) / (mlip_ms * 1e-3) / 1e12 if mlip_ms > 0 else None,
+                        kernel_executed_tflops=edges * 2 * (2 * R * F + 2 * F * F) / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else None,
                         stage_ms_per_step={k: v["ms"] / args.steps for k, v in prof.items() if v["launches"]})
 
     if rank == 0:

@@ -64,14 +64,14 @@ __global__ void k_half_a(int n, const double* __restrict__ q, const double* __re
 }
 
 // B O B (= Eq. 7 Gaussian draw) followed by A(1/2):  p' = c1 p + b F + sigma xi;  q' = q_half + (dt/2) p'/m
-__global__ void k_bob_a(int n, uint64_t seed, uint64_t step, const double* __restrict__ p_prev, const double* __restrict__ Ft,
+__global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, uint64_t j, const double* __restrict__ p_prev, const double* __restrict__ Ft,
                         const double* __restrict__ qhalf, const double* __restrict__ mass, const double* __restrict__ sigma,
                         double c1, double b, double hdt, double* __restrict__ q_new, double* __restrict__ p_new)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double xi[3];
-    normals3(seed, step, (uint32_t)i, 0u, xi);
+    normals3(seed, *n0p + j, (uint32_t)i, 0u, xi);          // step index n0 + j; n0 lives in device memory so that a captured graph can be replayed
     const double m = mass[i], sg = sigma[i];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -98,10 +98,11 @@ __global__ void k_initial_momenta(int n, uint64_t seed, const double* __restrict
 constexpr int kTrThreads = 256;
 
 __global__ void __launch_bounds__(kTrThreads)
-k_transport_partial(int n, uint64_t seed, uint64_t n0, const double* __restrict__ Ft, const double* __restrict__ Fg,
+k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, const double* __restrict__ Ft, const double* __restrict__ Fg,
                     const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg)
 {
     const int j = blockIdx.y;                      // step j+1 of the window
+    const uint64_t n0 = *n0p;
     const size_t base = (size_t)j * 3 * n;
     double s1 = 0.0, s2 = 0.0;
     for (int i = blockIdx.x * kTrThreads + threadIdx.x; i < n; i += gridDim.x * kTrThreads) {
@@ -133,13 +134,14 @@ k_transport_partial(int n, uint64_t seed, uint64_t n0, const double* __restrict_
 }
 
 // ---- stage 2: ell_j = -S1 - S2/2, u_j, accept iff S2 == 0 or ln u <= min(0, ell) (R7, R8); first-reject scan (:424).
-__global__ void k_transport_final(int K, int nblk, uint64_t seed, uint64_t n0, const double* __restrict__ partial,
+__global__ void k_transport_final(int K, int nblk, uint64_t seed, const uint64_t* __restrict__ n0p, const double* __restrict__ partial,
                                   double* S1, double* S2, double* ell, double* lnu, int* reject, const int* flags,
                                   TransportResult* result)
 {
     __shared__ int rej[LSD_MAX_K];
     __shared__ double beta[LSD_MAX_K];
     const int j = threadIdx.x;
+    const uint64_t n0 = *n0p;
     if (j < K) {
         double a = 0.0, c = 0.0;
         for (int blk = 0; blk < nblk; ++blk) { a += partial[((size_t)j * nblk + blk) * 2]; c += partial[((size_t)j * nblk + blk) * 2 + 1]; }
@@ -162,7 +164,7 @@ __global__ void k_transport_final(int K, int nblk, uint64_t seed, uint64_t n0, c
 }
 
 // ---- stage 3: override of the first rejected step and map g (Eq. 8 else-branch; :602), or commit of y_K.
-__global__ void k_commit(int n, int K, uint64_t seed, uint64_t n0, const TransportResult* __restrict__ result,
+__global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict__ n0p, const TransportResult* __restrict__ result,
                          const double* __restrict__ S1, const double* __restrict__ S2, const double* __restrict__ Ft,
                          const double* __restrict__ Fg, const double* __restrict__ qhalf, const double* __restrict__ pstart,
                          double* __restrict__ yq, double* __restrict__ yp, const double* __restrict__ mass,
@@ -182,7 +184,7 @@ __global__ void k_commit(int n, int K, uint64_t seed, uint64_t n0, const Transpo
     const size_t base = (size_t)(l - 1) * 3 * n;
     const double* pprev = (l == 1) ? pstart : yp + (size_t)(l - 2) * 3 * n;
     double xi[3];
-    normals3(seed, n0 + (uint64_t)l, (uint32_t)i, 0u, xi);
+    normals3(seed, *n0p + (uint64_t)l, (uint32_t)i, 0u, xi);
     const double sg = sigma[i], m = mass[i], ratio = S1[l - 1] / S2[l - 1];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -214,14 +216,21 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
     prof_end(L, pid);
 }
 
-void launch_bob_a(Launcher L, int n, uint64_t seed, uint64_t step, const double* p_prev, const double* Ft,
+void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
                   double* q_new, double* p_new)
 {
     const int pid = prof_begin(L, PROF_INTEG);
-    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, step, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new);
+    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new);
     LSD_COUNT(L);
     prof_end(L, pid);
+}
+
+__global__ void k_set_u64(uint64_t* dst, uint64_t v) { *dst = v; }
+void launch_set_u64(Launcher L, uint64_t* dst, uint64_t v)
+{
+    k_set_u64<<<1, 1, 0, L.s>>>(dst, v);
+    LSD_COUNT(L);
 }
 
 void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p)
@@ -230,7 +239,7 @@ void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass
     LSD_COUNT(L);
 }
 
-void launch_transport(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const double* Ft, const double* Fg,
+void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const double* Ft, const double* Fg,
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
                       double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg)
 {
@@ -242,7 +251,7 @@ void launch_transport(Launcher L, int n, int K, uint64_t seed, uint64_t n0, cons
     prof_end(L, pid);
 }
 
-void launch_commit(Launcher L, int n, int K, uint64_t seed, uint64_t n0, const TransportResult* result,
+void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const TransportResult* result,
                    const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
                    double c1, double b, double hdt, double* q_base, double* p_base)

@@ -2,7 +2,9 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <map>
 #include <new>
 
 #include "lsd_internal.h"
@@ -11,10 +13,16 @@ namespace {
 
 thread_local std::string g_init_error;
 
+// A launch sequence that is identical from window to window (same slot, same K) is captured once into a CUDA graph and
+// replayed: the small configurations are launch-bound (cfg2: ~200 launches per window of 22 atoms).
+struct GraphEntry { cudaGraphExec_t exec = nullptr; int64_t launches = 0; int uses = 0; };
+
 struct WindowSlot {
     int K = 0;
     int drafted = 0, verified = 0;
-    uint64_t n0 = 0;
+    uint64_t n0 = 0;                                         // step index of the window's start state ...
+    uint64_t* n0_dev = nullptr;                              // ... and its device copy, read by the Philox-keyed kernels
+    std::map<int, GraphEntry> g_roll, g_verify, g_transport; // by K
     double *qstart = nullptr, *pstart = nullptr;             // [3][n]
     double *qhalf = nullptr, *Ft = nullptr, *yq = nullptr, *yp = nullptr;   // [kmax][3][n]
     int* img = nullptr;                                      // [n] images of the reference (start) state
@@ -54,6 +62,7 @@ struct lsd_ctx {
     VerletList vl_eval_mlip, vl_eval_pair;
     cudaStream_t side = nullptr;
     int64_t launches = 0;
+    bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
     Prof prof;
     lsd_stats stats{};
     std::string err;
@@ -92,6 +101,45 @@ template <typename T> lsd_status upload(lsd_ctx* ctx, T** p, const T* host, size
 #define TRY(expr) do { lsd_status s__ = (expr); if (s__ != LSD_OK) return s__; } while (0)
 
 Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, &ctx->launches, &ctx->prof}; }
+
+void drop_graphs(lsd_ctx* ctx)
+{
+    for (int s = 0; s < 2; ++s)
+        for (auto* m : {&ctx->slot[s].g_roll, &ctx->slot[s].g_verify, &ctx->slot[s].g_transport}) {
+            for (auto& kv : *m) if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+            m->clear();
+        }
+}
+
+// Runs `body` (stream-ordered launches on `st` only) directly the first time (allocations, function attributes), captures
+// it the second time and replays the graph from then on.  Never on the legacy default stream, never while profiling.
+template <class Body> lsd_status run_graphed(lsd_ctx* ctx, cudaStream_t st, GraphEntry& g, Body body)
+{
+    if (!ctx->use_graphs || st == nullptr || ctx->prof.on) return body();
+    if (g.uses++ == 0) return body();
+    if (!g.exec) {
+        const int64_t before = ctx->launches;
+        CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+        const lsd_status bs = body();
+        cudaGraph_t graph = nullptr;
+        const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+        if (bs != LSD_OK || ce != cudaSuccess || graph == nullptr) {          // not capturable here: fall back to direct launches for good
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            ctx->use_graphs = false;
+            ctx->launches = before;
+            return body();
+        }
+        g.launches = ctx->launches - before;
+        ctx->launches = before;
+        const cudaError_t ie = cudaGraphInstantiate(&g.exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ie != cudaSuccess) { g.exec = nullptr; cudaGetLastError(); ctx->use_graphs = false; return body(); }
+    }
+    CK(cudaGraphLaunch(g.exec, st));
+    ctx->launches += g.launches;
+    return LSD_OK;
+}
 
 lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
 {
@@ -330,6 +378,7 @@ void lsd_destroy(lsd_ctx* ctx)
 {
     if (!ctx) return;
     cudaDeviceSynchronize();
+    drop_graphs(ctx);
     for (void* p : ctx->allocs) cudaFree(p);
     cudaFree(ctx->grid.cell_count); cudaFree(ctx->grid.cell_start); cudaFree(ctx->grid.cell_cursor);
     cudaFree(ctx->grid.cell_atoms); cudaFree(ctx->grid.atom_cell);
@@ -412,7 +461,7 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
         WindowSlot& w = ctx->slot[s];
         TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
         TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
-        TRY(dalloc(ctx, &w.img, n)); TRY(dalloc(ctx, &w.flags, 1));
+        TRY(dalloc(ctx, &w.img, n)); TRY(dalloc(ctx, &w.flags, 1)); TRY(dalloc(ctx, &w.n0_dev, 1));
         CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
     }
     for (int w = 0; w < 2; ++w) if (ctx->pot[w].mlip.F > 0) TRY(alloc_work(ctx, ctx->pot[w].mlip, ctx->work[w], ctx->bmax[w]));
@@ -425,6 +474,7 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
     TRY(dalloc(ctx, &ctx->img_eval, n)); TRY(dalloc(ctx, &ctx->flags_eval, 1));
     CK(cudaMallocHost(&ctx->result_host, sizeof(TransportResult)));
     CK(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+    { const char* g = getenv("LSD_GRAPHS"); ctx->use_graphs = !(g && g[0] == '0'); }
     CK(cudaDeviceSynchronize());
     CK(cudaGetLastError());
     return LSD_OK;
@@ -448,6 +498,7 @@ lsd_status lsd_set_skin(lsd_ctx* ctx, double skin)
     if (!ctx || !(skin > 0)) return LSD_ERR_INVALID_ARG;
     CK(cudaDeviceSynchronize());
     ctx->cfg.skin = skin;
+    drop_graphs(ctx);                                        // captured pointers and the skin value change
     ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
     return setup_lists(ctx);      // old rows stay allocated until lsd_destroy
 }
@@ -475,18 +526,24 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
         CK(cudaMemcpyAsync(w.pstart, pv.yp + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         w.n0 = pv.n0 + (uint64_t)pv.K;
     }
-    CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
-    build_lists(ctx, L, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
-    const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
-    for (int j = 1; j <= K; ++j) {                                            // serial in j
-        const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
-        const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
-        double* qh = w.qhalf + n3 * (j - 1);
-        launch_half_a(L, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
-        eval_forces(ctx, L, LSD_DRAFT, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
-        launch_bob_a(L, n, ctx->cfg.seed, w.n0 + (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
-                     ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1));
-    }
+    launch_set_u64(L, w.n0_dev, w.n0);
+    TRY(run_graphed(ctx, st, w.g_roll[K], [&]() -> lsd_status {
+        Launcher Lg = mk(ctx, stream);
+        CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
+        build_lists(ctx, Lg, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
+        const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
+        for (int j = 1; j <= K; ++j) {                                        // serial in j
+            const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
+            const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
+            double* qh = w.qhalf + n3 * (j - 1);
+            launch_half_a(Lg, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
+            eval_forces(ctx, Lg, LSD_DRAFT, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
+            launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
+                         ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1));
+        }
+        return LSD_OK;
+    }));
+    ctx->cl_img[LSD_DRAFT] = w.img;                                           // (set by eval_forces only when the body runs)
     CK(cudaEventRecord(w.ev_drafted, st));
     w.K = K; w.drafted = 1; w.verified = 0;
     ctx->pending++;
@@ -502,7 +559,11 @@ lsd_status lsd_verify_window(lsd_ctx* ctx, int32_t K, void* stream)
     if (K != w.K) return fail(ctx, LSD_ERR_INVALID_ARG, "K differs from the drafted window length");
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
-    eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr);
+    TRY(run_graphed(ctx, st, w.g_verify[K], [&]() -> lsd_status {
+        eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr);
+        return LSD_OK;
+    }));
+    ctx->cl_img[LSD_TARGET] = w.img;
     w.verified = 1;
     CK(cudaGetLastError());
     return LSD_OK;
@@ -517,10 +578,14 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
     cudaStream_t st = (cudaStream_t)stream;
     Launcher L = mk(ctx, stream);
     const int n = ctx->sys.n;
-    launch_transport(L, n, K, ctx->cfg.seed, w.n0, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk, ctx->S1, ctx->S2,
-                     ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
-    launch_commit(L, n, K, ctx->cfg.seed, w.n0, ctx->result, ctx->S1, ctx->S2, w.Ft, ctx->Fg, w.qhalf, w.pstart, w.yq, w.yp,
-                  ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p);
+    TRY(run_graphed(ctx, st, w.g_transport[K], [&]() -> lsd_status {
+        Launcher Lg = mk(ctx, stream);
+        launch_transport(Lg, n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk, ctx->S1, ctx->S2,
+                         ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
+        launch_commit(Lg, n, K, ctx->cfg.seed, w.n0_dev, ctx->result, ctx->S1, ctx->S2, w.Ft, ctx->Fg, w.qhalf, w.pstart, w.yq, w.yp,
+                      ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p);
+        return LSD_OK;
+    }));
     CK(cudaMemcpyAsync(ctx->result_host, ctx->result, sizeof(TransportResult), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
@@ -650,7 +715,7 @@ lsd_status lsd_get_window_debug(lsd_ctx* ctx, int32_t what, void* out, int32_t w
         case LSD_DBG_REJECT:  return copy_out(ctx, out, ctx->reject, (size_t)K * sizeof(int), where);
         case LSD_DBG_XI: {
             if (!ctx->xi_dbg) TRY(dalloc(ctx, &ctx->xi_dbg, (size_t)3 * ctx->sys.n * ctx->cfg.k_max));
-            launch_transport(mk(ctx, nullptr), ctx->sys.n, K, ctx->cfg.seed, w.n0, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk,
+            launch_transport(mk(ctx, nullptr), ctx->sys.n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk,
                              ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
             CK(cudaDeviceSynchronize());
             return copy_out(ctx, out, ctx->xi_dbg, big, where);

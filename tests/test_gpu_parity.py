@@ -271,6 +271,32 @@ def test_committed_trajectory_independent_of_K_and_overlap(P, orc):
         assert np.array_equal(q, finals[0][0]) and np.array_equal(p, finals[0][1])
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,prec", [("cfg1", "fp64"), ("cfg2", "fp32"), ("cfg2", "bf16")])
+def test_cuda_graph_replay_is_bit_identical_to_direct_launches(P, orc, name, prec, monkeypatch):
+    """On a non-default stream the rollout / verification / transport launch sequences are captured into CUDA graphs and
+    replayed (lsd_api.cu run_graphed); decisions, committed trajectory and the launch count must not depend on it."""
+    import torch
+    w = L.make_workload(name)
+    p0 = orc.initial_momenta(w)
+    precision = {"fp64": None, "fp32": P.LSD_FP32, "bf16": P.LSD_BF16_TC}[prec]
+    out = []
+    for graphs in ("1", "0"):
+        monkeypatch.setenv("LSD_GRAPHS", graphs)
+        ctx = P.context_from_workload(w, k_max=8, precision=precision, p0=p0)
+        stream = torch.cuda.Stream()
+        decisions = []
+        for i in range(14):                                     # two window lengths: two graphs per stage and slot
+            decisions.append(ctx.window(8 if i % 3 else 5, stream))
+        P.lsd_run(ctx.h, 40, 8, overlap=True, stream=stream)    # speculative rollouts on the side stream
+        q, p, step = ctx.state()
+        out.append((decisions, q, p, step, P.lsd_launch_count(ctx.h)))
+        ctx.close()
+    assert out[0][0] == out[1][0] and out[0][3] == out[1][3]
+    assert np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
+    assert out[0][4] == out[1][4]                               # replayed kernel nodes are counted like direct launches
+
+
 def test_skin_violation_is_detected(P, orc):
     w = L.make_workload("cfg1")
     ctx = P.context_from_workload(w, k_max=2, skin=0.05)
