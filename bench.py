@@ -133,6 +133,25 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def reduce_over_ranks(ms, committed, device=None):
+    """Multi-GPU aggregation (independent replicas, no data-path collective): the step time is the MAX over
+    ranks, committed steps are SUMMED.  Works on any initialised process group (nccl on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms), float(committed)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([float(committed)], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(c.item())
+
+
+def replica_seed(base_seed, rank):
+    """Every rank runs its own replica of the workload: same system, different noise stream."""
+    return int(base_seed) + 1000 * int(rank)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -164,7 +183,7 @@ def main():
     w = L.make_workload(args.workload)
     K, N = w.K, w.n_atoms
     prec = {"fp32": P.LSD_FP32, "bf16": P.LSD_BF16_TC, None: None}[args.precision]
-    ctx = P.context_from_workload(w, precision=prec, seed=w.seed + 1000 * rank)
+    ctx = P.context_from_workload(w, precision=prec, seed=replica_seed(w.seed, rank))
     stream = torch.cuda.Stream()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     tgt = w.target.mlip
@@ -213,15 +232,7 @@ def main():
     prof = P.lsd_get_profile(ctx.h)
     P.lsd_profile(ctx.h, False)
     edges = P.lsd_get_edge_count(ctx.h, P.LSD_TARGET, 0, K) if tgt is not None else 0
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        c = torch.tensor([float(committed)], device="cuda", dtype=torch.float64)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        committed_all = float(c.item())
-    else:
-        committed_all = float(committed)
+    ms, committed_all = reduce_over_ranks(ms, committed, device="cuda")
     value = K * N * args.steps * world / (ms * 1e-3)
 
     # ---- end-to-end through the C ABI with HOST buffers (pinned): upload x_n, run the window, read x_{n+commit} back
@@ -238,10 +249,7 @@ def main():
         step0 = P.lsd_get_state(ctx.h, qh.numpy(), ph.numpy())
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s, _ = reduce_over_ranks(e2e_s, 0, device="cuda")
     e2e = dict(value=K * N * args.steps * world / e2e_s, unit=UNIT, h2d_bytes_per_step=2 * 3 * N * 8, d2h_bytes_per_step=2 * 3 * N * 8 + 8,
                ms_per_step=1e3 * e2e_s / args.steps)
 
