@@ -74,6 +74,8 @@ def lib():
             L.orc_lsd_window.restype = C.c_int32
             L.orc_transport_step.restype = C.c_int32
             L.orc_run_lsd.restype = C.c_int64
+            L.orc_lsd_window_ec.restype = C.c_int32
+            L.orc_run_lsd_ec.restype = C.c_int64
             L.orc_rejection_probability.restype = C.c_double
             L.orc_rejection_probability.argtypes = [C.c_double]
             _lib = L
@@ -209,8 +211,10 @@ def transport_step(w, Ft, F, xi, u, p_prev, q_half, par=None):
     return dict(reject=int(rej), S1=S1.value, S2=S2.value, ell=ell.value, q=qo, p=po)
 
 
-def lsd_window(w, q, p, n0, K=None, draft=None, target=None, par=None, debug=True):
-    """One synchronous window (Alg. 1).  Returns dict with new base state, committed trajectory, debug rows."""
+def lsd_window(w, q, p, n0, K=None, draft=None, target=None, par=None, debug=True, dF=None):
+    """One synchronous window (Alg. 1).  Returns dict with new base state, committed trajectory, debug rows.
+    dF ([N,3]) switches speculative error correction on (Alg. 3): the cache used by this window; "dF" in the result is the
+    cache after it."""
     s = System(w)
     D, T = Pot(draft or w.draft), Pot(target or w.target)
     par = par or params(w)
@@ -223,17 +227,22 @@ def lsd_window(w, q, p, n0, K=None, draft=None, target=None, par=None, debug=Tru
     S1, S2, ell, lnu = np.zeros(K), np.zeros(K), np.zeros(K), np.zeros(K)
     rej = np.zeros(K, np.int32)
     l = C.c_int32()
-    if debug:
+    if dF is not None:
+        dF = np.array(dF, np.float64, order="C", copy=True)
+        dbg = (_dp(qh), _dp(Ft), _dp(Fg), _dp(S1), _dp(S2), _dp(ell), _dp(lnu), _ip(rej)) if debug else (None,) * 8
+        nc = lib().orc_lsd_window_ec(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_uint64(n0), C.c_int32(K), _dp(q), _dp(p),
+                                     _dp(dF), C.byref(l), _dp(tq), _dp(tp), *dbg)
+    elif debug:
         nc = lib().orc_lsd_window(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_uint64(n0), C.c_int32(K), _dp(q), _dp(p),
                                   C.byref(l), _dp(tq), _dp(tp), _dp(qh), _dp(Ft), _dp(Fg), _dp(S1), _dp(S2), _dp(ell), _dp(lnu), _ip(rej))
     else:
         nc = lib().orc_lsd_window(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_uint64(n0), C.c_int32(K), _dp(q), _dp(p),
                                   C.byref(l), _dp(tq), _dp(tp), None, None, None, None, None, None, None, None)
     return dict(q=q, p=p, n_commit=int(nc), first_reject=int(l.value), traj_q=tq[:nc], traj_p=tp[:nc],
-                q_half=qh, Ft=Ft, F=Fg, S1=S1, S2=S2, ell=ell, lnu=lnu, reject=rej)
+                q_half=qh, Ft=Ft, F=Fg, S1=S1, S2=S2, ell=ell, lnu=lnu, reject=rej, dF=dF)
 
 
-def run_lsd(w, q, p, n_steps, K=None, draft=None, target=None, par=None, keep_traj=True):
+def run_lsd(w, q, p, n_steps, K=None, draft=None, target=None, par=None, keep_traj=True, ec=False):
     s = System(w)
     D, T = Pot(draft or w.draft), Pot(target or w.target)
     par = par or params(w)
@@ -243,10 +252,15 @@ def run_lsd(w, q, p, n_steps, K=None, draft=None, target=None, par=None, keep_tr
     tq = np.zeros((n_steps, s.n, 3)) if keep_traj else None
     tp = np.zeros((n_steps, s.n, 3)) if keep_traj else None
     stats = np.zeros(4)
-    lib().orc_run_lsd(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_int64(n_steps), C.c_int32(K), _dp(q), _dp(p),
-                      _dp(tq) if keep_traj else None, _dp(tp) if keep_traj else None, _dp(stats))
+    dF = np.zeros((s.n, 3)) if ec else None
+    if ec:
+        lib().orc_run_lsd_ec(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_int64(n_steps), C.c_int32(K), _dp(q), _dp(p),
+                             _dp(dF), _dp(tq) if keep_traj else None, _dp(tp) if keep_traj else None, _dp(stats))
+    else:
+        lib().orc_run_lsd(C.byref(s.c), C.byref(par), C.byref(D.c), C.byref(T.c), C.c_int64(n_steps), C.c_int32(K), _dp(q), _dp(p),
+                          _dp(tq) if keep_traj else None, _dp(tp) if keep_traj else None, _dp(stats))
     return dict(q=q, p=p, traj_q=tq, traj_p=tp, windows=int(stats[0]), rejections=int(stats[1]),
-                beta_sum=float(stats[2]), examined=int(stats[3]))
+                beta_sum=float(stats[2]), examined=int(stats[3]), dF=dF)
 
 
 def run_aboba(w, pot, q, p, n_steps, par=None, keep_traj=True):

@@ -19,6 +19,7 @@
  *   ABOBA               : harmonic-oscillator closed forms <q^2> = kT/k, <p^2>/m = kT/(1-dt^2 k/4m)
  *   transport           : 1-D mirror image (Fig. 2), Householder invariants, Monte-Carlo vs erf (Eq. 9)
  *   window              : draft==target => acceptance 1 and trajectory == plain ABOBA; K-invariance
+ *   window with EC      : dF = 0 == plain window; constant force error => S2 == 0 after one commit; target <q^2>
  * Functions with no independent pin: none ("parity unpinned" would be stated here).
  *
  * Layout: positions/momenta/forces are [N][3] doubles (AoS) inside the oracle.
@@ -675,3 +676,105 @@ void orc_run_aboba(const orc_system *sys, const orc_params *par, const orc_poten
 
 /* Eq. 9: rejection probability of one step, beta = erf(||delta|| / sqrt 8). */
 double orc_rejection_probability(double delta_norm) { return erf(delta_norm / sqrt(8.0)); }
+
+/* ------------------------------------------------------------------------------------------
+ * O-5: speculative error correction, EC ("Speculative error
+ * correction"; App. E :626-630; Alg. 3 :663-717), written for the synchronous window of O-3.
+ *   DRAFT_STEP(y, dF) (:675-684): F~ = DraftModel(q_half) is the BARE output and is what is stored;
+ *       <p~> = [Eq. 7](F~ + dF), i.e. p' = c1 p + b (F~ + dF) + sigma xi.
+ *   VERIFY_STEP (:686-700): <p~> = [Eq. 7](F~ + dF), <p> = [Eq. 7](F), so
+ *       d = (b / sigma)((F~ + dF) - F);  dF' = F - F~ uses the EC-UNCORRECTED draft forces (:628, :694)
+ *       "which avoids self-feedback instability".
+ *   PROCESS_NEW_RETURNS (:710-713): the cache becomes the dF' "stored in this step" when the step
+ *       is added to the verified queue V, i.e. committed.
+ * [reading R17] In the window form every draft step of a window is proposed before any of its target
+ * results exists, so the whole window uses the cache as it stands when the window is drafted (the
+ * dF' of the last step committed by the previous window); after the window the cache is the dF' of
+ * its LAST committed step c = l (the overridden step counts, R4) or K.
+ * dF: in = cache used by this window, out = cache after it.  dbg_Ft receives the bare F~.
+ * Pins (tests/test_oracle_ec.py): dF = 0 <=> orc_lsd_window bit for bit; draft = target + constant
+ * force => after the first committed step every step has S2 == 0 and is accepted (closed form);
+ * harmonic oscillator with a wrong draft keeps the target's <q^2> = kT/k (Thm. 3.1 holds for any
+ * draft law, :630); rejection count vs sum of erf(sqrt(S2)/sqrt 8) (Eq. 9).
+ * ---------------------------------------------------------------------------------------- */
+int32_t orc_lsd_window_ec(const orc_system *sys, const orc_params *par, const orc_potential *draft, const orc_potential *target,
+                          uint64_t n0, int32_t K, double *q, double *p, double *dF, int32_t *first_reject,
+                          double *traj_q, double *traj_p,
+                          double *dbg_qhalf, double *dbg_Ft, double *dbg_F, double *dbg_S1, double *dbg_S2,
+                          double *dbg_ell, double *dbg_lnu, int32_t *dbg_reject)
+{
+    const size_t n3 = 3 * (size_t)sys->n;
+    const int n = sys->n;
+    aboba_consts k = aboba_k(par);
+    double *yq = (double *)malloc(sizeof(double) * n3 * (K + 1)), *yp = (double *)malloc(sizeof(double) * n3 * (K + 1));
+    double *qh = (double *)malloc(sizeof(double) * n3 * K), *Ft = (double *)malloc(sizeof(double) * n3 * K);
+    double *xi = (double *)malloc(sizeof(double) * n3 * K), *Fg = (double *)malloc(sizeof(double) * n3);
+    double *xq = (double *)malloc(sizeof(double) * n3), *xp = (double *)malloc(sizeof(double) * n3);
+    double *Fe = (double *)malloc(sizeof(double) * n3), *Fc = (double *)malloc(sizeof(double) * n3);
+    memcpy(yq, q, sizeof(double) * n3); memcpy(yp, p, sizeof(double) * n3);
+    for (int j = 1; j <= K; ++j) {                                      /* DRAFT_STEP(y, dF), serial */
+        const double *q0 = yq + n3 * (j - 1), *p0 = yp + n3 * (j - 1);
+        double *q1 = yq + n3 * j, *p1 = yp + n3 * j, *qhj = qh + n3 * (j - 1), *Fb = Ft + n3 * (j - 1), *xj = xi + n3 * (j - 1);
+        for (int i = 0; i < n; ++i) for (int c = 0; c < 3; ++c)
+            qhj[3 * i + c] = q0[3 * i + c] + k.hdt * p0[3 * i + c] / (sys->mass_amu[i] * ORC_AMU);
+        orc_energy_forces(sys, draft, qhj, Fb);                         /* bare F~ */
+        orc_normals(par->seed, n0 + j, n, 0u, xj);
+        for (int i = 0; i < n; ++i) {
+            double sg = sigma_i(sys, par, k.c1, i);
+            for (int c = 0; c < 3; ++c) {
+                p1[3 * i + c] = k.c1 * p0[3 * i + c] + k.b * (Fb[3 * i + c] + dF[3 * i + c]) + sg * xj[3 * i + c];
+                q1[3 * i + c] = qhj[3 * i + c] + k.hdt * p1[3 * i + c] / (sys->mass_amu[i] * ORC_AMU);
+            }
+        }
+    }
+    int32_t l = 0;
+    for (int j = 1; j <= K; ++j) {                                      /* VERIFY_STEP for every j */
+        double S1, S2, ell, u = orc_uniform(par->seed, n0 + j);
+        orc_energy_forces(sys, target, qh + n3 * (j - 1), Fg);
+        for (size_t a = 0; a < n3; ++a) Fe[a] = Ft[n3 * (j - 1) + a] + dF[a];      /* <p~> was drawn around F~ + dF */
+        if (l == 0) memcpy(Fc, Fg, sizeof(double) * n3);                /* target forces of the last step that will be committed */
+        int32_t rej = orc_transport_step(sys, par, Fe, Fg, xi + n3 * (j - 1), u, yp + n3 * (j - 1), qh + n3 * (j - 1),
+                                         &S1, &S2, &ell, (l == 0) ? xq : NULL, (l == 0) ? xp : NULL);
+        if (dbg_qhalf) memcpy(dbg_qhalf + n3 * (j - 1), qh + n3 * (j - 1), sizeof(double) * n3);
+        if (dbg_Ft) memcpy(dbg_Ft + n3 * (j - 1), Ft + n3 * (j - 1), sizeof(double) * n3);
+        if (dbg_F) memcpy(dbg_F + n3 * (j - 1), Fg, sizeof(double) * n3);
+        if (dbg_S1) dbg_S1[j - 1] = S1; if (dbg_S2) dbg_S2[j - 1] = S2; if (dbg_ell) dbg_ell[j - 1] = ell;
+        if (dbg_lnu) dbg_lnu[j - 1] = log(u); if (dbg_reject) dbg_reject[j - 1] = rej;
+        if (rej && l == 0) l = j;
+        if (l != 0 && !dbg_reject && !dbg_F) break;
+    }
+    int32_t n_commit = l ? l : K;
+    for (int j = 1; j <= n_commit; ++j) {
+        const double *sq = (l && j == l) ? xq : yq + n3 * j, *sp = (l && j == l) ? xp : yp + n3 * j;
+        if (traj_q) memcpy(traj_q + n3 * (j - 1), sq, sizeof(double) * n3);
+        if (traj_p) memcpy(traj_p + n3 * (j - 1), sp, sizeof(double) * n3);
+        if (j == n_commit) { memcpy(q, sq, sizeof(double) * n3); memcpy(p, sp, sizeof(double) * n3); }
+    }
+    for (size_t a = 0; a < n3; ++a) dF[a] = Fc[a] - Ft[n3 * (n_commit - 1) + a];   /* dF' = F - F~(bare) of the last committed step */
+    *first_reject = l;
+    free(yq); free(yp); free(qh); free(Ft); free(xi); free(Fg); free(xq); free(xp); free(Fe); free(Fc);
+    return n_commit;
+}
+
+/* orc_run_lsd with EC: the cache starts at zero (:669 "dF <- 0") and is carried from window to window. */
+int64_t orc_run_lsd_ec(const orc_system *sys, const orc_params *par, const orc_potential *draft, const orc_potential *target,
+                       int64_t n_steps, int32_t K, double *q, double *p, double *dF, double *traj_q, double *traj_p, double *stats)
+{
+    const size_t n3 = 3 * (size_t)sys->n;
+    int64_t n = 0, windows = 0, rejections = 0; double beta_sum = 0.0; int64_t examined = 0;
+    double *tq = (double *)malloc(sizeof(double) * n3 * K), *tp = (double *)malloc(sizeof(double) * n3 * K);
+    double *S2 = (double *)malloc(sizeof(double) * K);
+    while (n < n_steps) {
+        int32_t k = K; if (n + k > n_steps) k = (int32_t)(n_steps - n);
+        int32_t l;
+        int32_t nc = orc_lsd_window_ec(sys, par, draft, target, (uint64_t)n, k, q, p, dF, &l, tq, tp, NULL, NULL, NULL, NULL, S2, NULL, NULL, NULL);
+        for (int j = 0; j < nc; ++j) { beta_sum += erf(sqrt(S2[j]) / sqrt(8.0)); ++examined; }
+        if (l) ++rejections;
+        if (traj_q) memcpy(traj_q + n3 * n, tq, sizeof(double) * n3 * nc);
+        if (traj_p) memcpy(traj_p + n3 * n, tp, sizeof(double) * n3 * nc);
+        n += nc; ++windows;
+    }
+    if (stats) { stats[0] = (double)windows; stats[1] = (double)rejections; stats[2] = beta_sum; stats[3] = (double)examined; }
+    free(tq); free(tp); free(S2);
+    return n;
+}
