@@ -161,6 +161,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default=None, choices=[None, "fp32", "bf16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ec", type=int, default=0, help="1: speculative error correction (Alg. 3) on")
     ap.add_argument("--overlap", type=int, default=0, help="1: time lsd_run with the speculative second-stream rollout instead of explicit calls")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -184,6 +185,8 @@ def main():
     K, N = w.K, w.n_atoms
     prec = {"fp32": P.LSD_FP32, "bf16": P.LSD_BF16_TC, None: None}[args.precision]
     ctx = P.context_from_workload(w, precision=prec, seed=replica_seed(w.seed, rank))
+    if args.ec:
+        P.lsd_set_error_correction(ctx.h, True)
     stream = torch.cuda.Stream()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     tgt = w.target.mlip
@@ -285,7 +288,7 @@ def main():
                     higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
                     config=dict(workload=args.workload, n_atoms=N, window_K=K, atoms_per_window=K * N, integrator="ABOBA (Eq. 2)",
                                 l2="flushed between timed steps (256 MiB write)" if need_flush else "working set larger than L2",
-                                overlap=bool(args.overlap), replicas=world, peaks=peaks["source"]),
+                                overlap=bool(args.overlap), error_correction=bool(args.ec), replicas=world, peaks=peaks["source"]),
                     committed_md_steps_per_s=committed_all / (ms * 1e-3), committed_per_window=committed_all / (args.steps * world),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline)
         if not args.no_cpu_baseline and world == 1:

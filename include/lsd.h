@@ -157,6 +157,18 @@ lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out);
 /* Committed state j (1..n_commit) of the window most recently passed to lsd_transport_accept. */
 lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where);
 
+/* Speculative error correction, EC (App. E :626-630; Alg. 3 :663-717), window form:
+ * the draft kick uses F~ + dF, the transport map uses delta = (b/sigma)(F~ + dF - F), and after every window the cache
+ * becomes dF = F - F~ (BARE draft output, :628) of the window's last committed step.  A window uses the cache as it stood
+ * when it was drafted (a speculative next-window rollout inherits the cache of the window before it).  Target exactness
+ * is unaffected (Thm. 3.1 holds for any draft law, :630); the committed trajectory is no longer independent of K.
+ * lsd_set_error_correction: enable != 0 switches EC on; either way the cache is zeroed (:669) and drafted windows are
+ * dropped.  lsd_get/set_ec_cache: dF is [3][n_atoms] fp64, `where` = LSD_HOST | LSD_DEVICE; set requires EC on (STATE).
+ * lsd_set_state also zeroes the cache.  All three synchronise the device. */
+lsd_status lsd_set_error_correction(lsd_ctx* ctx, int32_t enable);
+lsd_status lsd_get_ec_cache(lsd_ctx* ctx, double* dF, int32_t where);
+lsd_status lsd_set_ec_cache(lsd_ctx* ctx, const double* dF, int32_t where);
+
 /* Debug rows of that window (parity tests).  `what`: */
 #define LSD_DBG_QHALF    0   /* double [K][3][n]   positions after the first A half-step                */
 #define LSD_DBG_FDRAFT   1   /* double [K][3][n]   F~_j                                                */

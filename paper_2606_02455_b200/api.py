@@ -21,7 +21,8 @@ _STATUS = {0: "LSD_OK", -1: "LSD_ERR_INVALID_ARG", -2: "LSD_ERR_CUDA", -3: "LSD_
 
 EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_rollout", "lsd_verify_window", "lsd_transport_accept",
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
-                    "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled"]
+                    "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
+                    "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache"]
 
 
 class LsdError(RuntimeError):
@@ -183,6 +184,20 @@ def lsd_set_state(h, q, p, step):
     (qp, wq), (pp, wp) = _ptr(q), _ptr(p)
     assert wq == wp
     _check(h, load_library().lsd_set_state(h, qp, pp, C.c_int64(step), C.c_int32(wq)))
+
+
+def lsd_set_error_correction(h, enable: bool):
+    _check(h, load_library().lsd_set_error_correction(h, C.c_int32(int(bool(enable)))))
+
+
+def lsd_get_ec_cache(h, dF):
+    ptr, where = _ptr(dF)
+    _check(h, load_library().lsd_get_ec_cache(h, ptr, C.c_int32(where)))
+
+
+def lsd_set_ec_cache(h, dF):
+    ptr, where = _ptr(dF)
+    _check(h, load_library().lsd_set_ec_cache(h, ptr, C.c_int32(where)))
 
 
 def lsd_get_stats(h) -> dict:

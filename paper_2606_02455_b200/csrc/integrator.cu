@@ -66,7 +66,8 @@ __global__ void k_half_a(int n, const double* __restrict__ q, const double* __re
 // B O B (= Eq. 7 Gaussian draw) followed by A(1/2):  p' = c1 p + b F + sigma xi;  q' = q_half + (dt/2) p'/m
 __global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, uint64_t j, const double* __restrict__ p_prev, const double* __restrict__ Ft,
                         const double* __restrict__ qhalf, const double* __restrict__ mass, const double* __restrict__ sigma,
-                        double c1, double b, double hdt, double* __restrict__ q_new, double* __restrict__ p_new)
+                        double c1, double b, double hdt, double* __restrict__ q_new, double* __restrict__ p_new,
+                        const double* __restrict__ dF)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -75,7 +76,8 @@ __global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, 
     const double m = mass[i], sg = sigma[i];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double pn = c1 * p_prev[c * n + i] + b * Ft[c * n + i] + sg * xi[c];
+        const double Fe = dF ? Ft[c * n + i] + dF[c * n + i] : Ft[c * n + i];      // EC (Alg. 3): <p~> = [Eq. 7](F~ + dF)
+        const double pn = c1 * p_prev[c * n + i] + b * Fe + sg * xi[c];
         p_new[c * n + i] = pn;
         q_new[c * n + i] = qhalf[c * n + i] + hdt * pn / m;
     }
@@ -99,7 +101,8 @@ constexpr int kTrThreads = 256;
 
 __global__ void __launch_bounds__(kTrThreads)
 k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, const double* __restrict__ Ft, const double* __restrict__ Fg,
-                    const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg)
+                    const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg,
+                    const double* __restrict__ dF)
 {
     const int j = blockIdx.y;                      // step j+1 of the window
     const uint64_t n0 = *n0p;
@@ -111,7 +114,8 @@ k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, cons
         const double bs = b / sigma[i];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const double d = bs * (Ft[base + (size_t)c * n + i] - Fg[base + (size_t)c * n + i]);
+            const double Fe = dF ? Ft[base + (size_t)c * n + i] + dF[c * n + i] : Ft[base + (size_t)c * n + i];   // EC: the draft was drawn around F~ + dF
+            const double d = bs * (Fe - Fg[base + (size_t)c * n + i]);
             s1 += xi[c] * d;
             s2 += d * d;
             if (xi_dbg) xi_dbg[base + (size_t)c * n + i] = xi[c];
@@ -169,12 +173,17 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
                          const double* __restrict__ Fg, const double* __restrict__ qhalf, const double* __restrict__ pstart,
                          double* __restrict__ yq, double* __restrict__ yp, const double* __restrict__ mass,
                          const double* __restrict__ sigma, double c1, double b, double hdt, double* __restrict__ q_base,
-                         double* __restrict__ p_base)
+                         double* __restrict__ p_base, const double* __restrict__ dF, double* __restrict__ dF_out)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     if (result->flags != 0) return;                  // skin / overflow / non-finite: nothing is committed
     const int l = result->first_reject;
+    if (dF_out) {                                    // EC cache <- F - F~ (bare draft output) of the last committed step
+        const size_t cb = (size_t)((l ? l : K) - 1) * 3 * n;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) dF_out[c * n + i] = Fg[cb + (size_t)c * n + i] - Ft[cb + (size_t)c * n + i];
+    }
     if (l == 0) {
         const size_t base = (size_t)(K - 1) * 3 * n;
 #pragma unroll
@@ -189,7 +198,8 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const double F = Fg[base + (size_t)c * n + i];
-        const double d = b / sg * (Ft[base + (size_t)c * n + i] - F);
+        const double Fe = dF ? Ft[base + (size_t)c * n + i] + dF[c * n + i] : Ft[base + (size_t)c * n + i];
+        const double d = b / sg * (Fe - F);
         const double ps = c1 * pprev[c * n + i] + b * F + sg * (xi[c] - 2.0 * ratio * d);
         const double qs = qhalf[base + (size_t)c * n + i] + hdt * ps / m;
         p_base[c * n + i] = ps; q_base[c * n + i] = qs;
@@ -218,10 +228,10 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
 
 void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
-                  double* q_new, double* p_new)
+                  double* q_new, double* p_new, const double* dF)
 {
     const int pid = prof_begin(L, PROF_INTEG);
-    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new);
+    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new, dF);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
@@ -241,10 +251,10 @@ void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass
 
 void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const double* Ft, const double* Fg,
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
-                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg)
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
-    k_transport_partial<<<dim3(nblk, K), kTrThreads, 0, L.s>>>(n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg);
+    k_transport_partial<<<dim3(nblk, K), kTrThreads, 0, L.s>>>(n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg, dF);
     LSD_COUNT(L);
     k_transport_final<<<1, LSD_MAX_K, 0, L.s>>>(K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
     LSD_COUNT(L);
@@ -254,11 +264,11 @@ void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n
 void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const TransportResult* result,
                    const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
-                   double c1, double b, double hdt, double* q_base, double* p_base)
+                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
     k_commit<<<(n + 127) / 128, 128, 0, L.s>>>(n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
-                                               c1, b, hdt, q_base, p_base);
+                                               c1, b, hdt, q_base, p_base, dF, dF_out);
     LSD_COUNT(L);
     prof_end(L, pid);
 }

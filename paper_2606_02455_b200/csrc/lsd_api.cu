@@ -22,6 +22,7 @@ struct WindowSlot {
     int drafted = 0, verified = 0;
     uint64_t n0 = 0;                                         // step index of the window's start state ...
     uint64_t* n0_dev = nullptr;                              // ... and its device copy, read by the Philox-keyed kernels
+    double* dF = nullptr;                                    // [3][n] EC cache as it stood when this window was drafted (Alg. 3)
     std::map<int, GraphEntry> g_roll, g_verify, g_transport; // by K
     double *qstart = nullptr, *pstart = nullptr;             // [3][n]
     double *qhalf = nullptr, *Ft = nullptr, *yq = nullptr, *yp = nullptr;   // [kmax][3][n]
@@ -62,6 +63,8 @@ struct lsd_ctx {
     VerletList vl_eval_mlip, vl_eval_pair;
     cudaStream_t side = nullptr;
     int64_t launches = 0;
+    int ec = 0;                                              // speculative error correction (Alg. 3) on / off
+    double* dF = nullptr;                                    // [3][n] EC cache: F - F~(bare) of the last committed step
     bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
     Prof prof;
     lsd_stats stats{};
@@ -462,10 +465,12 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
         TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
         TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
         TRY(dalloc(ctx, &w.img, n)); TRY(dalloc(ctx, &w.flags, 1)); TRY(dalloc(ctx, &w.n0_dev, 1));
+        TRY(dalloc(ctx, &w.dF, n3)); CK(cudaMemset(w.dF, 0, n3 * sizeof(double)));
         CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
     }
     for (int w = 0; w < 2; ++w) if (ctx->pot[w].mlip.F > 0) TRY(alloc_work(ctx, ctx->pot[w].mlip, ctx->work[w], ctx->bmax[w]));
     TRY(dalloc(ctx, &ctx->Fg, n3 * kmax));
+    TRY(dalloc(ctx, &ctx->dF, n3)); CK(cudaMemset(ctx->dF, 0, n3 * sizeof(double)));
     ctx->nblk = transport_blocks(n);
     TRY(dalloc(ctx, &ctx->partial, (size_t)2 * ctx->nblk * kmax));
     TRY(dalloc(ctx, &ctx->S1, kmax)); TRY(dalloc(ctx, &ctx->S2, kmax)); TRY(dalloc(ctx, &ctx->ell, kmax)); TRY(dalloc(ctx, &ctx->lnu, kmax));
@@ -518,12 +523,14 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
     if (ctx->pending == 0) {
         CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         CK(cudaMemcpyAsync(w.pstart, ctx->p, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        if (ctx->ec) CK(cudaMemcpyAsync(w.dF, ctx->dF, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         w.n0 = (uint64_t)ctx->step;
     } else {                                                                  // speculative: continue from y_K of the unverified window
         WindowSlot& pv = ctx->slot[si ^ 1];
         CK(cudaStreamWaitEvent(st, pv.ev_drafted, 0));
         CK(cudaMemcpyAsync(w.qstart, pv.yq + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         CK(cudaMemcpyAsync(w.pstart, pv.yp + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        if (ctx->ec) CK(cudaMemcpyAsync(w.dF, pv.dF, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));   // the cache has not seen the unverified window
         w.n0 = pv.n0 + (uint64_t)pv.K;
     }
     launch_set_u64(L, w.n0_dev, w.n0);
@@ -539,7 +546,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
             launch_half_a(Lg, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
             eval_forces(ctx, Lg, LSD_DRAFT, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
             launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
-                         ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1));
+                         ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ctx->ec ? w.dF : nullptr);
         }
         return LSD_OK;
     }));
@@ -581,9 +588,9 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
     TRY(run_graphed(ctx, st, w.g_transport[K], [&]() -> lsd_status {
         Launcher Lg = mk(ctx, stream);
         launch_transport(Lg, n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk, ctx->S1, ctx->S2,
-                         ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
+                         ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr);
         launch_commit(Lg, n, K, ctx->cfg.seed, w.n0_dev, ctx->result, ctx->S1, ctx->S2, w.Ft, ctx->Fg, w.qhalf, w.pstart, w.yq, w.yp,
-                      ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p);
+                      ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p, ctx->ec ? w.dF : nullptr, ctx->ec ? ctx->dF : nullptr);
         return LSD_OK;
     }));
     CK(cudaMemcpyAsync(ctx->result_host, ctx->result, sizeof(TransportResult), cudaMemcpyDeviceToHost, st));
@@ -670,7 +677,36 @@ lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t
     CK(cudaMemcpy(ctx->q, q, bytes, kind));
     CK(cudaMemcpy(ctx->p, p, bytes, kind));
     ctx->step = step; ctx->stats.step = step;
+    CK(cudaMemset(ctx->dF, 0, bytes));                        // a new trajectory starts with an empty EC cache
     ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
+    return LSD_OK;
+}
+
+lsd_status lsd_set_error_correction(lsd_ctx* ctx, int32_t enable)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    ctx->ec = enable ? 1 : 0;
+    CK(cudaMemset(ctx->dF, 0, (size_t)3 * ctx->sys.n * sizeof(double)));
+    drop_graphs(ctx);                                        // the captured kernels take the cache pointer (or null) by value
+    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
+    return LSD_OK;
+}
+
+lsd_status lsd_get_ec_cache(lsd_ctx* ctx, double* dF, int32_t where)
+{
+    if (!ctx || !dF) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    return copy_out(ctx, dF, ctx->dF, (size_t)3 * ctx->sys.n * sizeof(double), where);
+}
+
+lsd_status lsd_set_ec_cache(lsd_ctx* ctx, const double* dF, int32_t where)
+{
+    if (!ctx || !dF) return LSD_ERR_INVALID_ARG;
+    if (!ctx->ec) return fail(ctx, LSD_ERR_STATE, "error correction is off (lsd_set_error_correction)");
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(ctx->dF, dF, (size_t)3 * ctx->sys.n * sizeof(double), where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice));
+    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0;
     return LSD_OK;
 }
 
@@ -716,7 +752,7 @@ lsd_status lsd_get_window_debug(lsd_ctx* ctx, int32_t what, void* out, int32_t w
         case LSD_DBG_XI: {
             if (!ctx->xi_dbg) TRY(dalloc(ctx, &ctx->xi_dbg, (size_t)3 * ctx->sys.n * ctx->cfg.k_max));
             launch_transport(mk(ctx, nullptr), ctx->sys.n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk,
-                             ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg);
+                             ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr);
             CK(cudaDeviceSynchronize());
             return copy_out(ctx, out, ctx->xi_dbg, big, where);
         }

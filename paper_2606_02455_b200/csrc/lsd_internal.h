@@ -147,16 +147,16 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
 void launch_set_u64(Launcher L, uint64_t* dst, uint64_t v);
 void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
-                  double* q_new, double* p_new);
+                  double* q_new, double* p_new, const double* dF /*EC cache or null*/);
 void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p);
 struct TransportResult { int first_reject, n_commit, flags, pad; double beta_sum; };
 void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_dev, const double* Ft, const double* Fg,
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
-                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg);
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF);
 void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_dev, const TransportResult* result,
                    const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
-                   double c1, double b, double hdt, double* q_base, double* p_base);
+                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out);
 int transport_blocks(int n);
 
 // ---- neighbor.cu
