@@ -238,6 +238,29 @@ def main():
     ms, committed_all = reduce_over_ranks(ms, committed, device="cuda")
     value = K * N * args.steps * world / (ms * 1e-3)
 
+    # ---- the serial baselines of the paper's speed-up definition: plain Langevin with the target alone and
+    # with the draft alone, same kernels, same stream; c = t_draft / t_target (:155); synchronous-window prediction Eq. 21
+    # (:559) without the bonus step (R3).  Context only: alpha and c are those of the synthetic models.
+    def plain_rate(which):
+        nst = K * max(1, min(args.steps, 8))
+        P.lsd_plain_langevin(ctx.h, which, K, stream)                      # warm (graph capture on the second chunk)
+        P.lsd_plain_langevin(ctx.h, which, K, stream)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        P.lsd_plain_langevin(ctx.h, which, nst, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        return nst / (a.elapsed_time(b) * 1e-3)
+    st_all = P.lsd_get_stats(ctx.h)
+    alpha = 1.0 - st_all["rejections"] / max(st_all["committed_steps"], 1)
+    plain_t, plain_d = plain_rate(P.LSD_TARGET), plain_rate(P.LSD_DRAFT)
+    cfrac = plain_t / plain_d
+    pred = (K if alpha >= 1.0 else (1.0 - alpha ** K) / (1.0 - alpha)) / (K * cfrac + 1.0)
+    committed_rate = committed_all / world / (ms * 1e-3)
+    speedup = dict(plain_target_md_steps_per_s=plain_t, plain_draft_md_steps_per_s=plain_d, cost_fraction_c=cfrac, acceptance_alpha=alpha,
+                   measured_speedup_vs_plain_target=committed_rate / plain_t, eq21_sync_prediction_K_target_instances=pred,
+                   note="one B200 evaluates the K target calls as ONE batched call, not on K instances: Eq. 21 is the paper's multi-GPU model")
+
     # ---- end-to-end through the C ABI with HOST buffers (pinned): upload x_n, run the window, read x_{n+commit} back
     qh = torch.empty((3, N), dtype=torch.float64).pin_memory()
     ph = torch.empty((3, N), dtype=torch.float64).pin_memory()
@@ -290,7 +313,7 @@ def main():
                                 l2="flushed between timed steps (256 MiB write)" if need_flush else "working set larger than L2",
                                 overlap=bool(args.overlap), error_correction=bool(args.ec), replicas=world, peaks=peaks["source"]),
                     committed_md_steps_per_s=committed_all / (ms * 1e-3), committed_per_window=committed_all / (args.steps * world),
-                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline)
+                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, speedup=speedup)
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = {k: v for k, v in cpu_baseline(args.workload).items() if k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))

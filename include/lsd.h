@@ -149,6 +149,14 @@ lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject);
  * (the last window is shortened).  Synchronous. */
 lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream);
 
+/* Plain Langevin dynamics (no speculation): n_steps ABOBA steps (Eq. 2) with the forces of potential `which`
+ * (LSD_TARGET: the serial baseline in the paper's definition of speed-up; LSD_DRAFT: the draft alone) from
+ * the base state, same kernels and same noise keying as the draft rollout (R5), committed in chunks of k_max steps that
+ * share one neighbour list; synchronises once per chunk.  With `which` = LSD_TARGET the trajectory equals LSD with
+ * draft = target.  Errors: STATE (a drafted window is pending), SKIN_VIOLATED / NBR_OVERFLOW / NONFINITE (the base state
+ * is then undefined: restore it with lsd_set_state). */
+lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void* stream);
+
 /* Base state x_n: q, p [3][n_atoms] (either may be NULL), *step = n.  Synchronises. */
 lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int32_t where);
 lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t step, int32_t where);

@@ -23,7 +23,7 @@ struct WindowSlot {
     uint64_t n0 = 0;                                         // step index of the window's start state ...
     uint64_t* n0_dev = nullptr;                              // ... and its device copy, read by the Philox-keyed kernels
     double* dF = nullptr;                                    // [3][n] EC cache as it stood when this window was drafted (Alg. 3)
-    std::map<int, GraphEntry> g_roll, g_verify, g_transport; // by K
+    std::map<int, GraphEntry> g_roll, g_verify, g_transport, g_plain; // by K (g_plain: by 2 K + which)
     double *qstart = nullptr, *pstart = nullptr;             // [3][n]
     double *qhalf = nullptr, *Ft = nullptr, *yq = nullptr, *yp = nullptr;   // [kmax][3][n]
     int* img = nullptr;                                      // [n] images of the reference (start) state
@@ -108,7 +108,7 @@ Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, 
 void drop_graphs(lsd_ctx* ctx)
 {
     for (int s = 0; s < 2; ++s)
-        for (auto* m : {&ctx->slot[s].g_roll, &ctx->slot[s].g_verify, &ctx->slot[s].g_transport}) {
+        for (auto* m : {&ctx->slot[s].g_roll, &ctx->slot[s].g_verify, &ctx->slot[s].g_transport, &ctx->slot[s].g_plain}) {
             for (auto& kv : *m) if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
             m->clear();
         }
@@ -362,6 +362,29 @@ lsd_status copy_out(lsd_ctx* ctx, void* dst, const void* src_dev, size_t bytes, 
     return LSD_OK;
 }
 
+// K serial ABOBA steps (PAPER.md:584-593 DRAFT_STEP; Eq. 2, Eq. 7) with the forces of potential `which` from the slot's start
+// state: window-shared lists, then per step A(1/2), forces, B O B + A(1/2).  Stream-ordered launches only (capturable).
+lsd_status rollout_body(lsd_ctx* ctx, WindowSlot& w, int K, int which, void* stream, bool ec)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = ctx->sys.n;
+    const size_t n3 = (size_t)3 * n;
+    Launcher Lg = mk(ctx, stream);
+    CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
+    build_lists(ctx, Lg, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
+    const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
+    for (int j = 1; j <= K; ++j) {                                            // serial in j
+        const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
+        const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
+        double* qh = w.qhalf + n3 * (j - 1);
+        launch_half_a(Lg, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
+        eval_forces(ctx, Lg, which, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
+        launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
+                     ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ec ? w.dF : nullptr);
+    }
+    return LSD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -534,22 +557,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
         w.n0 = pv.n0 + (uint64_t)pv.K;
     }
     launch_set_u64(L, w.n0_dev, w.n0);
-    TRY(run_graphed(ctx, st, w.g_roll[K], [&]() -> lsd_status {
-        Launcher Lg = mk(ctx, stream);
-        CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
-        build_lists(ctx, Lg, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
-        const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
-        for (int j = 1; j <= K; ++j) {                                        // serial in j
-            const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
-            const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
-            double* qh = w.qhalf + n3 * (j - 1);
-            launch_half_a(Lg, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
-            eval_forces(ctx, Lg, LSD_DRAFT, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
-            launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
-                         ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ctx->ec ? w.dF : nullptr);
-        }
-        return LSD_OK;
-    }));
+    TRY(run_graphed(ctx, st, w.g_roll[K], [&]() -> lsd_status { return rollout_body(ctx, w, K, LSD_DRAFT, stream, ctx->ec != 0); }));
     ctx->cl_img[LSD_DRAFT] = w.img;                                           // (set by eval_forces only when the body runs)
     CK(cudaEventRecord(w.ev_drafted, st));
     w.K = K; w.drafted = 1; w.verified = 0;
@@ -654,6 +662,35 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
         }
     }
     if (ctx->pending) { CK(cudaStreamSynchronize(ctx->side)); ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; }
+    return LSD_OK;
+}
+
+lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void* stream)
+{
+    if (!ctx || (which != LSD_DRAFT && which != LSD_TARGET) || n_steps < 0) return LSD_ERR_INVALID_ARG;
+    if (ctx->pending) return fail(ctx, LSD_ERR_STATE, "a drafted window is pending");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n3 = (size_t)3 * ctx->sys.n;
+    WindowSlot& w = ctx->slot[ctx->verify_idx];
+    int64_t remaining = n_steps;
+    while (remaining > 0) {
+        const int K = (int)std::min<int64_t>(ctx->cfg.k_max, remaining);
+        if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
+        CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(w.pstart, ctx->p, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        w.n0 = (uint64_t)ctx->step;
+        launch_set_u64(mk(ctx, stream), w.n0_dev, w.n0);
+        TRY(run_graphed(ctx, st, w.g_plain[2 * K + which], [&]() -> lsd_status { return rollout_body(ctx, w, K, which, stream, false); }));
+        CK(cudaMemcpyAsync(ctx->q, w.yq + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(ctx->p, w.yp + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        int flags = 0;
+        CK(cudaMemcpyAsync(&flags, w.flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (flags) return flags_to_status(ctx, flags);            // the chunk's states are not to be trusted (the base state was overwritten)
+        ctx->step += K; ctx->stats.step = ctx->step;
+        remaining -= K;
+    }
+    w.drafted = 0; w.verified = 0;
     return LSD_OK;
 }
 

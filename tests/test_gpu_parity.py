@@ -318,3 +318,31 @@ def test_call_order_is_enforced(P):
     with pytest.raises(P.LsdError):
         P.lsd_draft_rollout(ctx.h, 99)
     ctx.close()
+
+
+def test_plain_langevin_is_lsd_with_draft_equal_target_and_matches_the_oracle(P, orc):
+    """lsd_plain_langevin(LSD_TARGET): the serial baseline.  Same kernels and noise keying as the rollout, so it equals LSD
+    with draft = target bit for bit (north_star: "the trajectory equals plain target Langevin under the same noise"), and
+    the oracle's plain ABOBA (cfg1, fp64) to round-off."""
+    w = L.make_workload("cfg1")
+    p0 = orc.initial_momenta(w)
+    ctx = P.context_from_workload(w, p0=p0)
+    P.lsd_plain_langevin(ctx.h, P.LSD_TARGET, 50)
+    qa, pa, step = ctx.state()
+    assert step == 50
+    ref = orc.run_aboba(w, w.target, w.q0, p0, 50)
+    assert np.abs(qa.T - ref["q"]).max() <= 1e-9 and np.abs(pa.T - ref["p"]).max() <= 1e-9 * np.abs(ref["p"]).max()
+    ctx.close()
+    wt = L.with_target_as_draft(w)
+    ctx = P.context_from_workload(wt, p0=p0)
+    n = 0
+    while n < 50:
+        l, nc = ctx.window(min(4, 50 - n))
+        assert l == 0
+        n += nc
+    qb, pb, _ = ctx.state()
+    assert np.array_equal(qa, qb) and np.array_equal(pa, pb)
+    with pytest.raises(P.LsdError):
+        P.lsd_draft_rollout(ctx.h, 4)
+        P.lsd_plain_langevin(ctx.h, P.LSD_TARGET, 4)             # STATE: a drafted window is pending
+    ctx.close()
