@@ -148,13 +148,17 @@ lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject);
  * internal stream when overlap != 0), transport, rollback} until n_steps more steps are committed
  * (the last window is shortened).  Synchronous. */
 lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream);
+/* lsd_run with K = 0: adaptive lookahead (the window length is the paper's free parameter L): K moves
+ * over {1, 2, 4, ..., k_max} by hill climbing on the measured committed steps per second.  With error correction off the
+ * committed trajectory does not depend on the K sequence (R5).  lsd_get_adaptive_k: the length it last settled on (0: never). */
+int32_t lsd_get_adaptive_k(const lsd_ctx* ctx);
 
 /* Plain Langevin dynamics (no speculation): n_steps ABOBA steps (Eq. 2) with the forces of potential `which`
  * (LSD_TARGET: the serial baseline in the paper's definition of speed-up; LSD_DRAFT: the draft alone) from
  * the base state, same kernels and same noise keying as the draft rollout (R5), committed in chunks of k_max steps that
  * share one neighbour list; synchronises once per chunk.  With `which` = LSD_TARGET the trajectory equals LSD with
- * draft = target.  Errors: STATE (a drafted window is pending), SKIN_VIOLATED / NBR_OVERFLOW / NONFINITE (the base state
- * is then undefined: restore it with lsd_set_state). */
+ * draft = target.  A skin violation or row overflow inside a chunk is answered like in lsd_run (lists rebuilt with a larger
+ * skin, chunk repeated).  Errors: STATE (a drafted window is pending), NONFINITE (the base state is the last good one). */
 lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void* stream);
 
 /* Base state x_n: q, p [3][n_atoms] (either may be NULL), *step = n.  Synchronises. */

@@ -22,7 +22,7 @@ _STATUS = {0: "LSD_OK", -1: "LSD_ERR_INVALID_ARG", -2: "LSD_ERR_CUDA", -3: "LSD_
 EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_rollout", "lsd_verify_window", "lsd_transport_accept",
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
-                    "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin"]
+                    "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k"]
 
 
 class LsdError(RuntimeError):
@@ -169,6 +169,10 @@ def lsd_rollback(h, first_reject):
 
 def lsd_run(h, n_steps, K, overlap=True, stream=None):
     _check(h, load_library().lsd_run(h, C.c_int64(n_steps), C.c_int32(K), C.c_int32(int(overlap)), _stream(stream)))
+
+
+def lsd_get_adaptive_k(h) -> int:
+    return int(load_library().lsd_get_adaptive_k(h))
 
 
 def lsd_plain_langevin(h, which, n_steps, stream=None):

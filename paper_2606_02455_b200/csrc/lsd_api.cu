@@ -1,5 +1,6 @@
 // C ABI of liblsd_b200.so (include/lsd.h): context, window slots, call sequencing.  No torch types, no CPU fallback.
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -63,6 +64,7 @@ struct lsd_ctx {
     VerletList vl_eval_mlip, vl_eval_pair;
     cudaStream_t side = nullptr;
     int64_t launches = 0;
+    int adaptive_k = 0;                                      // window length lsd_run's adaptive mode settled on last
     int ec = 0;                                              // speculative error correction (Alg. 3) on / off
     double* dF = nullptr;                                    // [3][n] EC cache: F - F~(bare) of the last committed step
     bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
@@ -638,7 +640,27 @@ lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject)
 lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream)
 {
     if (!ctx) return LSD_ERR_INVALID_ARG;
-    if (K < 1 || K > ctx->cfg.k_max || n_steps < 0) return fail(ctx, LSD_ERR_INVALID_ARG, "bad K or n_steps");
+    if (K < 0 || K > ctx->cfg.k_max || n_steps < 0) return fail(ctx, LSD_ERR_INVALID_ARG, "bad K or n_steps");
+    // K == 0: adaptive lookahead (the paper's lookahead L is a free parameter).
+    // Hill climbing over K in {1, 2, 4, ..., k_max} on the MEASURED committed steps per second of whole windows (host clock
+    // around windows that end in a synchronising read anyway): 8 windows per visit, a move to the better neighbour, an
+    // unexplored neighbour is visited once, the neighbours are re-measured every 64 windows.  On one GPU the batched target
+    // call costs ~K target evaluations once the batch fills the device, so large systems with low acceptance settle at K = 1;
+    // small latency-bound systems settle where the verified run length saturates.
+    const bool adaptive = K == 0;
+    constexpr int kVisit = 8, kRefresh = 64;
+    double a_nc[8] = {0}, a_t[8] = {0};                      // per log2(K): committed steps and seconds (decayed)
+    int a_idx = 0, a_in_visit = 0, a_since_refresh = 0, a_home = 0;
+    int kmax_idx = 0;
+    while ((2 << kmax_idx) <= ctx->cfg.k_max && kmax_idx < 7) ++kmax_idx;
+    if (adaptive) {
+        a_idx = ctx->adaptive_k > 0 ? (int)std::lround(std::log2((double)ctx->adaptive_k)) : kmax_idx;
+        a_idx = std::min(std::max(a_idx, 0), kmax_idx);
+        a_home = a_idx;
+        K = 1 << a_idx;
+    }
+    auto rate = [&](int i) { return a_t[i] > 0 ? a_nc[i] / a_t[i] : -1.0; };
+    std::chrono::steady_clock::time_point t_win = std::chrono::steady_clock::now();
     int64_t remaining = n_steps;
     while (remaining > 0) {
         if (ctx->pending == 0) TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining), stream));
@@ -656,6 +678,33 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
         TRY(ts);
         TRY(lsd_rollback(ctx, l));
         remaining -= nc;
+        if (adaptive) {
+            const auto now = std::chrono::steady_clock::now();
+            const double dt = std::chrono::duration<double>(now - t_win).count();
+            t_win = now;
+            if (k == (1 << a_idx)) { a_nc[a_idx] = 0.9 * a_nc[a_idx] + nc; a_t[a_idx] = 0.9 * a_t[a_idx] + dt; }   // (shortened last windows do not count)
+            ++a_since_refresh;
+            if (++a_in_visit >= kVisit) {
+                a_in_visit = 0;
+                if (a_idx != a_home) {                       // back from a visit: stay if it was better
+                    if (rate(a_idx) > rate(a_home)) a_home = a_idx;
+                    a_idx = a_home;
+                } else {
+                    const int lo = a_home - 1, hi = a_home + 1;
+                    if (a_since_refresh >= kRefresh) { a_since_refresh = 0; if (lo >= 0) a_t[lo] = 0; if (hi <= kmax_idx) a_t[hi] = 0; }
+                    if (lo >= 0 && rate(lo) < 0) a_idx = lo;                 // unexplored (or due for a refresh)
+                    else if (hi <= kmax_idx && rate(hi) < 0) a_idx = hi;
+                    else {
+                        if (lo >= 0 && rate(lo) > rate(a_home)) a_home = lo;
+                        else if (hi <= kmax_idx && rate(hi) > rate(a_home)) a_home = hi;
+                        a_idx = a_home;
+                    }
+                }
+                const int newK = 1 << a_idx;
+                K = newK;                                    // a speculative window already in flight keeps its own length (slot.K)
+                ctx->adaptive_k = 1 << a_home;
+            }
+        }
         if (ctx->pending == 1 && ctx->slot[ctx->verify_idx].K > remaining) {   // cannot happen with the K choice above; defensive
             CK(cudaStreamSynchronize(ctx->side));
             ctx->pending = 0; ctx->slot[ctx->verify_idx].drafted = 0;
@@ -664,6 +713,8 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
     if (ctx->pending) { CK(cudaStreamSynchronize(ctx->side)); ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; }
     return LSD_OK;
 }
+
+int32_t lsd_get_adaptive_k(const lsd_ctx* ctx) { return ctx ? ctx->adaptive_k : 0; }
 
 lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void* stream)
 {
@@ -681,12 +732,17 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
         w.n0 = (uint64_t)ctx->step;
         launch_set_u64(mk(ctx, stream), w.n0_dev, w.n0);
         TRY(run_graphed(ctx, st, w.g_plain[2 * K + which], [&]() -> lsd_status { return rollout_body(ctx, w, K, which, stream, false); }));
-        CK(cudaMemcpyAsync(ctx->q, w.yq + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
-        CK(cudaMemcpyAsync(ctx->p, w.yp + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         int flags = 0;
         CK(cudaMemcpyAsync(&flags, w.flags, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        if (flags) return flags_to_status(ctx, flags);            // the chunk's states are not to be trusted (the base state was overwritten)
+        if (flags & (LSD_FLAG_SKIN | LSD_FLAG_OVERFLOW)) {            // as in lsd_run: answered by a rebuild with a larger skin; the base state is untouched
+            if (flags & LSD_FLAG_NONFINITE) return flags_to_status(ctx, flags);
+            TRY(lsd_set_skin(ctx, (flags & LSD_FLAG_SKIN) ? 2.0 * ctx->cfg.skin : ctx->cfg.skin));
+            continue;
+        }
+        if (flags) return flags_to_status(ctx, flags);
+        CK(cudaMemcpyAsync(ctx->q, w.yq + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(ctx->p, w.yp + n3 * (K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         ctx->step += K; ctx->stats.step = ctx->step;
         remaining -= K;
     }

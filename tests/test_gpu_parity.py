@@ -346,3 +346,24 @@ def test_plain_langevin_is_lsd_with_draft_equal_target_and_matches_the_oracle(P,
         P.lsd_draft_rollout(ctx.h, 4)
         P.lsd_plain_langevin(ctx.h, P.LSD_TARGET, 4)             # STATE: a drafted window is pending
     ctx.close()
+
+
+def test_adaptive_lookahead_does_not_change_the_trajectory(P, orc):
+    """lsd_run with K = 0 chooses the window length by measurement; with noise keyed by the step index (R5) the committed
+    trajectory is the same as with any fixed K, with and without the speculative second-stream rollout."""
+    import torch
+    w = L.make_workload("cfg2")
+    p0 = orc.initial_momenta(w)
+    finals = []
+    for K, overlap in ((16, False), (0, False), (0, True)):
+        ctx = P.context_from_workload(w, k_max=16, precision=P.LSD_FP32, p0=p0)
+        stream = torch.cuda.Stream()
+        P.lsd_run(ctx.h, 300, K, overlap=overlap, stream=stream)
+        q, p, step = ctx.state()
+        assert step == 300
+        if K == 0:
+            assert P.lsd_get_adaptive_k(ctx.h) in (1, 2, 4, 8, 16)
+        finals.append((q, p))
+        ctx.close()
+    for q, p in finals[1:]:
+        assert np.array_equal(q, finals[0][0]) and np.array_equal(p, finals[0][1])
