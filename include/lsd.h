@@ -169,6 +169,13 @@ lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out);
 /* Committed state j (1..n_commit) of the window most recently passed to lsd_transport_accept. */
 lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where);
 
+/* (OBABO) output of committed step j (1 <= j <= n_commit) of the window lsd_transport_accept handled last, recovered by time
+ * staggering (App. F :632-753): q = q_half_j (:753), p = p_mid of Eq. 30 from the committed
+ * momenta before and after the step, the target force F_j already evaluated by the verification (no force call) and one
+ * extra normal per component drawn from Philox stream tag 3 at step index n0 + j (R18).  Valid until the next
+ * lsd_verify_window (it overwrites F).  q, p: [3][n_atoms] or NULL; `where` = LSD_HOST | LSD_DEVICE.  Synchronises. */
+lsd_status lsd_get_window_obabo(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where);
+
 /* Speculative error correction, EC (App. E :626-630; Alg. 3 :663-717), window form:
  * the draft kick uses F~ + dF, the transport map uses delta = (b/sigma)(F~ + dF - F), and after every window the cache
  * becomes dF = F - F~ (BARE draft output, :628) of the window's last committed step.  A window uses the cache as it stood

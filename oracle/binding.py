@@ -242,6 +242,16 @@ def lsd_window(w, q, p, n0, K=None, draft=None, target=None, par=None, debug=Tru
                 q_half=qh, Ft=Ft, F=Fg, S1=S1, S2=S2, ell=ell, lnu=lnu, reject=rej, dF=dF)
 
 
+def obabo_momentum(w, step, p_prev, p_new, F, par=None):
+    """(OBABO) output momentum of committed step `step` (App. F Eq. 26-30); arrays [N,3]."""
+    s = System(w)
+    par = par or params(w)
+    out = np.zeros((s.n, 3))
+    a, b, c = (np.ascontiguousarray(x, np.float64) for x in (p_prev, p_new, F))
+    lib().orc_obabo_momentum(C.byref(s.c), C.byref(par), C.c_uint64(step), _dp(a), _dp(b), _dp(c), _dp(out))
+    return out
+
+
 def run_lsd(w, q, p, n_steps, K=None, draft=None, target=None, par=None, keep_traj=True, ec=False):
     s = System(w)
     D, T = Pot(draft or w.draft), Pot(target or w.target)

@@ -778,3 +778,39 @@ int64_t orc_run_lsd_ec(const orc_system *sys, const orc_params *par, const orc_p
     free(tq); free(tp); free(S2);
     return n;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * O-6: (OBABO) output momentum of a committed step by time staggering
+ * (App. F :632-753).  The ABOBA run already contains the staggered states: after the B O B
+ * block of step n the state is ybar_n = (q_half_n, p_n), and A(dt) = A(1/2) A(1/2) leads to q_half_{n+1}
+ * (Eq. 25 :652).  With F = F_target(q_half_n) (known from the verification, :735), p_prev = pbar_{n-1},
+ * p_new = pbar_n:
+ *   Sigma_half = M kT (1 - e^{-gamma dt})                                   (:648)
+ *   w      = Sigma_half^{-1/2} (p_new - e^{-gamma dt} p_prev - (1 + e^{-gamma dt}) (dt/2) F)      Eq. 28
+ *   xi1*   ~ N( e^{-gamma dt/2} / (1 + e^{-gamma dt}) w ,  1 / (1 + e^{-gamma dt}) I )             Eq. 29
+ *   p_mid  = e^{-gamma dt/2} (p_prev + (dt/2) F) + Sigma_half^{1/2} xi1*                           Eq. 30
+ * and the OBABO output position is q_half_n (:753).  [reading R18] The extra standard normal is drawn
+ * from the same counter-based generator, stream tag 3, keyed by the step index like every other draw (R5).
+ * Pins (tests/test_oracle_obabo.py): stationary covariance of (q, p_mid) on the harmonic oscillator vs the
+ * discrete Lyapunov solution of the OBABO map Eq. 24 composed in numpy; the implied second half-step
+ * noise xi2 = w - e^{-gamma dt/2} xi1* is standard normal and uncorrelated with xi1*.
+ * ---------------------------------------------------------------------------------------- */
+void orc_obabo_momentum(const orc_system *sys, const orc_params *par, uint64_t step, const double *p_prev,
+                        const double *p_new, const double *F, double *p_mid)
+{
+    const int n = sys->n;
+    const double c1 = exp(-par->friction_per_fs * par->dt_fs), ch = exp(-0.5 * par->friction_per_fs * par->dt_fs);
+    const double hdt = 0.5 * par->dt_fs;
+    double *zeta = (double *)malloc(sizeof(double) * 3 * (size_t)n);
+    orc_normals(par->seed, step, n, 3u, zeta);
+    for (int i = 0; i < n; ++i) {
+        const double sh = sqrt(sys->mass_amu[i] * ORC_AMU * ORC_KB * par->temperature_K * (1.0 - c1));
+        for (int c = 0; c < 3; ++c) {
+            const int a = 3 * i + c;
+            const double w = (p_new[a] - c1 * p_prev[a] - (1.0 + c1) * hdt * F[a]) / sh;
+            const double xi1 = ch / (1.0 + c1) * w + sqrt(1.0 / (1.0 + c1)) * zeta[a];
+            p_mid[a] = ch * (p_prev[a] + hdt * F[a]) + sh * xi1;
+        }
+    }
+    free(zeta);
+}

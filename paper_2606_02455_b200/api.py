@@ -219,6 +219,11 @@ def lsd_get_window_state(h, j, q=None, p=None):
     _check(h, load_library().lsd_get_window_state(h, C.c_int32(j), qp, pp, C.c_int32(wq if q is not None else wp)))
 
 
+def lsd_get_window_obabo(h, j, q=None, p=None):
+    (qp, wq), (pp, wp) = _ptr(q), _ptr(p)
+    _check(h, load_library().lsd_get_window_obabo(h, C.c_int32(j), qp, pp, C.c_int32(wq if q is not None else wp)))
+
+
 def lsd_get_window_debug(h, what, out):
     ptr, where = _ptr(out)
     _check(h, load_library().lsd_get_window_debug(h, C.c_int32(DBG[what] if isinstance(what, str) else what), ptr, C.c_int32(where)))

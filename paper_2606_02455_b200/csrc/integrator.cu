@@ -207,7 +207,35 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
     }
 }
 
+// (OBABO) output momentum of committed step j of the window by time staggering (App. F Eq. 26-30, :700-753):
+// w = Sigma_half^{-1/2}(p_new - c1 p_prev - (1 + c1)(dt/2) F);  xi1* = ch/(1 + c1) w + (1 + c1)^{-1/2} zeta (zeta: Philox tag 3);
+// p_mid = ch (p_prev + (dt/2) F) + Sigma_half^{1/2} xi1*,  Sigma_half = m kT (1 - c1), ch = e^{-gamma dt/2}, c1 = e^{-gamma dt}.
+__global__ void k_obabo(int n, uint64_t seed, const uint64_t* __restrict__ n0p, uint64_t j, const double* __restrict__ p_prev,
+                        const double* __restrict__ p_new, const double* __restrict__ F, const double* __restrict__ mass,
+                        double kT, double c1, double ch, double hdt, double* __restrict__ p_mid)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double zeta[3];
+    normals3(seed, *n0p + j, (uint32_t)i, 3u, zeta);
+    const double sh = sqrt(mass[i] * kT * (1.0 - c1));
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double pp = p_prev[c * n + i], f = F[c * n + i];
+        const double w = (p_new[c * n + i] - c1 * pp - (1.0 + c1) * hdt * f) / sh;
+        const double xi1 = ch / (1.0 + c1) * w + sqrt(1.0 / (1.0 + c1)) * zeta[c];
+        p_mid[c * n + i] = ch * (pp + hdt * f) + sh * xi1;
+    }
+}
+
 }  // namespace
+
+void launch_obabo(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* p_new,
+                  const double* F, const double* mass, double kT, double c1, double ch, double hdt, double* p_mid)
+{
+    k_obabo<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, p_new, F, mass, kT, c1, ch, hdt, p_mid);
+    LSD_COUNT(L);
+}
 
 int transport_blocks(int n)
 {

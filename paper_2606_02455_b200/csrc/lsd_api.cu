@@ -53,6 +53,7 @@ struct lsd_ctx {
     double rc_mlip_max = 0, rc_pair_max = 0;
     int cap_mlip = 0, cap_pair = 0;
     double* Fg = nullptr;
+    double* obabo_p = nullptr;                               // scratch of lsd_get_window_obabo
     double *partial = nullptr, *S1 = nullptr, *S2 = nullptr, *ell = nullptr, *lnu = nullptr, *xi_dbg = nullptr;
     int* reject = nullptr;
     int nblk = 1;
@@ -807,6 +808,27 @@ lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out)
 {
     if (!ctx || !out) return LSD_ERR_INVALID_ARG;
     *out = ctx->stats; out->step = ctx->step;
+    return LSD_OK;
+}
+
+lsd_status lsd_get_window_obabo(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where)
+{
+    if (!ctx) return LSD_ERR_INVALID_ARG;
+    if (ctx->last_slot < 0) return fail(ctx, LSD_ERR_STATE, "no window has been transported yet");
+    if (j < 1 || j > ctx->last_nc) return fail(ctx, LSD_ERR_INVALID_ARG, "j must be in 1..n_commit");
+    CK(cudaDeviceSynchronize());
+    const WindowSlot& w = ctx->slot[ctx->last_slot];
+    const int n = ctx->sys.n;
+    const size_t n3 = (size_t)3 * n;
+    if (q) TRY(copy_out(ctx, q, w.qhalf + n3 * (j - 1), n3 * sizeof(double), where));      // the (B O B) block leaves positions fixed (:753)
+    if (p) {
+        if (!ctx->obabo_p) TRY(dalloc(ctx, &ctx->obabo_p, n3));
+        launch_obabo(mk(ctx, nullptr), n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, j == 1 ? w.pstart : w.yp + n3 * (j - 2), w.yp + n3 * (j - 1),
+                     ctx->Fg + n3 * (j - 1), ctx->sys.mass, ctx->kT, ctx->c1, std::exp(-0.5 * ctx->cfg.friction_per_fs * ctx->cfg.dt_fs), ctx->hdt,
+                     ctx->obabo_p);
+        CK(cudaDeviceSynchronize());
+        TRY(copy_out(ctx, p, ctx->obabo_p, n3 * sizeof(double), where));
+    }
     return LSD_OK;
 }
 

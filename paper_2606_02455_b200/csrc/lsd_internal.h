@@ -158,6 +158,8 @@ void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_d
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
                    double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out);
 int transport_blocks(int n);
+void launch_obabo(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* p_new,
+                  const double* F, const double* mass, double kT, double c1, double ch, double hdt, double* p_mid);
 
 // ---- neighbor.cu
 void cellgrid_setup(CellGrid& g, const SysDev& sys, double rc_skin);

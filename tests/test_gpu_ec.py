@@ -145,3 +145,35 @@ def test_ec_graph_replay_and_overlap_are_deterministic(P, orc, monkeypatch):
         ctx.close()
     for a, b in ((0, 1), (2, 3)):
         assert np.array_equal(out[a][0], out[b][0]) and np.array_equal(out[a][1], out[b][1]) and out[a][2] == out[b][2]
+
+
+@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", {})])
+def test_obabo_outputs_match_the_oracle(P, orc, name, kw):
+    """lsd_get_window_obabo (App. F Eq. 26-30): q = q_half_j, p = p_mid recovered from the GPU's own committed momenta and
+    target forces; the oracle's recovery on the same arrays (same Philox tag-3 draw) agrees to round-off, for accepted and
+    for overridden steps."""
+    w = L.make_workload(name, **kw)
+    p0 = orc.initial_momenta(w)
+    K = 8 if name == "cfg2" else 4
+    ctx = P.context_from_workload(w, k_max=K, precision=P.LSD_FP32, p0=p0)
+    p_base, n = p0, 0
+    saw_override = False
+    for win in range(12):
+        P.lsd_draft_rollout(ctx.h, K); P.lsd_verify_window(ctx.h, K)
+        l, nc = P.lsd_transport_accept(ctx.h, K)
+        qh, Fg = ctx.debug("q_half", K), ctx.debug("F_target", K)
+        prev = p_base
+        for j in range(1, nc + 1):
+            qs, ps = np.empty((3, w.n_atoms)), np.empty((3, w.n_atoms))
+            P.lsd_get_window_state(ctx.h, j, qs, ps)
+            qo, po = np.empty((3, w.n_atoms)), np.empty((3, w.n_atoms))
+            P.lsd_get_window_obabo(ctx.h, j, qo, po)
+            assert np.array_equal(qo, qh[j - 1])
+            ref = orc.obabo_momentum(w, n + j, prev, ps.T, Fg[j - 1].T)
+            assert np.abs(po.T - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max())
+            prev = ps.T.copy()
+        saw_override |= l != 0
+        P.lsd_rollback(ctx.h, l)
+        p_base, n = prev, n + nc
+    assert saw_override
+    ctx.close()
