@@ -34,7 +34,7 @@ constexpr int kR = LSD_NRBF;            // 32 = K of the first contraction (per 
 constexpr int kTeams = 4;
 constexpr int kTT = 128;                // threads per team = accumulator rows
 constexpr int kThreadsTC = kTeams * kTT;
-constexpr int kCH = 64;                 // atoms per chunk
+constexpr int kCH = 64;                 // atoms per chunk (buffers are sized for it; small batches use chunks of 16, see launch_edge_tc_f)
 constexpr int kGE = 16;                 // edge slots per group
 constexpr int kMaxGroups = kCH * (512 / kGE);   // rows hold at most 512 slots (neighbor.cu)
 
@@ -132,13 +132,14 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int F, bool BWD>
+template <int F, bool BWD, int CH>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
 {
+    static_assert(CH <= kCH && CH % (128 / F) == 0, "chunk size");
     using C = TcCfg<F, BWD>;
     constexpr int Q = C::Q, GPT = C::GPT, NT = C::NT, NCOLS = C::NCOLS, ET = C::ET;
-    constexpr int AQ = kCH / Q;                        // atoms per set and chunk
+    constexpr int AQ = CH / Q;                         // atoms per set and chunk
     constexpr int TPE = kTT / ET;                      // threads per edge in the staging phase
     constexpr int KPT = kR / TPE;                      // radial basis functions per staging thread
     constexpr int RCH = F / 8;                         // 16-byte chunks per bf16 feature row
@@ -212,13 +213,13 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
         const int chunk = blockIdx.x + s_chunk[team] * gridDim.x;
         if (chunk >= nchunks) break;
         const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
-        const int g0 = b * n + ci * kCH;                               // first feature row of the chunk
-        const int natoms = min(kCH, n - ci * kCH);
-        if (tt < kCH) { const int c = tt < natoms ? a.count[g0 + tt] : 0; cnts[tt] = c; pref[tt + 1] = (c + kGE - 1) / kGE; }
+        const int g0 = b * n + ci * CH;                                // first feature row of the chunk
+        const int natoms = min(CH, n - ci * CH);
+        if (tt < CH) { const int c = tt < natoms ? a.count[g0 + tt] : 0; cnts[tt] = c; pref[tt + 1] = (c + kGE - 1) / kGE; }
         team_bar(team);
-        if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= kCH; ++i) { s += pref[i]; pref[i] = s; } }
+        if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= CH; ++i) { s += pref[i]; pref[i] = s; } }
         team_bar(team);
-        if (tt < kCH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
+        if (tt < CH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
         {   // atoms without neighbours: their sums are empty
             float* out = BWD ? a.ybar : a.m_out;
             if (out && tt < F) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * F + tt] = 0.f;
@@ -445,7 +446,7 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
         if (BWD) {
             team_bar(team);
             if (tt < natoms && cnts[tt] > 0) {
-                const int i = ci * kCH + tt;
+                const int i = ci * CH + tt;
                 const float* fp = fpart + tt * (F / 32) * 3;
                 double sx = 0.0, sy = 0.0, sz = 0.0;
 #pragma unroll
@@ -476,21 +477,32 @@ uint16_t bf16_rne(double x)
     return (uint16_t)(u >> 16);
 }
 
-template <int F>
-void launch_edge_tc_f(Launcher L, const EdgeArgs& a, bool backward)
+template <int F, int CH>
+void launch_edge_tc_ch(Launcher L, const EdgeArgs& a, bool backward)
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_edge_tc<F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, false>::Smem);
-        cudaFuncSetAttribute(k_edge_tc<F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, true>::Smem);
+        cudaFuncSetAttribute(k_edge_tc<F, false, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, false>::Smem);
+        cudaFuncSetAttribute(k_edge_tc<F, true, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, true>::Smem);
         configured = true;
     }
-    const int cps = (a.n + kCH - 1) / kCH;
+    const int cps = (a.n + CH - 1) / CH;
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(tc_num_sms(), nchunks));
-    if (backward) k_edge_tc<F, true><<<grid, kThreadsTC, TcCfg<F, true>::Smem, L.s>>>(a, cps, nchunks);
-    else k_edge_tc<F, false><<<grid, kThreadsTC, TcCfg<F, false>::Smem, L.s>>>(a, cps, nchunks);
+    if (backward) k_edge_tc<F, true, CH><<<grid, kThreadsTC, TcCfg<F, true>::Smem, L.s>>>(a, cps, nchunks);
+    else k_edge_tc<F, false, CH><<<grid, kThreadsTC, TcCfg<F, false>::Smem, L.s>>>(a, cps, nchunks);
     LSD_COUNT(L);
+}
+
+// A team works through a chunk serially (tile after tile), so a small batch (a draft step of a few thousand atoms) is spread
+// over all teams of the device with chunks of 16 atoms; the per-atom sums do not depend on the chunking (thread-serial in row
+// order), so both variants return identical bits.
+template <int F>
+void launch_edge_tc_f(Launcher L, const EdgeArgs& a, bool backward)
+{
+    const long chunks64 = (long)((a.n + kCH - 1) / kCH) * (a.total / a.n);
+    if (chunks64 < 2L * tc_num_sms() * kTeams) launch_edge_tc_ch<F, 16>(L, a, backward);
+    else launch_edge_tc_ch<F, kCH>(L, a, backward);
 }
 
 }  // namespace
