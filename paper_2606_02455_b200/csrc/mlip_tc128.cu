@@ -57,10 +57,11 @@ constexpr float kP0 = -0.49872449040412903f, kP1 = 0.2356506735086441f, kP2 = -0
 
 __device__ __forceinline__ void team_bar(int team) { asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTT) : "memory"); }
 
-template <bool BWD>
+template <bool BWD, int CH>
 __global__ void __launch_bounds__(kThreads, 1)
 k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
 {
+    static_assert(CH <= kCH, "buffers are sized for chunks of kCH atoms");
     using C = Cfg<BWD>;
     constexpr int GPT = C::GPT, NT = C::NT, NCOLS = C::NCOLS, SEG = C::SEG, RECF = C::RecFloats;
     constexpr int KPT = BWD ? 8 : 16;                  // radial basis functions per staging thread
@@ -163,13 +164,13 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         const int chunk = blockIdx.x + s_chunk[team] * gridDim.x;
         if (chunk >= nchunks) { if (tt == 0) s_done[team] = 1; team_bar(team); warp_arrive(rdy1, lane); break; }
         const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
-        const int g0 = b * n + ci * kCH;                               // first feature row of the chunk
-        const int natoms = min(kCH, n - ci * kCH);
-        if (tt < kCH) { const int c = tt < natoms ? a.count[g0 + tt] : 0; cnts[tt] = c; pref[tt + 1] = (c + kGE - 1) / kGE; }
+        const int g0 = b * n + ci * CH;                                // first feature row of the chunk
+        const int natoms = min(CH, n - ci * CH);
+        if (tt < CH) { const int c = tt < natoms ? a.count[g0 + tt] : 0; cnts[tt] = c; pref[tt + 1] = (c + kGE - 1) / kGE; }
         team_bar(team);
-        if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= kCH; ++i) { s += pref[i]; pref[i] = s; } }
+        if (tt == 0) { int s = 0; pref[0] = 0; for (int i = 1; i <= CH; ++i) { s += pref[i]; pref[i] = s; } }
         team_bar(team);
-        if (tt < kCH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
+        if (tt < CH) for (int g = pref[tt]; g < pref[tt + 1]; ++g) gatom[g] = (uint8_t)tt;
         {   // atoms without neighbours: their sums are empty
             float* out = BWD ? a.ybar : a.m_out;
             uint16_t* out16 = BWD ? a.ybar16_out : a.m16_out;
@@ -177,7 +178,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
             else if (out) for (int i = 0; i < natoms; ++i) if (cnts[i] == 0) out[(size_t)(g0 + i) * kF + tt] = 0.f;
         }
         team_bar(team);
-        const int G = pref[kCH];                                       // groups of the chunk
+        const int G = pref[CH];                                        // groups of the chunk
         const int ntiles = (G + GPT - 1) / GPT;
 
         // bulk asynchronous copy of the record groups (512 bytes each) of tile t into buffer (gt0 + t) % kRecBufs, issued by one
@@ -399,7 +400,7 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
         if (BWD) {
             team_bar(team);
             if (tt < natoms && cnts[tt] > 0) {
-                const int i = ci * kCH + tt;
+                const int i = ci * CH + tt;
                 const float* fp = fpart + tt * 4 * 3;
                 double sx = 0.0, sy = 0.0, sz = 0.0;
 #pragma unroll
@@ -424,18 +425,27 @@ int sm_count()
 
 }  // namespace
 
-void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward)
+template <int CH> static void launch_edge_tc128_ch(Launcher L, const EdgeArgs& a, bool backward)
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_edge_tc128<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<false>::Smem);
-        cudaFuncSetAttribute(k_edge_tc128<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<true>::Smem);
+        cudaFuncSetAttribute(k_edge_tc128<false, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<false>::Smem);
+        cudaFuncSetAttribute(k_edge_tc128<true, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<true>::Smem);
         configured = true;
     }
-    const int cps = (a.n + kCH - 1) / kCH;
+    const int cps = (a.n + CH - 1) / CH;
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(sm_count(), nchunks));
-    if (backward) k_edge_tc128<true><<<grid, kThreads, Cfg<true>::Smem, L.s>>>(a, cps, nchunks);
-    else k_edge_tc128<false><<<grid, kThreads, Cfg<false>::Smem, L.s>>>(a, cps, nchunks);
+    if (backward) k_edge_tc128<true, CH><<<grid, kThreads, Cfg<true>::Smem, L.s>>>(a, cps, nchunks);
+    else k_edge_tc128<false, CH><<<grid, kThreads, Cfg<false>::Smem, L.s>>>(a, cps, nchunks);
     LSD_COUNT(L);
+}
+
+// small batches (one state of a few thousand atoms) are spread over all teams with chunks of 16 atoms; the sums do not depend
+// on the chunking (thread-serial in row order)
+void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward)
+{
+    const long chunks64 = (long)((a.n + kCH - 1) / kCH) * (a.total / a.n);
+    if (chunks64 < 2L * sm_count() * kTeams) launch_edge_tc128_ch<16>(L, a, backward);
+    else launch_edge_tc128_ch<kCH>(L, a, backward);
 }
