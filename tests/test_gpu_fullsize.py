@@ -1,0 +1,81 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (cfg5: 65,536 atoms, K = 8, bf16 tcgen05
+path; cfg4: 4,096 atoms, K = 32).  The oracle cannot evaluate the 6-block network on 65,536 atoms in test time, so the forces
+are checked through properties that hold at any size and everything the oracle CAN do at full size is compared directly:
+neighbour lists (cell-list oracle, bit-exact), the transport map / decisions on the GPU's own forces, the noise."""
+import math
+
+import numpy as np
+import pytest
+
+import lsd_inputs as L
+
+pytestmark = pytest.mark.gpu
+BAND = 1e-6
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_02455_b200 as P
+    P.load_library()
+    return P
+
+
+@pytest.mark.parametrize("name", ["cfg5", "cfg4"])
+def test_full_size_window(P, orc, name):
+    import torch
+    w = L.make_workload(name)
+    K, N = w.K, w.n_atoms
+    p0 = orc.initial_momenta(w)
+    ctx = P.context_from_workload(w, precision=P.LSD_BF16_TC, p0=p0)
+    assert P.lsd_tc_enabled(ctx.h)
+    stream = torch.cuda.Stream()
+    par = orc.params(w)
+    m = (w.mass_amu * L.AMU)[:, None]
+    for win in range(2):                                        # the second window replays the captured graphs
+        q_base, p_base, n = ctx.state()
+        P.lsd_draft_rollout(ctx.h, K, stream); P.lsd_verify_window(ctx.h, K, stream)
+        l, nc = P.lsd_transport_accept(ctx.h, K, stream)
+        qh, Ft, Fg = ctx.debug("q_half", K), ctx.debug("F_draft", K), ctx.debug("F_target", K)
+        S1, S2, rej, yp = ctx.debug("S1", K), ctx.debug("S2", K), ctx.debug("reject", K), ctx.debug("yp", K)
+        assert np.isfinite(Fg).all() and np.isfinite(Ft).all()
+        # --- properties of the batched target forces at full size
+        for j in range(K):
+            tot = np.abs(Fg[j]).sum()
+            assert np.abs(Fg[j].sum(axis=1)).max() <= 1e-4 * tot / 3          # sum_i F_i = 0 (every term is a pair term)
+        # --- neighbour lists of two window states against the oracle's cell list, bit-exact (T1)
+        if win == 0:
+            for b in (0, K - 1):
+                got = P.lsd_get_neighbors(ctx.h, P.LSD_TARGET, 0, b, N)
+                want = orc.neighbors(w, np.ascontiguousarray(qh[b].T), w.target.mlip.cutoff, "cell")
+                assert np.array_equal(got[0], want[0]) and np.array_equal(got[1], want[1]) and np.array_equal(got[2], want[2])
+        # --- first A half-step from the committed base state (T4) and the transport map on the GPU's own forces (T3)
+        assert np.abs(qh[0] - (q_base + w.dt_fs / 2 * p_base / m.T)).max() <= 1e-12
+        first = 0
+        for j in range(K):
+            p_prev = p_base.T if j == 0 else yp_before[j - 1].T
+            if j == 0:
+                yp_before = yp.copy()
+            xo = orc.normals(w.seed, n + j + 1, N)
+            u = orc.uniform(w.seed, n + j + 1)
+            t = orc.transport_step(w, Ft[j].T, Fg[j].T, xo, u, p_prev, qh[j].T, par)
+            assert S1[j] == pytest.approx(t["S1"], rel=1e-9, abs=1e-9) and S2[j] == pytest.approx(t["S2"], rel=1e-10)
+            if abs(t["ell"] - math.log(u)) >= BAND:
+                assert rej[j] == t["reject"], (win, j)
+            if t["reject"] and not first:
+                first, x_q, x_p = j + 1, t["q"], t["p"]
+        assert l == first and nc == (first if first else K)
+        P.lsd_rollback(ctx.h, l)
+        qg, pg, step = ctx.state()
+        assert step == n + nc
+        if first:
+            assert np.abs(qg.T - x_q).max() <= 1e-9 and np.abs(pg.T - x_p).max() <= 1e-9 * np.abs(x_p).max()
+    # --- batch invariance at full size: one state alone == the same state inside the batch of K
+    Q = np.ascontiguousarray(qh[:2])
+    F2, _ = ctx.forces(P.LSD_TARGET, Q)
+    F1, _ = ctx.forces(P.LSD_TARGET, Q[1:2])
+    assert np.array_equal(F1[0], F2[1])
+    assert np.array_equal(F2[0], Fg[0])                         # and equal to what the (graph-replayed) verification produced
+    ctx.close()
