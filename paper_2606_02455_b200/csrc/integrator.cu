@@ -67,7 +67,8 @@ __global__ void k_half_a(int n, const double* __restrict__ q, const double* __re
 __global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, uint64_t j, const double* __restrict__ p_prev, const double* __restrict__ Ft,
                         const double* __restrict__ qhalf, const double* __restrict__ mass, const double* __restrict__ sigma,
                         double c1, double b, double hdt, double* __restrict__ q_new, double* __restrict__ p_new,
-                        const double* __restrict__ dF)
+                        const double* __restrict__ dF, double* __restrict__ qhalf_next, const double* __restrict__ qref,
+                        double skin_half2, int* flags)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -80,6 +81,19 @@ __global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, 
         const double pn = c1 * p_prev[c * n + i] + b * Fe + sg * xi[c];
         p_new[c * n + i] = pn;
         q_new[c * n + i] = qhalf[c * n + i] + hdt * pn / m;
+    }
+    if (qhalf_next) {                                // first A(1/2) of the next step of a rollout (the same arithmetic as k_half_a): one launch less per step
+        double d2 = 0.0;
+        bool bad = false;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double v = q_new[c * n + i] + hdt * p_new[c * n + i] / m;
+            qhalf_next[c * n + i] = v;
+            const double d = v - qref[c * n + i]; d2 += d * d;
+            bad |= !isfinite(v);
+        }
+        if (d2 > skin_half2) atomicOr(flags, LSD_FLAG_SKIN);
+        if (bad) atomicOr(flags, LSD_FLAG_NONFINITE);
     }
 }
 
@@ -256,10 +270,10 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
 
 void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
-                  double* q_new, double* p_new, const double* dF)
+                  double* q_new, double* p_new, const double* dF, double* qhalf_next, const double* qref, double skin_half2, int* flags)
 {
     const int pid = prof_begin(L, PROF_INTEG);
-    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new, dF);
+    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new, dF, qhalf_next, qref, skin_half2, flags);
     LSD_COUNT(L);
     prof_end(L, pid);
 }

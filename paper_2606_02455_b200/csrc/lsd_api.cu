@@ -161,6 +161,17 @@ lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
     };
     TRY(up(w, m.n_species, F, false, &d.emb));
     const double* blk = w + (size_t)m.n_species * F;
+    {   // y table of the first block (fp64 on the host, rounded once)
+        std::vector<float> yt((size_t)m.n_species * F);
+        const double* Win0 = blk;
+        for (int sp = 0; sp < m.n_species; ++sp)
+            for (int c = 0; c < F; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < F; ++k) acc += Win0[(size_t)c * F + k] * w[(size_t)sp * F + k];
+                yt[(size_t)sp * F + c] = (float)acc;
+            }
+        TRY(upload(ctx, &d.ytab0, yt.data(), yt.size()));
+    }
     const size_t per_block = (size_t)4 * F * F + (size_t)F * R;
     d.WinT.resize(T); d.Win.resize(T); d.Wf1T.resize(T); d.Wf2T.resize(T); d.Wo1T.resize(T); d.Wo1.resize(T); d.Wo2T.resize(T); d.Wo2.resize(T);
     for (int t = 0; t < T; ++t) {
@@ -258,7 +269,7 @@ lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
         w.y16.resize(net.T);
         for (int t = 0; t < net.T; ++t) TRY(dalloc(ctx, &w.y16[t], e));
         TRY(dalloc(ctx, &w.mbar16, e));
-        if (net.F == 128) { TRY(dalloc(ctx, &w.ym16, e)); TRY(dalloc(ctx, &w.ytab, (size_t)net.ns * net.F)); }
+        if (net.F == 128) TRY(dalloc(ctx, &w.ym16, e));
     }
     return LSD_OK;
 }
@@ -377,13 +388,13 @@ lsd_status rollout_body(lsd_ctx* ctx, WindowSlot& w, int K, int which, void* str
     build_lists(ctx, Lg, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
     const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
     for (int j = 1; j <= K; ++j) {                                            // serial in j
-        const double* qp = j == 1 ? w.qstart : w.yq + n3 * (j - 2);
         const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
         double* qh = w.qhalf + n3 * (j - 1);
-        launch_half_a(Lg, n, qp, pp, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
+        if (j == 1) launch_half_a(Lg, n, w.qstart, w.pstart, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
         eval_forces(ctx, Lg, which, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
         launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
-                     ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ec ? w.dF : nullptr);
+                     ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ec ? w.dF : nullptr,
+                     j < K ? w.qhalf + n3 * j : nullptr, w.qstart, sh2, w.flags);       // + the first A(1/2) of step j + 1
     }
     return LSD_OK;
 }

@@ -36,6 +36,7 @@ struct MlipDev {
     int F = 0, T = 0, R = LSD_NRBF, ns = 0;
     float rc = 0.f, alpha = 0.f;
     float* emb = nullptr;                       // [ns][F]
+    float* ytab0 = nullptr;                     // [ns][F]  W_in(0) Emb[s]: y of the first block depends on the species only
     // per block, fp32, all stored k-major [K][N] for  C[rows][N] = A[rows][K] * W[K][N]
     std::vector<float*> WinT, Win, Wf1T, Wf2T, Wo1T, Wo1, Wo2T, Wo2;
     float* Wr1 = nullptr;                       // [F/2][F]
@@ -108,7 +109,6 @@ struct MlipWork {                    // activations of one batched evaluation (k
     std::vector<uint16_t*> y16;      // [T] bf16 copies of y gathered by the tcgen05 edge kernels (LSD_BF16_TC only)
     uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
     uint32_t* ym16 = nullptr;        // width 128 only: rows of (y, mbar) bf16 pairs gathered by the backward tcgen05 kernel
-    float* ytab = nullptr;           // width 128: [ns][F] y of the first block per species
     double* e_atom = nullptr;        // [bmax*n]
 };
 
@@ -147,7 +147,9 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
 void launch_set_u64(Launcher L, uint64_t* dst, uint64_t v);
 void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* Ft,
                   const double* qhalf, const double* mass, const double* sigma, double c1, double b, double hdt,
-                  double* q_new, double* p_new, const double* dF /*EC cache or null*/);
+                  double* q_new, double* p_new, const double* dF /*EC cache or null*/,
+                  double* qhalf_next = nullptr /*also write the next step's q_half and check the skin against qref*/,
+                  const double* qref = nullptr, double skin_half2 = 0.0, int* flags = nullptr);
 void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass, double kT, double* p);
 struct TransportResult { int first_reject, n_commit, flags, pad; double beta_sum; };
 void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_dev, const double* Ft, const double* Fg,

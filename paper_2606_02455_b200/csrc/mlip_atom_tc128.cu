@@ -266,14 +266,6 @@ k_atom_tc128(AtomArgs a)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
-// y table of the first block: W_in(0) Emb[s] for every species (x(0) = Emb[s] does not depend on the positions)
-__global__ void k_ytab(int F, const float* __restrict__ emb, const float* __restrict__ WinT, float* __restrict__ ytab)
-{
-    const int s = blockIdx.x, c = threadIdx.x;
-    float acc = 0.f;
-    for (int k = 0; k < F; ++k) acc = fmaf(emb[s * F + k], WinT[k * F + c], acc);
-    ytab[s * F + c] = acc;
-}
 // x = Emb[s] (fp32) and y16 = bf16(W_in(0) Emb[s]); 4 channels per thread
 __global__ void k_embed_tc(int total, int n, const int* __restrict__ species, const float* __restrict__ emb, const float* __restrict__ ytab,
                            float* __restrict__ x, uint16_t* __restrict__ y16)
@@ -337,8 +329,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
     int pid = prof_begin(L, PROF_DENSE);
-    k_ytab<<<net.ns, kF, 0, L.s>>>(kF, net.emb, net.WinT[0], w.ytab); LSD_COUNT(L);
-    k_embed_tc<<<(int)(((size_t)total * (kF / 4) + 255) / 256), 256, 0, L.s>>>(total, sys.n, sys.species, net.emb, w.ytab, w.x, w.y16[0]); LSD_COUNT(L);
+    k_embed_tc<<<(int)(((size_t)total * (kF / 4) + 255) / 256), 256, 0, L.s>>>(total, sys.n, sys.species, net.emb, net.ytab0, w.x, w.y16[0]); LSD_COUNT(L);
     prof_end(L, pid);
     EdgeArgs ea{};
     ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs; ea.rec_zero = cl.rec_zero;

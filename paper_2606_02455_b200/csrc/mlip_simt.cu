@@ -85,12 +85,19 @@ __device__ __forceinline__ void load_weights(float* dst, const float* __restrict
 }
 
 // ------------------------------------------------------------------------------------------------ embedding (M4)
-__global__ void k_embed(int total, int n, int F, const int* __restrict__ species, const float* __restrict__ emb, float* __restrict__ x)
+
+// x = Emb[s] and the first block's y = W_in(0) Emb[s] from the per-species table (M4, M5): no contraction needed
+__global__ void k_embed_y(int total, int n, int F, const int* __restrict__ species, const float* __restrict__ emb, const float* __restrict__ ytab,
+                          float* __restrict__ x, float* __restrict__ y, uint16_t* __restrict__ y16)
 {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (size_t)total * F) return;
     const int g = (int)(t / F), f = (int)(t % F);
-    x[t] = emb[species[g % n] * F + f];
+    const int s = species[g % n];
+    x[t] = emb[s * F + f];
+    const float yv = ytab[s * F + f];
+    y[t] = yv;
+    if (y16) { const __nv_bfloat16 b = __float2bfloat16_rn(yv); y16[t] = *reinterpret_cast<const uint16_t*>(&b); }
 }
 
 // ------------------------------------------------------------------------------------------------ atom-wise layers
@@ -371,14 +378,17 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     const int sms = num_sms();
     const int grid_tiles = std::max(1, std::min(sms, (total + kWarps * 8 - 1) / (kWarps * 8)));
     const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
-    k_embed<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, w.x); LSD_COUNT(L);
+    k_embed_y<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, net.ytab0, w.x, w.y[0], use_tc ? w.y16[0] : nullptr); LSD_COUNT(L);
     EdgeArgs ea{};
     ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs; ea.rec_zero = cl.rec_zero;
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
     for (int t = 0; t < net.T; ++t) {
-        int pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t], use_tc ? w.y16[t] : nullptr); LSD_COUNT(L);
-        prof_end(L, pid);
+        int pid = -1;
+        if (t > 0) {
+            pid = prof_begin(L, PROF_DENSE);
+            k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t], use_tc ? w.y16[t] : nullptr); LSD_COUNT(L);
+            prof_end(L, pid);
+        }
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
         pid = prof_begin(L, PROF_EDGE_FWD);
         if (use_tc) {
