@@ -47,6 +47,7 @@ __device__ __forceinline__ double uniform53(uint64_t seed, uint64_t step)
 __global__ void k_half_a(int n, const double* __restrict__ q, const double* __restrict__ p, const double* __restrict__ mass,
                          double hdt, double* __restrict__ qhalf, const double* __restrict__ qref, double skin_half2, int* flags)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double m = mass[i];
@@ -70,6 +71,7 @@ __global__ void k_bob_a(int n, uint64_t seed, const uint64_t* __restrict__ n0p, 
                         const double* __restrict__ dF, double* __restrict__ qhalf_next, const double* __restrict__ qref,
                         double skin_half2, int* flags)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double xi[3];
@@ -118,6 +120,7 @@ k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, cons
                     const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg,
                     const double* __restrict__ dF)
 {
+    pdl_sync();
     const int j = blockIdx.y;                      // step j+1 of the window
     const uint64_t n0 = *n0p;
     const size_t base = (size_t)j * 3 * n;
@@ -156,6 +159,7 @@ __global__ void k_transport_final(int K, int nblk, uint64_t seed, const uint64_t
                                   double* S1, double* S2, double* ell, double* lnu, int* reject, const int* flags,
                                   TransportResult* result)
 {
+    pdl_sync();
     __shared__ int rej[LSD_MAX_K];
     __shared__ double beta[LSD_MAX_K];
     const int j = threadIdx.x;
@@ -189,6 +193,7 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
                          const double* __restrict__ sigma, double c1, double b, double hdt, double* __restrict__ q_base,
                          double* __restrict__ p_base, const double* __restrict__ dF, double* __restrict__ dF_out)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     if (result->flags != 0) return;                  // skin / overflow / non-finite: nothing is committed
@@ -263,7 +268,7 @@ void launch_half_a(Launcher L, int n, const double* q, const double* p, const do
                    double* qhalf, const double* qref, double skin_half2, int* flags)
 {
     const int pid = prof_begin(L, PROF_INTEG);
-    k_half_a<<<(n + 255) / 256, 256, 0, L.s>>>(n, q, p, mass, hdt, qhalf, qref, skin_half2, flags);
+    launch_pdl(L, k_half_a, dim3((n + 255) / 256), dim3(256), 0, n, q, p, mass, hdt, qhalf, qref, skin_half2, flags);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
@@ -273,15 +278,15 @@ void launch_bob_a(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint
                   double* q_new, double* p_new, const double* dF, double* qhalf_next, const double* qref, double skin_half2, int* flags)
 {
     const int pid = prof_begin(L, PROF_INTEG);
-    k_bob_a<<<(n + 127) / 128, 128, 0, L.s>>>(n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new, dF, qhalf_next, qref, skin_half2, flags);
+    launch_pdl(L, k_bob_a, dim3((n + 127) / 128), dim3(128), 0, n, seed, n0_dev, j, p_prev, Ft, qhalf, mass, sigma, c1, b, hdt, q_new, p_new, dF, qhalf_next, qref, skin_half2, flags);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
 
-__global__ void k_set_u64(uint64_t* dst, uint64_t v) { *dst = v; }
+__global__ void k_set_u64(uint64_t* dst, uint64_t v) { pdl_sync(); *dst = v; }
 void launch_set_u64(Launcher L, uint64_t* dst, uint64_t v)
 {
-    k_set_u64<<<1, 1, 0, L.s>>>(dst, v);
+    launch_pdl(L, k_set_u64, dim3(1), dim3(1), 0, dst, v);
     LSD_COUNT(L);
 }
 
@@ -296,9 +301,9 @@ void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n
                       double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
-    k_transport_partial<<<dim3(nblk, K), kTrThreads, 0, L.s>>>(n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg, dF);
+    launch_pdl(L, k_transport_partial, dim3(nblk, K), dim3(kTrThreads), 0, n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg, dF);
     LSD_COUNT(L);
-    k_transport_final<<<1, LSD_MAX_K, 0, L.s>>>(K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
+    launch_pdl(L, k_transport_final, dim3(1), dim3(LSD_MAX_K), 0, K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
@@ -309,7 +314,7 @@ void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, 
                    double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
-    k_commit<<<(n + 127) / 128, 128, 0, L.s>>>(n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
+    launch_pdl(L, k_commit, dim3((n + 127) / 128), dim3(128), 0, n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
                                                c1, b, hdt, q_base, p_base, dF, dF_out);
     LSD_COUNT(L);
     prof_end(L, pid);

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string>
 #include <vector>
 
@@ -129,6 +130,36 @@ struct Launcher {                    // stream + launch counter (+ profiler)
     int draft = 0;                   // 1: kernels of the draft potential (their MLIP launches are timed as one class)
 };
 #define LSD_COUNT(L) (++(*(L).counter))
+
+// Programmatic dependent launch (PDL): the small kernels of a window form one long dependency chain (a draft step is ~10
+// kernels of a few microseconds), so each kernel is launched with the programmatic-stream-serialization attribute and begins
+// with pdl_sync(): wait until the kernels before it have completed and flushed, then let the next kernel's CTAs be scheduled
+// (they block in their own wait until this grid has completed), which takes the launch latency off the critical path.
+// pdl_sync() must be the first statement of the kernel, before any early return (completion is transitive only if every
+// CTA waits).  A kernel without the attribute, or behind a kernel without pdl_sync(), simply keeps the full dependency.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_sync()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+inline bool lsd_pdl_enabled()
+{
+    static const bool on = [] { const char* v = getenv("LSD_PDL"); return !(v && v[0] == '0'); }();
+    return on;
+}
+template <typename... KA, typename... A>
+inline void launch_pdl(const Launcher& L, void (*kernel)(KA...), dim3 grid, dim3 block, size_t smem, A&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = L.s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = lsd_pdl_enabled() ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KA>(args)...);
+}
+#endif
 inline int prof_begin(const Launcher& L, int cls)
 {
     Prof* p = L.prof;

@@ -15,6 +15,7 @@ struct BoxC { double L[3]; int periodic; };
 // wrapped image index of every atom at the reference state: q = qw + img L, qw in [0, L)
 __global__ void k_images(int n, BoxC box, const double* __restrict__ q, int* __restrict__ img)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int im[3] = {0, 0, 0};
@@ -52,6 +53,7 @@ struct GridC { int nc[3]; };
 __global__ void k_cell_count(int n, BoxC box, GridC g, const double* __restrict__ q, const int* __restrict__ img,
                              int* __restrict__ atom_cell, int* __restrict__ cell_count)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int c = cell_of(box, g.nc, q, n, i, img[i]);
@@ -61,6 +63,7 @@ __global__ void k_cell_count(int n, BoxC box, GridC g, const double* __restrict_
 
 __global__ void k_cell_scan(int ncell, const int* __restrict__ cell_count, int* __restrict__ cell_start, int* __restrict__ cell_cursor)
 {
+    pdl_sync();
     // single block exclusive scan (ncell is a few thousand)
     __shared__ int carry;
     __shared__ int buf[1024];
@@ -88,6 +91,7 @@ __global__ void k_cell_scan(int ncell, const int* __restrict__ cell_count, int* 
 
 __global__ void k_cell_fill(int n, const int* __restrict__ atom_cell, int* __restrict__ cell_cursor, int* __restrict__ cell_atoms)
 {
+    pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     cell_atoms[atomicAdd(&cell_cursor[atom_cell[i]], 1)] = i;     // order inside a cell is fixed later by the row sort
@@ -121,6 +125,7 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
                const int* __restrict__ atom_cell, const int* __restrict__ cell_start, const int* __restrict__ cell_atoms,
                double rcs2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags)
 {
+    pdl_sync();
     __shared__ uint32_t rows[kVlWarps][kVlMaxRow];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i = blockIdx.x * kVlWarps + warp;
@@ -181,6 +186,7 @@ k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __res
           const double* __restrict__ pair_rc2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags,
           float* __restrict__ recs, float inv_rc)
 {
+    pdl_sync();
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= n * B) return;
     const int b = warp / n, i = warp % n;
@@ -280,7 +286,7 @@ void cellgrid_setup(CellGrid& g, const SysDev& sys, double rc_skin)
 
 void launch_pack_ref(Launcher L, const SysDev& sys, const double* qref, int* img)
 {
-    k_images<<<(sys.n + 255) / 256, 256, 0, L.s>>>(sys.n, make_box(sys), qref, img);
+    launch_pdl(L, k_images, dim3((sys.n + 255) / 256), dim3(256), 0, sys.n, make_box(sys), qref, img);
     LSD_COUNT(L);
 }
 
@@ -291,10 +297,10 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
     const int pid = prof_begin(L, PROF_NBR);
     GridC gc; gc.nc[0] = g.nc[0]; gc.nc[1] = g.nc[1]; gc.nc[2] = g.nc[2];
     cudaMemsetAsync(g.cell_count, 0, sizeof(int) * g.ncell, L.s);
-    k_cell_count<<<(n + 255) / 256, 256, 0, L.s>>>(n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_count); LSD_COUNT(L);
-    k_cell_scan<<<1, 1024, 0, L.s>>>(g.ncell, g.cell_count, g.cell_start, g.cell_cursor); LSD_COUNT(L);
-    k_cell_fill<<<(n + 255) / 256, 256, 0, L.s>>>(n, g.atom_cell, g.cell_cursor, g.cell_atoms); LSD_COUNT(L);
-    k_build_verlet<<<(n + kVlWarps - 1) / kVlWarps, kVlWarps * 32, 0, L.s>>>(n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_start,
+    launch_pdl(L, k_cell_count, dim3((n + 255) / 256), dim3(256), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_count); LSD_COUNT(L);
+    launch_pdl(L, k_cell_scan, dim3(1), dim3(1024), 0, g.ncell, g.cell_count, g.cell_start, g.cell_cursor); LSD_COUNT(L);
+    launch_pdl(L, k_cell_fill, dim3((n + 255) / 256), dim3(256), 0, n, g.atom_cell, g.cell_cursor, g.cell_atoms); LSD_COUNT(L);
+    launch_pdl(L, k_build_verlet, dim3((n + kVlWarps - 1) / kVlWarps), dim3(kVlWarps * 32), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_start,
                                                                              g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags);
     LSD_COUNT(L);
     prof_end(L, pid);
@@ -306,7 +312,7 @@ void launch_compact(Launcher L, const SysDev& sys, int B, const double* q, const
     const size_t warps = (size_t)sys.n * B;
     const int blocks = (int)((warps * 32 + 255) / 256);
     const int pid = prof_begin(L, PROF_NBR);
-    k_compact<<<blocks, 256, 0, L.s>>>(sys.n, B, make_box(sys), q, img, sys.species, sys.ns, vl.count, vl.keys, vl.cap, rc2_single,
+    launch_pdl(L, k_compact, dim3(blocks), dim3(256), 0, sys.n, B, make_box(sys), q, img, sys.species, sys.ns, vl.count, vl.keys, vl.cap, rc2_single,
                                        pair_rc2, cl.cap, cl.count, cl.keys, flags, rc_records > 0.f ? cl.recs : nullptr,
                                        rc_records > 0.f ? 1.f / rc_records : 0.f);
     LSD_COUNT(L);

@@ -27,6 +27,7 @@ k_prior(int n, int B, BoxC box, const double* __restrict__ q, const int* __restr
         int n_bonds, const int* __restrict__ bonds, const double* __restrict__ bond_k, const double* __restrict__ bond_r0,
         const int* __restrict__ angles, const double* __restrict__ angle_k, const double* __restrict__ angle_t0, double* __restrict__ F)
 {
+    pdl_sync();
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= n * B) return;
     const int b = warp / n, i = warp % n;
@@ -107,7 +108,7 @@ void launch_prior_forces(Launcher L, const SysDev& sys, const PotDev& pot, int B
     const size_t warps = (size_t)sys.n * B;
     const int blocks = (int)((warps * 32 + 255) / 256);
     const int pid = prof_begin(L, PROF_PRIOR);
-    k_prior<<<blocks, 256, 0, L.s>>>(sys.n, B, box, q, img, sys.species, sys.ns, pot.pair, pot.has_tether ? pot.tether : nullptr,
+    launch_pdl(L, k_prior, dim3(blocks), dim3(256), 0, sys.n, B, box, q, img, sys.species, sys.ns, pot.pair, pot.has_tether ? pot.tether : nullptr,
                                      pl ? pl->count : nullptr, pl ? pl->keys : nullptr, pl ? pl->cap : 0,
                                      pot.use_bonded && (sys.n_bonds + sys.n_angles) > 0, sys.bt_start, sys.bt_term, sys.n_bonds, sys.bonds,
                                      sys.bond_k, sys.bond_r0, sys.angles, sys.angle_k, sys.angle_t0, F);
