@@ -207,6 +207,13 @@ lsd_status upload_mlip(lsd_ctx* ctx, const lsd_mlip& m, MlipDev& d)
                 TRY(upk(Wo1, false, &d.Wo1_tc[t])); TRY(upk(Wo1, true, &d.Wo1T_tc[t]));
                 TRY(upk(Wo2, false, &d.Wo2_tc[t])); TRY(upk(Wo2, true, &d.Wo2T_tc[t]));
             }
+            const double* Wr1d = blk + (size_t)T * per_block;
+            for (int tr = 0; tr < 2; ++tr) {
+                tc_pack_rect128(Wr1d, F / 2, F, tr == 1, p1);
+                uint16_t* dev = nullptr;
+                TRY(upload(ctx, &dev, p1.data(), p1.size()));
+                (tr ? d.Wr1T_tc : d.Wr1_tc) = dev;
+            }
         }
     }
     const double* Wr1 = blk + (size_t)T * per_block;

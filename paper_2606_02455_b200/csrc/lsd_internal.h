@@ -46,6 +46,7 @@ struct MlipDev {
     std::vector<void*> Wf1_bf16, Wf2_bf16;
     // width 128: bf16 A operand images of the atom-wise layers and their transposes (mlip_atom_tc128.cu)
     std::vector<void*> Win_tc, WinT_tc, Wo1_tc, Wo1T_tc, Wo2_tc, Wo2T_tc;
+    void *Wr1_tc = nullptr, *Wr1T_tc = nullptr;   // readout W_r1 [F/2][F] and its transpose, zero padded to 128 x 128
 };
 
 struct PotDev {
@@ -230,8 +231,6 @@ struct EdgeArgs {
 void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                 const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);
 size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
-void launch_readout(Launcher L, int F, int total, float alpha, const float* x, const float* Wr1, const float* wr2, float* xbar,
-                    uint16_t* xbar16 /*optional bf16 copy*/, double* e_atom);
 
 // ---- mlip_tc.cu (bf16 tcgen05 filter path)
 bool mlip_tc_supported(const MlipDev& net);
@@ -245,5 +244,6 @@ void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& 
 
 // ---- mlip_atom_tc128.cu (width 128: atom-wise layers on the tensor cores, whole bf16 network driver)
 void tc_pack_square128(const double* W, bool transpose, std::vector<uint16_t>& out);
+void tc_pack_rect128(const double* W, int rows, int cols, bool transpose, std::vector<uint16_t>& out);
 void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                  const int* img, const CompactList& cl, double* F, double* e_atom);

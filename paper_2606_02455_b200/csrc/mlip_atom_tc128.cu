@@ -4,6 +4,7 @@
 //   forward  block t : h = W_o1 m ;  x += W_o2 ssp(h) ;  y' = W_in(t+1) x                       (k_atom_tc128<FWD3 / FWD2>)
 //   backward block t : xbar += W_in(t+1)^T ybar ;  hbar = logistic(h) . W_o2^T xbar ;  mbar = W_o1^T hbar
 //                                                                                             (k_atom_tc128<BWD3 / BWD2>)
+//   readout          : z = W_r1 x ;  e = alpha w_r2 . ssp(z) ;  xbar = alpha W_r1^T (logistic(z) . w_r2)   (k_atom_tc128<READOUT>)
 //
 // "Channels are rows", as in the edge kernels: D[128 channels x NT atoms] = W[128 x 128] B[128 x NT]; TMEM lane = channel =
 // thread, TMEM column = atom, so every global access of an epilogue is one coalesced 128-byte (fp32) or 64-byte (bf16)
@@ -35,7 +36,7 @@ constexpr int kSmem = 3 * kWBytes + kTeams * kTeamBytes;
 constexpr int kBars = 5 + kRing;                       // per team: 3 x "contraction complete", 2 x "operand written", ring slots
 static_assert(kSmem + 1024 <= 227 * 1024, "shared memory budget");
 
-enum AtomMode { FWD3 = 0, FWD2 = 1, BWD3 = 2, BWD2 = 3 };
+enum AtomMode { FWD3 = 0, FWD2 = 1, BWD3 = 2, BWD2 = 3, READOUT = 4 };
 
 struct AtomArgs {
     int total;                    // rows (states x atoms)
@@ -46,6 +47,11 @@ struct AtomArgs {
     uint16_t* y16_out;            // FWD3: y of the next block
     const uint16_t* y16;          // backward: y of the block
     uint32_t* ym16;               // backward: (y, mbar) bf16 pairs gathered by the backward edge kernel
+    uint16_t* x16_out;            // FWD2: bf16 copy of the final x (operand of the readout chain)
+    // READOUT (M6 and the seed of M9): z = W_r1 x; e = alpha w_r2 . ssp(z); xbar = alpha W_r1^T (logistic(z) . w_r2)
+    const float* wr2;             // [64]
+    float alpha;
+    double* e_atom;               // optional per-atom energies
 };
 
 constexpr float kLn2 = 0.69314718055994530942f;
@@ -57,7 +63,8 @@ __global__ void __launch_bounds__(kThreads, 1)
 k_atom_tc128(AtomArgs a)
 {
     constexpr bool FWD = MODE == FWD3 || MODE == FWD2;
-    constexpr bool HAS0 = MODE != BWD2, HAS2 = MODE != FWD2;
+    constexpr bool RO = MODE == READOUT;
+    constexpr bool HAS0 = MODE != BWD2, HAS2 = MODE != FWD2 && !RO;
     extern __shared__ __align__(128) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[kBars * kTeams];
     __shared__ uint32_t tmem_base_s;
@@ -135,6 +142,8 @@ k_atom_tc128(AtomArgs a)
         const int tt = tid & (kTT - 1), wq = warp & 3;
         uint8_t* const B2 = smem + 3 * kWBytes + team * kTeamBytes + kRing * kBBytes;
         const uint32_t tl = tD + ((uint32_t)(wq * 32) << 16);
+        const float wr2v = RO && tt < kF / 2 ? a.wr2[tt] : 0.f;
+        float* const escr = reinterpret_cast<float*>(smem + 2 * kWBytes) + team * (kF / 2) * kNT;   // READOUT: [64 channels][32 atoms], the unused third weight slot
         // cp.async piece of this thread in iteration i: atom 8 i + (lane & 7), channels 8 kc .. 8 kc + 7, kc = 4 wq + (lane >> 3):
         // a warp instruction covers 8 atoms x 64 bytes (full 32-byte sectors) and 8 distinct 16-byte bank groups
         const int pn = lane & 7, kc = 4 * wq + (lane >> 3);
@@ -180,7 +189,11 @@ k_atom_tc128(AtomArgs a)
 #pragma unroll
                     for (int c = 0; c < 16; c += 2) {
                         float o0, o1;
-                        if (FWD) {             // h kept for the backward; operand = ssp(h)
+                        if (RO) {              // operand = alpha logistic(z) w_r2 (rows >= 64 of the padded W_r1 image are zero)
+                            const float z0 = __uint_as_float(v[c]), z1 = __uint_as_float(v[c + 1]);
+                            o0 = a.alpha * logistic_f(z0) * wr2v; o1 = a.alpha * logistic_f(z1) * wr2v;
+                            if (a.e_atom && tt < kF / 2) { escr[tt * kNT + c0 + c] = wr2v * ssp_f(z0); escr[tt * kNT + c0 + c + 1] = wr2v * ssp_f(z1); }
+                        } else if (FWD) {      // h kept for the backward; operand = ssp(h)
                             const float h0 = __uint_as_float(v[c]), h1 = __uint_as_float(v[c + 1]);
                             if (c0 + c < nrow) a.h[base + (size_t)(c0 + c) * kF] = h0;
                             if (c0 + c + 1 < nrow) a.h[base + (size_t)(c0 + c + 1) * kF] = h1;
@@ -199,11 +212,21 @@ k_atom_tc128(AtomArgs a)
                 tc_fence_before();
                 fence_async_smem();
                 mbar_arrive(rdy1);
+                if (RO && a.e_atom) {          // per-atom energy: channels summed in index order by the atom's thread
+                    asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTT) : "memory");
+                    if (tt < nrow) {
+                        float e = 0.f;
+                        for (int ch = 0; ch < kF / 2; ++ch) e += escr[ch * kNT + tt];
+                        a.e_atom[row0 + tt] = (double)(a.alpha * e);
+                    }
+                }
             }
             {   // ---- epilogue of the second contraction
                 const float* src = FWD ? a.x : a.h;
+                if (!RO) {
 #pragma unroll
-                for (int c = 0; c < kNT; ++c) pre[c] = c < nrow ? src[base + (size_t)c * kF] : 0.f;
+                    for (int c = 0; c < kNT; ++c) pre[c] = c < nrow ? src[base + (size_t)c * kF] : 0.f;
+                }
                 mbar_wait(bar0 + 8, ph);
                 tc_fence_after();
 #pragma unroll
@@ -214,10 +237,20 @@ k_atom_tc128(AtomArgs a)
 #pragma unroll
                     for (int c = 0; c < 16; c += 2) {
                         float o0, o1;
-                        if (FWD) {             // x += W_o2 ssp(h)
+                        if (RO) {              // xbar, fp32 and the bf16 operand of the backward chain
+                            o0 = __uint_as_float(v[c]); o1 = __uint_as_float(v[c + 1]);
+                            const uint32_t pb = pack_bf16(o0, o1);
+                            if (c0 + c < nrow) { a.x[base + (size_t)(c0 + c) * kF] = o0; a.y16_out[base + (size_t)(c0 + c) * kF] = (uint16_t)(pb & 0xFFFFu); }
+                            if (c0 + c + 1 < nrow) { a.x[base + (size_t)(c0 + c + 1) * kF] = o1; a.y16_out[base + (size_t)(c0 + c + 1) * kF] = (uint16_t)(pb >> 16); }
+                        } else if (FWD) {      // x += W_o2 ssp(h)
                             o0 = pre[c0 + c] + __uint_as_float(v[c]); o1 = pre[c0 + c + 1] + __uint_as_float(v[c + 1]);
                             if (c0 + c < nrow) a.x[base + (size_t)(c0 + c) * kF] = o0;
                             if (c0 + c + 1 < nrow) a.x[base + (size_t)(c0 + c + 1) * kF] = o1;
+                            if (a.x16_out) {
+                                const uint32_t pb = pack_bf16(o0, o1);
+                                if (c0 + c < nrow) a.x16_out[base + (size_t)(c0 + c) * kF] = (uint16_t)(pb & 0xFFFFu);
+                                if (c0 + c + 1 < nrow) a.x16_out[base + (size_t)(c0 + c + 1) * kF] = (uint16_t)(pb >> 16);
+                            }
                         } else {               // hbar = logistic(h) . W_o2^T xbar
                             o0 = logistic_f(pre[c0 + c]) * __uint_as_float(v[c]); o1 = logistic_f(pre[c0 + c + 1]) * __uint_as_float(v[c + 1]);
                         }
@@ -317,6 +350,19 @@ void tc_pack_square128(const double* W, bool transpose, std::vector<uint16_t>& o
             out[((size_t)(m / 8) * 2048 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_bits(transpose ? W[(size_t)k * kF + m] : W[(size_t)m * kF + k]);
 }
 
+// A operand image [128][128] of a rows x cols matrix W (row-major fp64, rows, cols <= 128) or of its transpose, zero padded
+void tc_pack_rect128(const double* W, int rows, int cols, bool transpose, std::vector<uint16_t>& out)
+{
+    out.assign((size_t)kF * kF, 0);
+    for (int m = 0; m < kF; ++m)
+        for (int k = 0; k < kF; ++k) {
+            double v = 0.0;
+            if (!transpose) { if (m < rows && k < cols) v = W[(size_t)m * cols + k]; }
+            else if (k < rows && m < cols) v = W[(size_t)k * cols + m];
+            out[((size_t)(m / 8) * 2048 + (k / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2] = bf16_bits(v);
+        }
+}
+
 // Width-128 bf16 tensor-core network: edge kernels of mlip_tc128.cu + the chain kernels above.  bf16 aliases of fp32 work
 // buffers that this path does not need: m16 in w.m, ybar16 in w.ybar, xbar16 in w.mbar.
 void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
@@ -328,6 +374,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
+    uint16_t* const x16 = m16 + (size_t)w.bmax * sys.n * kF;       // upper half of w.m's buffer (m16 occupies the lower half)
     int pid = prof_begin(L, PROF_DENSE);
     k_embed_tc<<<(int)(((size_t)total * (kF / 4) + 255) / 256), 256, 0, L.s>>>(total, sys.n, sys.species, net.emb, net.ytab0, w.x, w.y16[0]); LSD_COUNT(L);
     prof_end(L, pid);
@@ -343,9 +390,14 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;
         aa.W[0] = net.Wo1_tc[t]; aa.W[1] = net.Wo2_tc[t];
         if (t + 1 < T) { aa.W[2] = net.Win_tc[t + 1]; aa.y16_out = w.y16[t + 1]; launch_atom<FWD3>(L, aa); }
-        else launch_atom<FWD2>(L, aa);
+        else { aa.x16_out = x16; launch_atom<FWD2>(L, aa); }
     }
-    launch_readout(L, kF, total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, xbar16, e_atom);
+    {   // readout chain
+        AtomArgs aa{};
+        aa.total = total; aa.in16 = x16; aa.W[0] = net.Wr1_tc; aa.W[1] = net.Wr1T_tc; aa.x = w.xbar; aa.y16_out = xbar16;
+        aa.wr2 = net.wr2; aa.alpha = net.alpha; aa.e_atom = e_atom;
+        launch_atom<READOUT>(L, aa);
+    }
     ea.m16_out = nullptr;
     for (int t = T - 1; t >= 0; --t) {
         if (t == T - 1) {

@@ -205,7 +205,7 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
 template <int F>
 __global__ void __launch_bounds__(kThreads)
 k_readout(int total, float alpha, const float* __restrict__ x, const float* __restrict__ Wr1, const float* __restrict__ wr2,
-          float* __restrict__ xbar, double* __restrict__ e_atom, uint16_t* __restrict__ xbar16 = nullptr)
+          float* __restrict__ xbar, double* __restrict__ e_atom)
 {
     constexpr int H = F / 2, LD = F + 1;
     extern __shared__ __align__(16) float smem[];
@@ -234,7 +234,6 @@ k_readout(int total, float alpha, const float* __restrict__ x, const float* __re
             float v = 0.f;
             for (int k = 0; k < H; ++k) v = fmaf(Ws[k * LD + f], ss[k], v);
             xbar[(size_t)g * F + f] = alpha * v;
-            if (xbar16) { const __nv_bfloat16 b = __float2bfloat16_rn(alpha * v); xbar16[(size_t)g * F + f] = *reinterpret_cast<const uint16_t*>(&b); }
         }
         if (lane == 0 && e_atom) e_atom[g] = (double)(alpha * e);
         __syncwarp();
@@ -423,20 +422,6 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
 }
 
 }  // namespace
-
-void launch_readout(Launcher L, int F, int total, float alpha, const float* x, const float* Wr1, const float* wr2, float* xbar,
-                    uint16_t* xbar16, double* e_atom)
-{
-    const int grid = std::max(1, std::min(num_sms(), (total + kWarps - 1) / kWarps));
-    const int pid = prof_begin(L, PROF_DENSE);
-    if (F == 128) {
-        static bool configured = false;
-        if (!configured) { set_smem(k_readout<128>, smem_readout<128>()); configured = true; }
-        k_readout<128><<<grid, kThreads, smem_readout<128>(), L.s>>>(total, alpha, x, Wr1, wr2, xbar, e_atom, xbar16);
-    }
-    LSD_COUNT(L);
-    prof_end(L, pid);
-}
 
 size_t mlip_work_bytes(const MlipDev& net, int n, int bmax)
 {
