@@ -79,3 +79,22 @@ def test_full_size_window(P, orc, name):
     assert np.array_equal(F1[0], F2[1])
     assert np.array_equal(F2[0], Fg[0])                         # and equal to what the (graph-replayed) verification produced
     ctx.close()
+
+
+@pytest.mark.parametrize("name,kw", [("cfg4", {"n_atoms": 700}), ("cfg5", {"cells": (5, 5, 4)}), ("cfg3", {"n_grid": 7})])
+def test_bf16_runs_are_reproducible_bit_for_bit(P, orc, name, kw):
+    """Two independent contexts, 40 windows each on their own streams (graph replay, tcgen05 kernels with dynamic tile
+    scheduling, asynchronous copies, mbarrier hand-offs): a race or an order-dependent sum would show up as a difference."""
+    import torch
+    w = L.make_workload(name, **kw)
+    p0 = orc.initial_momenta(w)
+    finals = []
+    for rep in range(2):
+        ctx = P.context_from_workload(w, k_max=4, precision=P.LSD_BF16_TC, p0=p0)
+        stream = torch.cuda.Stream()
+        hist = [ctx.window(4, stream) for _ in range(40)]
+        finals.append((hist, *ctx.state()))
+        ctx.close()
+    assert finals[0][0] == finals[1][0]
+    assert np.array_equal(finals[0][1], finals[1][1]) and np.array_equal(finals[0][2], finals[1][2]) and finals[0][3] == finals[1][3]
+    assert np.isfinite(finals[0][1]).all()
