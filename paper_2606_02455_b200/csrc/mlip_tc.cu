@@ -500,8 +500,10 @@ void launch_edge_tc_ch(Launcher L, const EdgeArgs& a, bool backward)
 template <int F>
 void launch_edge_tc_f(Launcher L, const EdgeArgs& a, bool backward)
 {
-    const long chunks64 = (long)((a.n + kCH - 1) / kCH) * (a.total / a.n);
-    if (chunks64 < 2L * tc_num_sms() * kTeams) launch_edge_tc_ch<F, 16>(L, a, backward);
+    const long B = a.total / a.n, teams = (long)tc_num_sms() * kTeams;
+    const long chunks64 = (long)((a.n + kCH - 1) / kCH) * B, chunks16 = (long)((a.n + 15) / 16) * B;
+    if (chunks16 < teams) launch_edge_tc_ch<F, 8>(L, a, backward);            // (a draft step of a few thousand atoms)
+    else if (chunks64 < 2 * teams) launch_edge_tc_ch<F, 16>(L, a, backward);
     else launch_edge_tc_ch<F, kCH>(L, a, backward);
 }
 
