@@ -25,7 +25,7 @@ constexpr int kF = 128;
 constexpr int kR = LSD_NRBF;
 constexpr int kTeams = 3;
 constexpr int kTT = 128;                               // edges of a tile
-constexpr int kSplit = 1;                              // threads per edge: each owns 64 of the 128 channels
+constexpr int kSplit = 1;                              // threads per edge (2: each owns 64 of the 128 channels; measured slower)
 constexpr int kTeamThreads = kTT * kSplit;
 constexpr int kThreads = kTeams * kTeamThreads + kTeams * 32;
 constexpr int kCH = 16;                                // atoms per chunk = columns of D3
@@ -54,11 +54,6 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
                    "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
                    "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
                  : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]) : "r"(taddr) : "memory");
 }
 __device__ __forceinline__ uint32_t hmul2_bf16(uint32_t a, uint32_t b)
 {
