@@ -319,12 +319,16 @@ lsd_status setup_lists(lsd_ctx* ctx)
     ctx->cap_mlip = ctx->cap_pair = 0;
     if (ctx->rc_mlip_max > 0) TRY(probe_capacity(ctx, ctx->rc_mlip_max + skin, &ctx->cap_mlip));
     if (ctx->rc_pair_max > 0) TRY(probe_capacity(ctx, ctx->rc_pair_max + skin, &ctx->cap_pair));
+    // equal cutoffs (cfg5: Morse and network both 6 A): one Verlet list serves both, build_lists builds it once
+    const bool shared = ctx->cap_mlip && ctx->cap_pair && ctx->rc_mlip_max == ctx->rc_pair_max;
     for (int s = 0; s < 2; ++s) {
         if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->slot[s].vl_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
-        if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->slot[s].vl_pair, ctx->cap_pair, ctx->rc_pair_max));
+        if (shared) ctx->slot[s].vl_pair = ctx->slot[s].vl_mlip;
+        else if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->slot[s].vl_pair, ctx->cap_pair, ctx->rc_pair_max));
     }
     if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->vl_eval_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
-    if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->vl_eval_pair, ctx->cap_pair, ctx->rc_pair_max));
+    if (shared) ctx->vl_eval_pair = ctx->vl_eval_mlip;
+    else if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->vl_eval_pair, ctx->cap_pair, ctx->rc_pair_max));
     for (int w = 0; w < 2; ++w) {
         if (ctx->pot[w].mlip.F > 0) TRY(alloc_compact(ctx, ctx->cl_mlip[w], ctx->cap_mlip, ctx->bmax[w], true));
         if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w], false));
@@ -340,7 +344,7 @@ void build_lists(lsd_ctx* ctx, Launcher L, const double* qref, int* img, VerletL
         cellgrid_setup(ctx->grid, ctx->sys, ctx->rc_mlip_max + ctx->cfg.skin);
         launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_mlip_max + ctx->cfg.skin, vm, flags);
     }
-    if (ctx->cap_pair) {
+    if (ctx->cap_pair && vp.keys != vm.keys) {                   // (shared list when the cutoffs are equal, setup_lists)
         cellgrid_setup(ctx->grid, ctx->sys, ctx->rc_pair_max + ctx->cfg.skin);
         launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_pair_max + ctx->cfg.skin, vp, flags);
     }
