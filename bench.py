@@ -319,6 +319,20 @@ def main():
                         kernel_executed_tflops=edges * 2 * (2 * R * F + 2 * F * F) / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else None,
                         stage_ms_per_step={k: v["ms"] / args.steps for k, v in prof.items() if v["launches"]})
 
+    if roofline is not None and dtype == "bf16" and tgt.width == 128:
+        # the other two kernel families of the width-128 tensor-core path, from the same profiled pass
+        T, rows = tgt.n_blocks, K * N
+        chain_bytes = rows * (2048 * T + 1024 + 1536 + 2560 * (T - 1))          # algorithmic bytes per row of the chain kernels
+        dense_ms = prof["mlip_dense"]["ms"] / args.steps
+        fwd_ms = prof["mlip_edge_fwd"]["ms"] / args.steps
+        roofline["other_kernels"] = dict(
+            atom_chain=dict(bound="hbm", achieved=chain_bytes / (dense_ms * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                            frac=chain_bytes / (dense_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], ms_per_step=dense_ms,
+                            note="k_atom_tc128<*> incl. the embedding kernel; ncu: profiles/r1_atom_tc128_cfg5.md"),
+            edge_forward=dict(bound="tensor", achieved=edges * T * (2 * R * F + 2 * F * F) / (fwd_ms * 1e-3) / 1e12, peak=peaks["bf16"], unit="TFLOP/s",
+                              frac=edges * T * (2 * R * F + 2 * F * F) / (fwd_ms * 1e-3) / 1e12 / peaks["bf16"], ms_per_step=fwd_ms,
+                              note="k_edge_er128_fwd, executed filter flops (the strict count shares the value with the backward); MUFU-bound, DESIGN.md 4.1"))
+
     if rank == 0:
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms / args.steps,
                     higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
