@@ -17,7 +17,7 @@
 
 namespace {
 
-constexpr int kWarps = 8;
+constexpr int kWarps = 12;
 constexpr int kThreads = kWarps * 32;
 constexpr float kLn2 = 0.69314718055994530942f;
 
