@@ -17,8 +17,8 @@
 
 namespace {
 
-constexpr int kWarps = 12;
-constexpr int kThreads = kWarps * 32;
+constexpr int kMaxWarps = 16;          // warps per CTA: 16 for batches that fill the device, 8 for small ones (run_fp32)
+constexpr int kMaxThreads = kMaxWarps * 32;
 constexpr float kLn2 = 0.69314718055994530942f;
 
 __device__ __forceinline__ float ssp(float x) { return fmaxf(x, 0.f) + log1pf(expf(-fabsf(x))) - kLn2; }          // M3
@@ -81,7 +81,7 @@ __device__ __forceinline__ void warp_gemm8(const float* __restrict__ As, int lda
 
 __device__ __forceinline__ void load_weights(float* dst, const float* __restrict__ src, int count)
 {
-    for (int i = threadIdx.x * 4; i < count; i += kThreads * 4) *reinterpret_cast<float4*>(dst + i) = *reinterpret_cast<const float4*>(src + i);
+    for (int i = threadIdx.x * 4; i < count; i += blockDim.x * 4) *reinterpret_cast<float4*>(dst + i) = *reinterpret_cast<const float4*>(src + i);
 }
 
 // ------------------------------------------------------------------------------------------------ embedding (M4)
@@ -108,7 +108,7 @@ enum DenseMode { DENSE_IN = 0, DENSE_OUT = 1, BWD_OUT = 2, BWD_IN = 3 };
 // BWD_OUT  : out = (logistic(aux) . (in * W0)) * W1          (mbar = W_o1^T (logistic(h) . W_o2^T xbar))
 // BWD_IN   : io += in * W0                                   (xbar += W_in^T ybar)
 template <int F, int MODE>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kMaxThreads, 1)
 k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, const float* __restrict__ W1,
         float* __restrict__ aux, float* __restrict__ out, uint16_t* __restrict__ out16,
         const uint16_t* __restrict__ pair16 = nullptr, uint32_t* __restrict__ outpair = nullptr)
@@ -124,7 +124,7 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ntiles = (total + 7) / 8;
-    for (int tile = blockIdx.x * kWarps + warp; tile < ntiles; tile += gridDim.x * kWarps) {
+    for (int tile = blockIdx.x * (blockDim.x >> 5) + warp; tile < ntiles; tile += gridDim.x * (blockDim.x >> 5)) {
         const int g0 = tile * 8;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -203,7 +203,7 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
 // ------------------------------------------------------------------------------------------------ readout (M6) + xbar seed
 // z = W_r1 x ; e = alpha w_r2 . ssp(z) ; xbar = alpha W_r1^T (logistic(z) . w_r2).  One warp per atom.
 template <int F>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kMaxThreads)
 k_readout(int total, float alpha, const float* __restrict__ x, const float* __restrict__ Wr1, const float* __restrict__ wr2,
           float* __restrict__ xbar, double* __restrict__ e_atom)
 {
@@ -212,12 +212,12 @@ k_readout(int total, float alpha, const float* __restrict__ x, const float* __re
     float* Ws = smem;                       // [H][F+1]
     float* w2 = Ws + H * LD;                // [H]
     float* xs = w2 + H + (threadIdx.x >> 5) * (F + H);   // per warp: x[F], s[H]
-    for (int i = threadIdx.x; i < H * F; i += kThreads) Ws[(i / F) * LD + (i % F)] = Wr1[i];
-    for (int i = threadIdx.x; i < H; i += kThreads) w2[i] = wr2[i];
+    for (int i = threadIdx.x; i < H * F; i += blockDim.x) Ws[(i / F) * LD + (i % F)] = Wr1[i];
+    for (int i = threadIdx.x; i < H; i += blockDim.x) w2[i] = wr2[i];
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* ss = xs + F;
-    for (int g = blockIdx.x * kWarps + warp; g < total; g += gridDim.x * kWarps) {
+    for (int g = blockIdx.x * (blockDim.x >> 5) + warp; g < total; g += gridDim.x * (blockDim.x >> 5)) {
         for (int f = lane; f < F; f += 32) xs[f] = x[(size_t)g * F + f];
         __syncwarp();
         float e = 0.f;
@@ -243,7 +243,7 @@ k_readout(int total, float alpha, const float* __restrict__ x, const float* __re
 // ------------------------------------------------------------------------------------------------ continuous-filter convolution
 
 template <int F, bool BWD>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kMaxThreads, 1)
 k_edge(EdgeArgs a)
 {
     constexpr int CPT = F / 32, LDA = F + 4, LDG = LSD_NRBF + 4, SPW = BWD ? 4 : 8;
@@ -257,7 +257,7 @@ k_edge(EdgeArgs a)
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = a.n;
-    for (int g = blockIdx.x * kWarps + warp; g < a.total; g += gridDim.x * kWarps) {
+    for (int g = blockIdx.x * (blockDim.x >> 5) + warp; g < a.total; g += gridDim.x * (blockDim.x >> 5)) {
         const int b = g / n, i = g % n;
         const int cnt = a.count[g];
         float part[CPT], ya[CPT], mba[CPT];
@@ -352,9 +352,9 @@ k_edge(EdgeArgs a)
     }
 }
 
-template <int F> size_t smem_dense(bool two) { return sizeof(float) * ((two ? 2 : 1) * F * F + kWarps * 8 * (F + 4)); }
-template <int F> size_t smem_edge() { return sizeof(float) * (LSD_NRBF * F + F * F + kWarps * (8 * (LSD_NRBF + 4) + 8 * (F + 4))); }
-template <int F> size_t smem_readout() { return sizeof(float) * ((F / 2) * (F + 1) + F / 2 + kWarps * (F + F / 2)); }
+template <int F> size_t smem_dense(bool two, int kWarps) { return sizeof(float) * ((two ? 2 : 1) * F * F + kWarps * 8 * (F + 4)); }
+template <int F> size_t smem_edge(int kWarps) { return sizeof(float) * (LSD_NRBF * F + F * F + kWarps * (8 * (LSD_NRBF + 4) + 8 * (F + 4))); }
+template <int F> size_t smem_readout(int kWarps) { return sizeof(float) * ((F / 2) * (F + 1) + F / 2 + kWarps * (F + F / 2)); }
 
 int g_num_sms = 0;
 int num_sms() { if (!g_num_sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev); if (g_num_sms <= 0) g_num_sms = 148; } return g_num_sms; }
@@ -368,13 +368,17 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     const int total = B * sys.n;
     static bool configured = false;
     if (!configured) {
-        set_smem(k_dense<F, DENSE_IN>, smem_dense<F>(false)); set_smem(k_dense<F, BWD_IN>, smem_dense<F>(false));
-        set_smem(k_dense<F, DENSE_OUT>, smem_dense<F>(true)); set_smem(k_dense<F, BWD_OUT>, smem_dense<F>(true));
-        set_smem(k_edge<F, false>, smem_edge<F>()); set_smem(k_edge<F, true>, smem_edge<F>());
-        set_smem(k_readout<F>, smem_readout<F>());
+        set_smem(k_dense<F, DENSE_IN>, smem_dense<F>(false, kMaxWarps)); set_smem(k_dense<F, BWD_IN>, smem_dense<F>(false, kMaxWarps));
+        set_smem(k_dense<F, DENSE_OUT>, smem_dense<F>(true, kMaxWarps)); set_smem(k_dense<F, BWD_OUT>, smem_dense<F>(true, kMaxWarps));
+        set_smem(k_edge<F, false>, smem_edge<F>(kMaxWarps)); set_smem(k_edge<F, true>, smem_edge<F>(kMaxWarps));
+        set_smem(k_readout<F>, smem_readout<F>(kMaxWarps));
         configured = true;
     }
     const int sms = num_sms();
+    // 16 warps per CTA once every SM has at least 16 atoms to work on (occupancy: +8 % at cfg4 fp32); 8 for small batches,
+    // whose kernels are latency-bound (a bigger CTA only adds to the weight-load and barrier time).  Same arithmetic either way.
+    const int kWarps = total >= sms * kMaxWarps ? kMaxWarps : 8;
+    const int kThreads = kWarps * 32;
     const int grid_tiles = std::max(1, std::min(sms, (total + kWarps * 8 - 1) / (kWarps * 8)));
     const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
     k_embed_y<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, net.ytab0, w.x, w.y[0], use_tc ? w.y16[0] : nullptr); LSD_COUNT(L);
@@ -385,7 +389,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         int pid = -1;
         if (t > 0) {
             pid = prof_begin(L, PROF_DENSE);
-            k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t], use_tc ? w.y16[t] : nullptr); LSD_COUNT(L);
+            k_dense<F, DENSE_IN><<<grid_tiles, kThreads, smem_dense<F>(false, kWarps), L.s>>>(total, w.x, net.WinT[t], nullptr, nullptr, w.y[t], use_tc ? w.y16[t] : nullptr); LSD_COUNT(L);
             prof_end(L, pid);
         }
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = w.m; ea.mbar = nullptr; ea.ybar = nullptr; ea.Fout = nullptr;
@@ -394,19 +398,19 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t];
             if (F == 128) launch_edge_tc128(L, ea, false); else launch_edge_tc(L, ea, F, false);
         }
-        else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
+        else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
         pid = prof_begin(L, PROF_DENSE);
-        k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x, nullptr); LSD_COUNT(L);
+        k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x, nullptr); LSD_COUNT(L);
         prof_end(L, pid);
     }
     int pidr = prof_begin(L, PROF_DENSE);
-    k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
+    k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(kWarps), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
     prof_end(L, pidr);
     for (int t = net.T - 1; t >= 0; --t) {
         int pid = prof_begin(L, PROF_DENSE);
         const bool pairs = use_tc && F == 128;
-        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc && !pairs ? w.mbar16 : nullptr,
+        k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc && !pairs ? w.mbar16 : nullptr,
                                                                                  pairs ? w.y16[t] : nullptr, pairs ? w.ym16 : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
@@ -415,9 +419,9 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; ea.ym16 = w.ym16;
             if (F == 128) launch_edge_tc128(L, ea, true); else launch_edge_tc(L, ea, F, true);
         }
-        else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(), L.s>>>(ea); LSD_COUNT(L); }
+        else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
-        if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar, nullptr); LSD_COUNT(L); prof_end(L, pid); }
+        if (t > 0) { pid = prof_begin(L, PROF_DENSE); k_dense<F, BWD_IN><<<grid_tiles, kThreads, smem_dense<F>(false, kWarps), L.s>>>(total, w.ybar, net.Win[t], nullptr, nullptr, w.xbar, nullptr); LSD_COUNT(L); prof_end(L, pid); }
     }
 }
 

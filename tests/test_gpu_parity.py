@@ -234,7 +234,7 @@ def test_stagewise_transport_parity(P, orc, name, kw, K):
     ctx.close()
 
 
-@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", {}), ("cfg5", {"cells": (4, 4, 4)})])
+@pytest.mark.parametrize("name,kw", [("cfg1", {}), ("cfg2", {}), ("cfg3", {"n_grid": 7}), ("cfg5", {"cells": (4, 4, 4)})])
 def test_draft_equals_target_accepts_everything(P, orc, name, kw):
     """draft = target: F~ and F are bit-identical (batch-invariant kernels), S2 == 0, acceptance exactly 1."""
     w = L.with_target_as_draft(L.make_workload(name, **kw))
