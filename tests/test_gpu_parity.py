@@ -367,3 +367,29 @@ def test_adaptive_lookahead_does_not_change_the_trajectory(P, orc):
         ctx.close()
     for q, p in finals[1:]:
         assert np.array_equal(q, finals[0][0]) and np.array_equal(p, finals[0][1])
+
+
+@pytest.mark.parametrize("K", [1, 64])
+def test_window_length_extremes_match_the_oracle(P, orc, K):
+    """K = 1 (every window is one step) and K = LSD_MAX_K = 64 (the largest batch the transport kernels accept), cfg1 in fp64
+    on both sides: decisions, first-reject index and committed state follow the oracle."""
+    w = L.make_workload("cfg1")
+    if K == 64:
+        w = dataclasses.replace(w, dt_fs=0.5)                   # 64 steps of 2 fs would leave the Verlet skin (the box allows 0.6 A at most)
+    p0 = orc.initial_momenta(w)
+    ctx = P.context_from_workload(w, p0=p0, k_max=K)
+    q, p, n = w.q0, p0, 0
+    for _ in range(6 if K == 64 else 40):
+        r = orc.lsd_window(w, q, p, n, K=K)
+        l, nc = ctx.window(K)
+        assert not (np.abs(r["ell"] - r["lnu"]) < BAND).any()
+        assert (l, nc) == (r["first_reject"], r["n_commit"])
+        assert np.array_equal(ctx.debug("reject", K), r["reject"])
+        q, p, n = r["q"], r["p"], n + nc
+        qg, pg, step = ctx.state()
+        assert step == n and np.abs(qg.T - q).max() <= POS_TOL
+    with pytest.raises(P.LsdError):
+        P.lsd_draft_rollout(ctx.h, K + 1)                       # beyond k_max
+    ctx.close()
+    with pytest.raises(P.LsdError):
+        P.context_from_workload(w, p0=p0, k_max=65)            # beyond LSD_MAX_K
