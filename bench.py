@@ -193,11 +193,20 @@ def main():
     work_bytes = 0 if tgt is None else 4 * N * K * tgt.width * (5 + 2 * tgt.n_blocks)
     need_flush = work_bytes < 2 * 126e6
 
+    skin = [float(w.skin)]
+
     def one_window():
         if args.overlap:
             P.lsd_run(ctx.h, K, K, overlap=True, stream=stream)
             return None
-        return ctx.window(K, stream)
+        try:
+            return ctx.window(K, stream)
+        except P.LsdError as e:                          # as lsd_run does: a skin violation is answered by larger lists, never ignored
+            if e.status != -7:
+                raise
+            skin[0] *= 2.0
+            P.lsd_set_skin(ctx.h, skin[0])
+            return ctx.window(K, stream)
 
     def timed_pass():
         """K timed windows, CUDA events on the launching stream around every window (L2 flush outside the events)."""
@@ -338,7 +347,7 @@ def main():
                     higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
                     config=dict(workload=args.workload, n_atoms=N, window_K=K, atoms_per_window=K * N, integrator="ABOBA (Eq. 2)",
                                 l2="flushed between timed steps (256 MiB write)" if need_flush else "working set larger than L2",
-                                overlap=bool(args.overlap), error_correction=bool(args.ec), replicas=world, peaks=peaks["source"]),
+                                overlap=bool(args.overlap), error_correction=bool(args.ec), skin_A=skin[0], replicas=world, peaks=peaks["source"]),
                     committed_md_steps_per_s=committed_all / (ms * 1e-3), committed_per_window=committed_all / (args.steps * world),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, speedup=speedup)
         if not args.no_cpu_baseline and world == 1:
