@@ -47,6 +47,7 @@ struct AtomArgs {
     uint16_t* y16_out;            // FWD3: y of the next block
     const uint16_t* y16;          // backward: y of the block
     uint32_t* ym16;               // backward: (y, mbar) bf16 pairs gathered by the backward edge kernel
+    int ym_pairs;                 // 0: word f = (y_f | mbar_f << 16); 1: per channel pair the words (y_f | y_f+1 << 16), (mbar_f | mbar_f+1 << 16)
     uint16_t* x16_out;            // FWD2: bf16 copy of the final x (operand of the readout chain)
     // READOUT (M6 and the seed of M9): z = W_r1 x; e = alpha w_r2 . ssp(z); xbar = alpha W_r1^T (logistic(z) . w_r2)
     const float* wr2;             // [64]
@@ -284,7 +285,11 @@ k_atom_tc128(AtomArgs a)
                             const __nv_bfloat16 b = __float2bfloat16_rn(__uint_as_float(v[c]));
                             const uint16_t bits = *reinterpret_cast<const uint16_t*>(&b);
                             if (FWD) a.y16_out[base + (size_t)(c0 + c) * kF] = bits;
-                            else a.ym16[base + (size_t)(c0 + c) * kF] = (uint32_t)yv[c0 + c] | ((uint32_t)bits << 16);
+                            else if (!a.ym_pairs) a.ym16[base + (size_t)(c0 + c) * kF] = (uint32_t)yv[c0 + c] | ((uint32_t)bits << 16);
+                            else {
+                                uint16_t* row = reinterpret_cast<uint16_t*>(a.ym16 + (size_t)(row0 + c0 + c) * kF) + 4 * (tt >> 1) + (tt & 1);
+                                row[0] = yv[c0 + c]; row[2] = bits;
+                            }
                         }
                     }
                 }
@@ -371,6 +376,8 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     (void)q; (void)img;
     const int total = B * sys.n, T = net.T;
     static const bool use_er = [] { const char* v = getenv("LSD_EDGE_ER"); return v == nullptr || v[0] != '0'; }();
+    // LSD_EDGE_ROWS=1: second-generation edge kernels (mlip_edge_rows.cu) instead of mlip_er128.cu forward / mlip_tc128.cu backward
+    static const bool use_rows = [] { const char* v = getenv("LSD_EDGE_ROWS"); return v != nullptr && v[0] == '1'; }();
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
@@ -384,7 +391,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
+        if (use_rows) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
         prof_end(L, pid);
         AtomArgs aa{};
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;
@@ -403,18 +410,18 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
         if (t == T - 1) {
             AtomArgs aa{};
             aa.total = total; aa.in16 = xbar16; aa.h = w.h[t]; aa.y16 = w.y16[t]; aa.ym16 = w.ym16;
-            aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t];
+            aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t]; aa.ym_pairs = use_rows;
             launch_atom<BWD2>(L, aa);
         }
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.ym16 = w.ym16;
         ea.ybar16_out = t > 0 ? ybar16 : nullptr; ea.ybar = nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        launch_edge_tc128(L, ea, true);
+        if (use_rows) launch_edge_rows(L, ea, true); else launch_edge_tc128(L, ea, true);
         prof_end(L, pid);
         if (t > 0) {
             AtomArgs aa{};
             aa.total = total; aa.in16 = ybar16; aa.x = w.xbar; aa.h = w.h[t - 1]; aa.y16 = w.y16[t - 1]; aa.ym16 = w.ym16;
-            aa.W[0] = net.WinT_tc[t]; aa.W[1] = net.Wo2T_tc[t - 1]; aa.W[2] = net.Wo1T_tc[t - 1];
+            aa.W[0] = net.WinT_tc[t]; aa.W[1] = net.Wo2T_tc[t - 1]; aa.W[2] = net.Wo1T_tc[t - 1]; aa.ym_pairs = use_rows;
             launch_atom<BWD3>(L, aa);
         }
     }
