@@ -376,8 +376,10 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     (void)q; (void)img;
     const int total = B * sys.n, T = net.T;
     static const bool use_er = [] { const char* v = getenv("LSD_EDGE_ER"); return v == nullptr || v[0] != '0'; }();
-    // LSD_EDGE_ROWS=1: second-generation edge kernels (mlip_edge_rows.cu) instead of mlip_er128.cu forward / mlip_tc128.cu backward
-    static const bool use_rows = [] { const char* v = getenv("LSD_EDGE_ROWS"); return v != nullptr && v[0] == '1'; }();
+    // LSD_EDGE_ROWS: which passes use the second-generation edge kernel (mlip_edge_rows.cu) instead of mlip_er128.cu (forward) /
+    // mlip_tc128.cu (backward): 0 none, 1 forward, 2 backward (default: measured faster there), 3 both
+    static const int rows_sel = [] { const char* v = getenv("LSD_EDGE_ROWS"); return v ? atoi(v) : 2; }();   // bit 0: forward, bit 1: backward
+    const bool use_rows_f = (rows_sel & 1) != 0, use_rows = (rows_sel & 2) != 0;
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
@@ -391,7 +393,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_rows) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
+        if (use_rows_f) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
         prof_end(L, pid);
         AtomArgs aa{};
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;

@@ -278,7 +278,11 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                     for (int i = 0; i < 8; ++i) {
                         const int el = 4 * i + (lane >> 3), s = s0 + (lane & 7);
                         const int jr = __shfl_sync(0xffffffffu, jrow, el);
-                        cp_async16(sStage + (uint32_t)(s * kSlab + (32 * wq + el) * 16), rows + (size_t)jr * ROWB + s * 16, 16);
+#ifndef LSD_EXP_NOGATHER
+                        // .ca: through L1, where the 8 lanes of a row coalesce to 4 sectors (with .cg every 16-byte piece fetched its
+                        // own 32-byte sector from L2: twice the traffic, 1.4 x the kernel time)
+                        cp_async16_ca(sStage + (uint32_t)(s * kSlab + (32 * wq + el) * 16), rows + (size_t)jr * ROWB + s * 16);
+#endif
                     }
                 }
             };
