@@ -238,6 +238,7 @@ bool mlip_tc_supported(const MlipDev& net);
 void launch_edge_tc(Launcher L, const EdgeArgs& a, int F, bool backward);
 void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_tc128.cu: width 128
 void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
+void launch_edge_pipe(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_pipe.cu: width 128, warp-specialised pipeline of the same tile algebra
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_rows.cu: width 128, edges-as-rows, activations in TMEM
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);

@@ -146,8 +146,8 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         uint8_t* const ST = own + L::OwnBytes;
         uint8_t* const gatom = ST + kSTBytes;                      // group -> atom of the chunk
         int* const pref = reinterpret_cast<int*>(gatom + kMaxGroups);             // first group of every atom (17 entries)
-        float* const gpart = reinterpret_cast<float*>(gatom + kMaxGroups + 128);  // bwd: [8 groups][4] force sums of the tile's groups
-        float* const gx = gpart + 32;                              // bwd, SPLIT = 2: [128][2] partial channel sums of the second part
+        float* const gx = reinterpret_cast<float*>(gatom + kMaxGroups + 128) + 32;
+        float* const gpart = gx;                                   // bwd: [2 tile parities][SPLIT parts][8 groups][4] force sums of the tile's groups
         float4* const accs = reinterpret_cast<float4*>(gx + 256);  // bwd: [4][128] float4: sums of channel e for atoms 4 j .. 4 j + 3
         float* const fsum = reinterpret_cast<float*>(tbuf + L::TeamBytes - 256);      // bwd: [16 atoms][4] force sums of the chunk
         float* const recS = reinterpret_cast<float*>(tbuf + L::TeamBytes - 256 - 5 * kTT * 4);   // [5 fields][128]: fc, fc', ux, uy, uz of the tile's slots
@@ -166,14 +166,15 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         const uint32_t id64 = make_idesc(128, 64, 0), id128 = make_idesc(128, 128, 0), id3 = make_idesc(128, kCH, 0) | (1u << 15);
         const uint64_t dW1 = make_desc(sW1, 128, 512), dW2 = make_desc(sW2, 128, 2048);
         const uint64_t dP = make_desc(sStage, 128, BWD ? 2 * kSlab : kSlab), dS = make_desc(sST, 128, 2048);
-        enum { R_G1H0 = 0, R_G1H1 = 1, R_G2O0 = 2, R_G2O1 = 3, R_G3 = 4, R_F1 = 5, R_F2 = 6, R_F3NEW = 7, R_F3ACC = 8 };
+        enum { R_G1H0 = 0, R_G1H1 = 1, R_G2O0 = 2, R_G2O1 = 3, R_G3 = 4, R_F1 = 5, R_F2 = 6, R_F3NEW = 7, R_F3ACC = 8, R_SYNC = 9 };
+        int tile_in_chunk = 0;
         auto publish = [&](int kind) {
             tc_fence_before();
             warp_arrive(rdy, lane);
             if (issuer) {
                 mbar_wait(rdy, phr); phr ^= 1u;
                 tc_fence_after();
-                if (elect_one()) {
+                if (kind != R_SYNC && elect_one()) {
                     if (kind == R_G1H0 || kind == R_G1H1) {        // x, x' of channel half h
                         const int h = kind - R_G1H0;
 #pragma unroll
@@ -205,6 +206,24 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                             umma(tb + kColD3f, dP + (uint64_t)(k16 * 16), dS + (uint64_t)(k16 * 16), id3, (kind == R_F3ACC || k16 > 0) ? 1u : 0u);
                     }
                     umma_commit(done);
+                }
+                __syncwarp();
+                if (BWD && (kind == R_G3 || kind == R_SYNC) && lane < kCH) {
+                    // every warp has published the force sums of its groups: atom `lane` adds those of its groups inside this tile,
+                    // in list order, part 0 then part 1
+                    const int t = tile_in_chunk;
+                    const int lo = max(pref[lane], t * kGPT), hi = min(pref[lane + 1], t * kGPT + kGPT);
+                    if (lo < hi) {
+                        float fax = fsum[4 * lane], fay = fsum[4 * lane + 1], faz = fsum[4 * lane + 2];
+                        for (int g = lo; g < hi; ++g) {
+#pragma unroll
+                            for (int pp = 0; pp < SPLIT; ++pp) {
+                                const float* gp = gpart + ((((t & 1) * SPLIT + pp) * kGPT) + (g - t * kGPT)) * 4;
+                                fax += gp[0]; fay += gp[1]; faz += gp[2];
+                            }
+                        }
+                        fsum[4 * lane] = fax; fsum[4 * lane + 1] = fay; fsum[4 * lane + 2] = faz;
+                    }
                 }
                 __syncwarp();
             }
@@ -414,29 +433,25 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                     // ---- force term of the edge, summed over the 16 edges of its group
                     float Al, Ah, Bl, Bh;
                     un2(A2, Al, Ah); un2(B2, Bl, Bh);
-                    float As = Al + Ah, Bs = Bl + Bh;
-                    if (SPLIT == 2) {
-                        if (part == 1) { gx[2 * e] = As; gx[2 * e + 1] = Bs; }
-                        team_bar<TT>(team);
-                        if (part == 0) { As += gx[2 * e]; Bs += gx[2 * e + 1]; }
-                    }
-                    float fc = 0.f;
-                    if (part == 0) {
-                        fc = recS[e];
+                    const float As = Al + Ah, Bs = Bl + Bh;        // this part's channels
+                    const float fc = recS[e];
+                    {
                         const float g = fc * As + recS[kTT + e] * Bs;
                         float fx = g * recS[2 * kTT + e], fy = g * recS[3 * kTT + e], fz = g * recS[4 * kTT + e];
 #pragma unroll
                         for (int o = 8; o > 0; o >>= 1) {
                             fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
                         }
-                        if (my_s == 0) { gpart[4 * my_g] = fx; gpart[4 * my_g + 1] = fy; gpart[4 * my_g + 2] = fz; }
-                        if (need_sum && at >= 0) {                 // S^T[e][at] = fc
+                        if (my_s == 0) { float* gp = gpart + ((((t & 1) * SPLIT + part) * kGPT) + my_g) * 4; gp[0] = fx; gp[1] = fy; gp[2] = fz; }
+                        if (need_sum && part == 0 && at >= 0) {    // S^T[e][at] = fc
                             const __nv_bfloat16 fb = __float2bfloat16_rn(fc);
                             *reinterpret_cast<uint16_t*>(ST + (at >> 3) * 2048 + (e >> 3) * 128 + (at & 7) * 16 + (e & 7) * 2) = *reinterpret_cast<const uint16_t*>(&fb);
                         }
                     }
                     TRACE(11);
                     if (t + 1 < ntiles) load_record(t + 1);        // lands under the last round trip
+                    tile_in_chunk = t;
+                    if (!need_sum) publish(R_SYNC);                // the issuing warp adds the groups' force sums
                     if (need_sum) {
                         fence_async_smem();
                         publish(R_G3);                             // -> D3 = P^T S
@@ -454,15 +469,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         }
                         if (part == 0 && at >= 0) *reinterpret_cast<uint16_t*>(ST + (at >> 3) * 2048 + (e >> 3) * 128 + (at & 7) * 16 + (e & 7) * 2) = 0;
                     }
-                    team_bar<TT>(team);                            // gpart of every group is written
                     TRACE(13);
-                    if (tt < kCH) {
-                        const int ng = min(kGPT, G - t * kGPT);
-                        float fax = fsum[4 * tt], fay = fsum[4 * tt + 1], faz = fsum[4 * tt + 2];
-                        for (int g = 0; g < ng; ++g)
-                            if (gatom[t * kGPT + g] == tt) { fax += gpart[4 * g]; fay += gpart[4 * g + 1]; faz += gpart[4 * g + 2]; }
-                        fsum[4 * tt] = fax; fsum[4 * tt + 1] = fay; fsum[4 * tt + 2] = faz;
-                    }
                 } else {
                     constexpr int NC = kF / SPLIT;                 // channels this thread handles: [NC part, NC part + NC)
                     // ---- activation (M3): D -> A2
@@ -546,10 +553,10 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         }
                     }
                 }
-                if (BWD && tt < natoms2) {
-                    const int i = ci2 * kCH + tt;
+                if (BWD && issuer && lane < natoms2) {           // the issuing warp holds the force sums (lane = atom)
+                    const int i = ci2 * kCH + lane;
                     double* Fb = a.Fout + (size_t)b2 * 3 * n;
-                    Fb[i] += (double)fsum[4 * tt]; Fb[n + i] += (double)fsum[4 * tt + 1]; Fb[2 * n + i] += (double)fsum[4 * tt + 2];
+                    Fb[i] += (double)fsum[4 * lane]; Fb[n + i] += (double)fsum[4 * lane + 1]; Fb[2 * n + i] += (double)fsum[4 * lane + 2];
                 }
             }
 #undef G
