@@ -22,7 +22,8 @@ _STATUS = {0: "LSD_OK", -1: "LSD_ERR_INVALID_ARG", -2: "LSD_ERR_CUDA", -3: "LSD_
 EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_rollout", "lsd_verify_window", "lsd_transport_accept",
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
-                    "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k"]
+                    "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k",
+                    "lsd_get_window_obabo", "lsd_get_edge_launch_info"]
 
 
 class LsdError(RuntimeError):
@@ -273,6 +274,15 @@ def lsd_get_profile(h) -> dict:
     ms, cnt = (C.c_double * 8)(), (C.c_int64 * 8)()
     _check(h, load_library().lsd_get_profile(h, ms, cnt))
     return {name: dict(ms=ms[i], launches=cnt[i]) for i, name in enumerate(PROFILE_CLASSES)}
+
+
+EDGE_KERNELS = {0: None, 1: "k_edge_tc", 2: "k_edge_tc128", 3: "k_edge_er128_fwd", 4: "k_edge_rows", 5: "k_edge_pipe"}
+
+
+def lsd_get_edge_launch_info(backward: bool) -> dict:
+    out = (C.c_int32 * 5)()
+    _check(None, load_library().lsd_get_edge_launch_info(C.c_int32(int(bool(backward))), out))
+    return dict(kernel=EDGE_KERNELS.get(out[0], out[0]), atoms_per_chunk=out[1], threads=out[2], grid=out[3], width=out[4])
 
 
 def lsd_tc_enabled(h) -> bool:

@@ -420,6 +420,14 @@ const char* lsd_last_error(const lsd_ctx* ctx) { return ctx ? ctx->err.c_str() :
 
 int64_t lsd_launch_count(const lsd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+lsd_status lsd_get_edge_launch_info(int32_t pass, int32_t* out)
+{
+    if (!out || pass < 0 || pass > 1) return LSD_ERR_INVALID_ARG;
+    const EdgeLaunchInfo& e = g_edge_last[pass];
+    out[0] = e.kernel; out[1] = e.atoms_per_chunk; out[2] = e.threads; out[3] = e.grid; out[4] = e.width;
+    return LSD_OK;
+}
+
 int32_t lsd_tc_enabled(const lsd_ctx* ctx)
 {
     return ctx && ctx->cfg.precision == LSD_BF16_TC && ctx->pot[LSD_TARGET].mlip.F > 0 && mlip_tc_supported(ctx->pot[LSD_TARGET].mlip) ? 1 : 0;

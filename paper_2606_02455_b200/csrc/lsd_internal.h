@@ -228,6 +228,26 @@ struct EdgeArgs {
     unsigned long long* trace = nullptr;   // debug (LSD_EDGE_TRACE=1): clock64 stamps of one chunk of block 0
 };
 
+// per-device one-time state (function attributes, SM count): indexed by the current device, not per process
+inline int lsd_current_device() { int d = 0; cudaGetDevice(&d); return (d < 0 || d >= 64) ? 0 : d; }
+inline int lsd_sm_count()
+{
+    static int sms[64] = {};
+    int& v = sms[lsd_current_device()];
+    if (!v) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev); if (v <= 0) v = 148; }
+    return v;
+}
+
+// which tcgen05 edge kernel the last forward / backward launch of this process used (parity tests assert that the timed
+// instantiation is the one they compared with the oracle): kernel 1 = k_edge_tc (mlip_tc.cu), 2 = k_edge_tc128, 3 = k_edge_er128_fwd,
+// 4 = k_edge_rows, 5 = k_edge_pipe
+struct EdgeLaunchInfo { int kernel = 0, atoms_per_chunk = 0, threads = 0, grid = 0, width = 0; };
+inline EdgeLaunchInfo g_edge_last[2];
+inline void note_edge_launch(bool backward, int kernel, int atoms_per_chunk, int threads, int grid, int width)
+{
+    g_edge_last[backward ? 1 : 0] = EdgeLaunchInfo{kernel, atoms_per_chunk, threads, grid, width};
+}
+
 // ---- mlip_simt.cu
 void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                 const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);

@@ -318,16 +318,12 @@ __global__ void k_embed_tc(int total, int n, const int* __restrict__ species, co
     *reinterpret_cast<uint2*>(y16 + (size_t)g * kF + f) = make_uint2(pack_bf16(y.x, y.y), pack_bf16(y.z, y.w));
 }
 
-int sm_count()
-{
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-    return sms;
-}
+int sm_count() { return lsd_sm_count(); }
 
 template <int MODE> void launch_atom(Launcher L, const AtomArgs& a)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
     if (!configured) { cudaFuncSetAttribute(k_atom_tc128<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem); configured = true; }
     const int ntiles = (a.total + kNT - 1) / kNT;
     const int grid = std::max(1, std::min(sm_count(), (ntiles + kTeams - 1) / kTeams));

@@ -583,6 +583,7 @@ template <bool BWD> void launch_pipe(Launcher L, const EdgeArgs& a)
     }
 #endif
     k_edge_pipe<BWD><<<grid, kThreads, Lay<BWD>::Smem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(BWD, 5, kCH, kThreads, grid, kF);
     LSD_COUNT(L);
 }
 

@@ -608,6 +608,7 @@ template <bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
         return;
     }
     k_edge_rows<BWD, SPLIT><<<grid, threads, Lay<BWD>::Smem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(BWD, 4, kCH, threads, grid, kF);
     LSD_COUNT(L);
 }
 

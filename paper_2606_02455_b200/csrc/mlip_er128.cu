@@ -318,18 +318,14 @@ k_edge_er128_fwd(EdgeArgs a, int chunks_per_state, int nchunks)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
-int sm_count()
-{
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-    return sms;
-}
+int sm_count() { return lsd_sm_count(); }
 
 }  // namespace
 
 void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
     if (!configured) {
         cudaFuncSetAttribute(k_edge_er128_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
         configured = true;
@@ -338,5 +334,6 @@ void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward)
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(sm_count(), (nchunks + kTeams - 1) / kTeams));
     if (!backward) k_edge_er128_fwd<<<grid, kThreads, kSmem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(backward, 3, kCH, kThreads, grid, kF);
     LSD_COUNT(L);
 }

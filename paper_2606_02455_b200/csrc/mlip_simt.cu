@@ -366,7 +366,8 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
               const CompactList& cl, double* Fout, double* e_atom, bool use_tc)
 {
     const int total = B * sys.n;
-    static bool configured = false;
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
     if (!configured) {
         set_smem(k_dense<F, DENSE_IN>, smem_dense<F>(false, kMaxWarps)); set_smem(k_dense<F, BWD_IN>, smem_dense<F>(false, kMaxWarps));
         set_smem(k_dense<F, DENSE_OUT>, smem_dense<F>(true, kMaxWarps)); set_smem(k_dense<F, BWD_OUT>, smem_dense<F>(true, kMaxWarps));

@@ -461,12 +461,7 @@ k_edge_tc(EdgeArgs a, int chunks_per_state, int nchunks)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
-int tc_num_sms()
-{
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-    return sms;
-}
+int tc_num_sms() { return lsd_sm_count(); }
 
 uint16_t bf16_rne(double x)
 {
@@ -480,7 +475,8 @@ uint16_t bf16_rne(double x)
 template <int F, int CH>
 void launch_edge_tc_ch(Launcher L, const EdgeArgs& a, bool backward)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
     if (!configured) {
         cudaFuncSetAttribute(k_edge_tc<F, false, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, false>::Smem);
         cudaFuncSetAttribute(k_edge_tc<F, true, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<F, true>::Smem);
@@ -491,6 +487,7 @@ void launch_edge_tc_ch(Launcher L, const EdgeArgs& a, bool backward)
     const int grid = std::max(1, std::min(tc_num_sms(), nchunks));
     if (backward) k_edge_tc<F, true, CH><<<grid, kThreadsTC, TcCfg<F, true>::Smem, L.s>>>(a, cps, nchunks);
     else k_edge_tc<F, false, CH><<<grid, kThreadsTC, TcCfg<F, false>::Smem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(backward, 1, CH, kThreadsTC, grid, F);
     LSD_COUNT(L);
 }
 

@@ -3,7 +3,7 @@
 //
 // Same tile algebra as mlip_tc.cu ("channels are rows": TMEM lane = channel = thread, TMEM column = edge; the per-atom
 // sums over edges are serial sums inside one thread, in the order of the atom's sorted neighbour row), re-organised
-// around the instruction-issue limit the round-1 profile showed (profiles/r1_edge_tc_cfg5.md):
+// around the instruction-issue limit the round-1 profile showed (profiles/r1_edge_tc128_fwd_cfg5.md):
 //   * one persistent CTA per SM, 4 teams of 128 threads; every team owns 128 TMEM columns (D1, D2) and its own operand
 //     buffers; the only team-wide barrier per tile publishes the asynchronous copies.  "Operand ready" is an mbarrier
 //     every thread arrives on without waiting; only the issuing thread waits for it.
@@ -416,18 +416,14 @@ k_edge_tc128(EdgeArgs a, int chunks_per_state, int nchunks)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
-int sm_count()
-{
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-    return sms;
-}
+int sm_count() { return lsd_sm_count(); }
 
 }  // namespace
 
 template <int CH> static void launch_edge_tc128_ch(Launcher L, const EdgeArgs& a, bool backward)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
     if (!configured) {
         cudaFuncSetAttribute(k_edge_tc128<false, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<false>::Smem);
         cudaFuncSetAttribute(k_edge_tc128<true, CH>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<true>::Smem);
@@ -438,6 +434,7 @@ template <int CH> static void launch_edge_tc128_ch(Launcher L, const EdgeArgs& a
     const int grid = std::max(1, std::min(sm_count(), nchunks));
     if (backward) k_edge_tc128<true, CH><<<grid, kThreads, Cfg<true>::Smem, L.s>>>(a, cps, nchunks);
     else k_edge_tc128<false, CH><<<grid, kThreads, Cfg<false>::Smem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(backward, 2, CH, kThreads, grid, kF);
     LSD_COUNT(L);
 }
 

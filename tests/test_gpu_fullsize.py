@@ -1,7 +1,9 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (cfg5: 65,536 atoms, K = 8, bf16 tcgen05
-path; cfg4: 4,096 atoms, K = 32).  The oracle cannot evaluate the 6-block network on 65,536 atoms in test time, so the forces
-are checked through properties that hold at any size and everything the oracle CAN do at full size is compared directly:
-neighbour lists (cell-list oracle, bit-exact), the transport map / decisions on the GPU's own forces, the noise."""
+path; cfg4: 4,096 atoms, K = 32; cfg3: 1,536 atoms, K = 16).  Forces are compared with the oracle element-wise per atom
+(test_full_size_forces_match_oracle: cfg3 / cfg4 two window states each in fp32 and bf16, cfg5 one state -- one oracle evaluation
+of the 6-block network on 65,536 atoms takes about a minute on the box's host cores); everything else the oracle can do at
+full size is compared directly too: neighbour lists (cell-list oracle, bit-exact), the transport map / decisions on the GPU's
+own forces, the noise; plus properties that hold at any size (sum of forces, batch invariance, reproducibility)."""
 import math
 
 import numpy as np
@@ -98,3 +100,52 @@ def test_bf16_runs_are_reproducible_bit_for_bit(P, orc, name, kw):
     assert finals[0][0] == finals[1][0]
     assert np.array_equal(finals[0][1], finals[1][1]) and np.array_equal(finals[0][2], finals[1][2]) and finals[0][3] == finals[1][3]
     assert np.isfinite(finals[0][1]).all()
+
+
+def _t2_error(Fg, Fo):
+    """T2: max_i |dF_i| / max(|F_i|, F_rms); Fg, Fo: [N, 3]."""
+    nrm = np.linalg.norm(Fo, axis=1)
+    rms = math.sqrt((Fo**2).sum(1).mean())
+    return float((np.linalg.norm(Fg - Fo, axis=1) / np.maximum(nrm, rms)).max())
+
+
+# (workload, precision, window states compared with the oracle).  One oracle evaluation costs about 0.2 s (cfg3), 1 s (cfg4) and one
+# minute (cfg5: 65,536 atoms, 6 blocks of width 128 in fp64 on the box's host cores), so cfg5 compares one state.
+FULL_FORCE_CASES = [("cfg3", "fp32", (0, 15)), ("cfg3", "bf16", (0, 15)), ("cfg4", "fp32", (0, 31)), ("cfg4", "bf16", (0, 31)),
+                    ("cfg5", "bf16", (7,))]
+
+
+@pytest.mark.parametrize("name,prec,states", FULL_FORCE_CASES)
+def test_full_size_forces_match_oracle(P, orc, name, prec, states):
+    """north_star: in-tolerance forces against the oracle on the configurations at the sizes BASELINE.json states, in the launch
+    configuration bench.py times: the batched target forces of a whole window of K states (second window of the context, i.e.
+    the graph-replayed launch sequence), element-wise per atom against the fp64 oracle at the same q_half (T2: 1e-5 fp32,
+    2e-2 bf16).  The test also asserts which edge kernel instantiation produced them."""
+    import torch
+    w = L.make_workload(name)
+    K, N = w.K, w.n_atoms
+    bf16 = prec == "bf16"
+    p0 = orc.initial_momenta(w)
+    ctx = P.context_from_workload(w, precision=P.LSD_BF16_TC if bf16 else P.LSD_FP32, p0=p0)
+    assert bool(P.lsd_tc_enabled(ctx.h)) == bf16
+    stream = torch.cuda.Stream()
+    ctx.window(K, stream)                                       # first window: plain launches, captures the graphs
+    P.lsd_draft_rollout(ctx.h, K, stream); P.lsd_verify_window(ctx.h, K, stream)
+    l, nc = P.lsd_transport_accept(ctx.h, K, stream)
+    qh, Fg = ctx.debug("q_half", K), ctx.debug("F_target", K)
+    if bf16:
+        fwd, bwd = P.lsd_get_edge_launch_info(False), P.lsd_get_edge_launch_info(True)
+        assert fwd["width"] == w.target.mlip.width and bwd["width"] == w.target.mlip.width     # the target's launches were the last ones
+        if w.target.mlip.width == 128:
+            # the kernels the cfg5 / cfg4 bench lines time (DESIGN.md section 4.1), with a grid that fills the device
+            assert bwd["kernel"] in ("k_edge_rows", "k_edge_pipe", "k_edge_tc128") and fwd["kernel"] in ("k_edge_er128_fwd", "k_edge_rows", "k_edge_pipe")
+            assert bwd["grid"] >= 148 and fwd["grid"] >= 148
+            if bwd["kernel"] == "k_edge_tc128":
+                assert bwd["atoms_per_chunk"] == 64                # not the small-batch instantiation
+    tol = 2e-2 if bf16 else 1e-5
+    for j in states:
+        Eo, Fo = orc.energy_forces(w, w.target, np.ascontiguousarray(qh[j].T))
+        err = _t2_error(Fg[j].T, Fo)
+        assert err <= tol, (name, prec, j, err)
+    P.lsd_rollback(ctx.h, l)
+    ctx.close()
