@@ -327,7 +327,7 @@ static double bonded_forces(const orc_system *sys, const double *q, double *F)
         double nu = sqrt(norm2(u)), nv = sqrt(norm2(v));
         double ct = (u[0] * v[0] + u[1] * v[1] + u[2] * v[2]) / (nu * nv);
         if (ct > 1.0) ct = 1.0; if (ct < -1.0) ct = -1.0;
-        double th = acos(ct), st = sqrt(1.0 - ct * ct), dth = th - sys->angle_t0[a];
+        double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12), dth = th - sys->angle_t0[a];   /* collinear arms: bounded, not 0/0 (R19) */
         E += 0.5 * sys->angle_k[a] * dth * dth;
         double dU = sys->angle_k[a] * dth;                         /* dU/dtheta */
         for (int c = 0; c < 3; ++c) {

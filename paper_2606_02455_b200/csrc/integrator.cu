@@ -160,7 +160,7 @@ __global__ void k_transport_final(int K, int nblk, uint64_t seed, const uint64_t
                                   TransportResult* result)
 {
     pdl_sync();
-    __shared__ int rej[LSD_MAX_K];
+    __shared__ int rej[LSD_MAX_K], bad[LSD_MAX_K];
     __shared__ double beta[LSD_MAX_K];
     const int j = threadIdx.x;
     const uint64_t n0 = *n0p;
@@ -172,6 +172,8 @@ __global__ void k_transport_final(int K, int nblk, uint64_t seed, const uint64_t
         const int r = (c > 0.0 && lu > fmin(0.0, l)) ? 1 : 0;
         S1[j] = a; S2[j] = c; ell[j] = l; lnu[j] = lu; reject[j] = r;
         rej[j] = r;
+        bad[j] = !(isfinite(a) && isfinite(c));      // a non-finite draft or target force (r -> 0 pair, overflow): comparisons with NaN are false,
+                                                     // i.e. the step would read as accepted
         beta[j] = erf(sqrt(c) / sqrt(8.0));           // Eq. 9
     }
     __syncthreads();
@@ -180,8 +182,9 @@ __global__ void k_transport_final(int K, int nblk, uint64_t seed, const uint64_t
         for (int t = 0; t < K; ++t) if (rej[t]) { l = t + 1; break; }   // l = min{j : x_j != y_j}
         const int nc = l ? l : K;                                      // R3 (no bonus step), R4 (x_l counts)
         double bs = 0.0;
-        for (int t = 0; t < nc; ++t) bs += beta[t];
-        result->first_reject = l; result->n_commit = nc; result->flags = *flags; result->beta_sum = bs;
+        int fl = *flags;
+        for (int t = 0; t < nc; ++t) { bs += beta[t]; if (bad[t]) fl |= LSD_FLAG_NONFINITE; }   // k_commit then commits nothing
+        result->first_reject = l; result->n_commit = nc; result->flags = fl; result->beta_sum = bs;
     }
 }
 

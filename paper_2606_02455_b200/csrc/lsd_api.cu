@@ -40,6 +40,9 @@ struct lsd_ctx {
     SysDev sys;
     PotDev pot[2];
     std::vector<void*> allocs;
+    std::vector<void*> list_allocs;                          // neighbour-list rows: freed and re-made by setup_lists (lsd_set_skin)
+    bool alloc_lists = false;                                // dalloc files under list_allocs
+    double cap_growth = 1.0;                                 // extra head room of the rows after an overflow (x 1.5 per retry)
     double c1 = 0, b = 0, hdt = 0, kT = 0;
     double *q = nullptr, *p = nullptr;
     int64_t step = 0;
@@ -93,7 +96,7 @@ template <typename T> lsd_status dalloc(lsd_ctx* ctx, T** p, size_t count)
 {
     void* v = nullptr;
     CK(cudaMalloc(&v, std::max<size_t>(count, 1) * sizeof(T)));
-    ctx->allocs.push_back(v);
+    (ctx->alloc_lists ? ctx->list_allocs : ctx->allocs).push_back(v);
     *p = (T*)v;
     return LSD_OK;
 }
@@ -302,13 +305,23 @@ lsd_status probe_capacity(lsd_ctx* ctx, double rc_skin, int* cap_out)
     cudaFree(count); cudaFree(keys); cudaFree(img); cudaFree(flags);
     if (hf & LSD_FLAG_OVERFLOW) return fail(ctx, LSD_ERR_NBR_OVERFLOW, "neighbour row exceeds 512 entries (cutoff + skin too large for this density)");
     int mx = 0; for (int v : h) mx = std::max(mx, v);
-    int cap = (int)(mx * 1.25) + 8;
+    int cap = (int)(mx * 1.25 * ctx->cap_growth) + 8;
     cap = (cap + 15) / 16 * 16;
     *cap_out = std::min(cap, 512);
     return LSD_OK;
 }
 
+lsd_status setup_lists_impl(lsd_ctx* ctx);
 lsd_status setup_lists(lsd_ctx* ctx)
+{
+    for (void* p : ctx->list_allocs) cudaFree(p);            // the superseded rows (the caller has synchronised the device)
+    ctx->list_allocs.clear();
+    ctx->alloc_lists = true;
+    const lsd_status s = setup_lists_impl(ctx);
+    ctx->alloc_lists = false;
+    return s;
+}
+lsd_status setup_lists_impl(lsd_ctx* ctx)
 {
     const double skin = ctx->cfg.skin;
     ctx->rc_mlip_max = std::max((double)ctx->pot[0].mlip.rc, (double)ctx->pot[1].mlip.rc);
@@ -375,7 +388,7 @@ void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, co
 
 lsd_status flags_to_status(lsd_ctx* ctx, int flags)
 {
-    if (flags & LSD_FLAG_NONFINITE) return fail(ctx, LSD_ERR_NONFINITE, "non-finite positions in the window");
+    if (flags & LSD_FLAG_NONFINITE) return fail(ctx, LSD_ERR_NONFINITE, "non-finite positions or forces in the window");
     if (flags & LSD_FLAG_OVERFLOW) return fail(ctx, LSD_ERR_NBR_OVERFLOW, "neighbour row capacity exceeded (call lsd_set_skin to re-size the lists)");
     if (flags & LSD_FLAG_SKIN) return fail(ctx, LSD_ERR_SKIN_VIOLATED, "an atom moved more than skin/2 from the list's reference state");
     return LSD_OK;
@@ -439,6 +452,7 @@ void lsd_destroy(lsd_ctx* ctx)
     cudaDeviceSynchronize();
     drop_graphs(ctx);
     for (void* p : ctx->allocs) cudaFree(p);
+    for (void* p : ctx->list_allocs) cudaFree(p);
     cudaFree(ctx->grid.cell_count); cudaFree(ctx->grid.cell_start); cudaFree(ctx->grid.cell_cursor);
     cudaFree(ctx->grid.cell_atoms); cudaFree(ctx->grid.atom_cell);
     for (int s = 0; s < 2; ++s) if (ctx->slot[s].ev_drafted) cudaEventDestroy(ctx->slot[s].ev_drafted);
@@ -561,7 +575,7 @@ lsd_status lsd_set_skin(lsd_ctx* ctx, double skin)
     ctx->cfg.skin = skin;
     drop_graphs(ctx);                                        // captured pointers and the skin value change
     ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
-    return setup_lists(ctx);      // old rows stay allocated until lsd_destroy
+    return setup_lists(ctx);      // frees the superseded rows
 }
 
 lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
@@ -693,6 +707,8 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
     auto rate = [&](int i) { return a_t[i] > 0 ? a_nc[i] / a_t[i] : -1.0; };
     std::chrono::steady_clock::time_point t_win = std::chrono::steady_clock::now();
     int64_t remaining = n_steps;
+    constexpr int kMaxListRetries = 6;                        // per call: a window that still fails returns its error
+    int list_retries = 0;
     while (remaining > 0) {
         if (ctx->pending == 0) TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining), stream));
         const int k = ctx->slot[ctx->verify_idx].K;
@@ -701,8 +717,11 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
             TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining - k), ctx->side));   // speculative, second stream
         int32_t l = 0, nc = 0;
         lsd_status ts = lsd_transport_accept(ctx, k, stream, &l, &nc);
-        if (ts == LSD_ERR_SKIN_VIOLATED || ts == LSD_ERR_NBR_OVERFLOW) {   // answered by a rebuild with a larger skin, never by an incomplete list
+        if ((ts == LSD_ERR_SKIN_VIOLATED || ts == LSD_ERR_NBR_OVERFLOW) && list_retries < kMaxListRetries) {
+            // answered by a rebuild, never by an incomplete list: twice the skin, or rows with 1.5 x the head room
+            ++list_retries;
             CK(cudaStreamSynchronize(ctx->side));
+            if (ts == LSD_ERR_NBR_OVERFLOW) ctx->cap_growth *= 1.5;
             TRY(lsd_set_skin(ctx, ts == LSD_ERR_SKIN_VIOLATED ? 2.0 * ctx->cfg.skin : ctx->cfg.skin));
             continue;
         }
@@ -754,6 +773,7 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
     cudaStream_t st = (cudaStream_t)stream;
     const size_t n3 = (size_t)3 * ctx->sys.n;
     WindowSlot& w = ctx->slot[ctx->verify_idx];
+    int list_retries = 0;
     int64_t remaining = n_steps;
     while (remaining > 0) {
         const int K = (int)std::min<int64_t>(ctx->cfg.k_max, remaining);
@@ -766,8 +786,10 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
         int flags = 0;
         CK(cudaMemcpyAsync(&flags, w.flags, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        if (flags & (LSD_FLAG_SKIN | LSD_FLAG_OVERFLOW)) {            // as in lsd_run: answered by a rebuild with a larger skin; the base state is untouched
+        if ((flags & (LSD_FLAG_SKIN | LSD_FLAG_OVERFLOW)) && list_retries < 6) {   // as in lsd_run: answered by a rebuild; the base state is untouched
             if (flags & LSD_FLAG_NONFINITE) return flags_to_status(ctx, flags);
+            ++list_retries;
+            if (flags & LSD_FLAG_OVERFLOW) ctx->cap_growth *= 1.5;
             TRY(lsd_set_skin(ctx, (flags & LSD_FLAG_SKIN) ? 2.0 * ctx->cfg.skin : ctx->cfg.skin));
             continue;
         }

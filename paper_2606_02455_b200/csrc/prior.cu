@@ -72,7 +72,7 @@ k_prior(int n, int B, BoxC box, const double* __restrict__ q, const int* __restr
                 const double nu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]), nv = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
                 double ct = (u[0] * v[0] + u[1] * v[1] + u[2] * v[2]) / (nu * nv);
                 ct = fmin(1.0, fmax(-1.0, ct));
-                const double th = acos(ct), st = sqrt(1.0 - ct * ct);
+                const double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);   // collinear arms: bounded instead of 0/0 (R19)
                 const double dU = angle_k[a] * (th - angle_t0[a]);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {

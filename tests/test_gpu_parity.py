@@ -393,3 +393,21 @@ def test_window_length_extremes_match_the_oracle(P, orc, K):
     ctx.close()
     with pytest.raises(P.LsdError):
         P.context_from_workload(w, p0=p0, k_max=65)            # beyond LSD_MAX_K
+
+
+def test_nonfinite_forces_are_reported_and_nothing_is_committed(P, orc):
+    """Two atoms on top of each other: the pair prior returns inf - inf = NaN for both the draft and the target.  Comparisons
+    with NaN are false, so without a check every step of the window would read as accepted and the NaN draft state would be
+    committed as target-exact.  The transport kernel raises the non-finite flag instead: LSD_ERR_NONFINITE, base state untouched."""
+    w = L.make_workload("cfg1")
+    ctx = P.context_from_workload(w, precision=P.LSD_FP32, p0=np.zeros_like(w.q0))
+    q, p, step = ctx.state()
+    q_bad = q.copy()
+    q_bad[:, 1] = q_bad[:, 0]
+    P.lsd_set_state(ctx.h, q_bad, np.zeros_like(q_bad), 0)
+    with pytest.raises(P.LsdError) as ei:
+        ctx.window(w.K)
+    assert ei.value.status == -8
+    q2, p2, step2 = ctx.state()
+    assert step2 == 0 and np.array_equal(q2, q_bad) and np.array_equal(p2, np.zeros_like(q_bad))
+    ctx.close()

@@ -179,3 +179,24 @@ def test_cell_list_equals_brute_force_and_is_symmetric(orc, name, kw, rc):
     want = set(np.nonzero((r < rc) & (np.arange(w.n_atoms) != i))[0].tolist())
     assert want == set(a[1][a[0][i]:a[0][i + 1]].tolist())
     assert (np.diff(a[1][a[0][i]:a[0][i + 1]]) > 0).all()           # sorted by j
+
+
+def test_angle_term_near_and_at_collinear_arms(orc):
+    """The angle force has the form 0/0 for collinear arms (theta = pi: numerator v - cos(theta) u and sin(theta) both vanish).
+    Reading R19: sin(theta) is bounded below by 1e-12, so the force stays finite there; next to the singular
+    point the analytic force still equals the finite-difference gradient."""
+    th0 = np.radians(110.0)
+    for eps in (1e-3, 1e-5):
+        q = np.array([[1.3, 0.0, 0.0], [0.0, 0.0, 0.0], [-1.1 * np.cos(eps), 1.1 * np.sin(eps), 0.0]])
+        w = custom(q, angles=[[0, 1, 2]], angle_k=2.0, angle_t0=th0)
+        E, F = orc.energy_forces(w, w.target, w.q0)
+        assert E == pytest.approx(0.5 * 2.0 * (np.pi - eps - th0) ** 2, rel=1e-9)
+        fd = fd_forces(lambda x: orc.energy_forces(w, w.target, x, want_forces=False)[0], q, h=1e-7, idx=[(0, 1), (2, 1), (1, 1)])
+        for (i, c), v in fd.items():
+            assert F[i, c] == pytest.approx(v, rel=1e-4, abs=1e-6)
+        # |F_a| = dU/dtheta / |arm|, perpendicular to the arm
+        # (sin(theta) = sqrt(1 - cos^2) loses digits next to pi: relative error ~ 1e-16 / eps^2)
+        assert np.linalg.norm(F[0]) == pytest.approx(2.0 * (np.pi - eps - th0) / 1.3, rel=1e-5)
+    w = custom([[1.3, 0.0, 0.0], [0.0, 0.0, 0.0], [-1.1, 0.0, 0.0]], angles=[[0, 1, 2]], angle_k=2.0, angle_t0=th0)
+    E, F = orc.energy_forces(w, w.target, w.q0)
+    assert np.isfinite(F).all() and E == pytest.approx(0.5 * 2.0 * (np.pi - th0) ** 2, rel=1e-12)
