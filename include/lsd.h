@@ -232,6 +232,10 @@ lsd_status lsd_get_edge_count(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t
 lsd_status lsd_profile(lsd_ctx* ctx, int32_t enable);
 lsd_status lsd_get_profile(lsd_ctx* ctx, double* ms, int64_t* count);
 
+/* Measured plain-FMA peak of the current device in TFLOP/s, kind 0 = fp32, 1 = fp64 (16 independent FMA chains per thread on a
+ * grid of resident warps, CUDA events on `stream`, best of three): the roofline denominators of the fp32 MLIP path and of the
+ * fp64 path ("measured fp32-FMA peak", "measured fp64 peak").  Synchronises.  Errors: INVALID_ARG, CUDA. */
+lsd_status lsd_measure_fma_peak(int32_t kind, void* stream, double* tflops);
 /* Number of kernels this library has launched on behalf of ctx (bench.py's gpu_launches). */
 int64_t     lsd_launch_count(const lsd_ctx* ctx);
 const char* lsd_version(void);

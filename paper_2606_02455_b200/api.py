@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_roll
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
                     "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k",
-                    "lsd_get_window_obabo", "lsd_get_edge_launch_info"]
+                    "lsd_get_window_obabo", "lsd_get_edge_launch_info", "lsd_measure_fma_peak"]
 
 
 class LsdError(RuntimeError):
@@ -283,6 +283,13 @@ def lsd_get_edge_launch_info(backward: bool) -> dict:
     out = (C.c_int32 * 5)()
     _check(None, load_library().lsd_get_edge_launch_info(C.c_int32(int(bool(backward))), out))
     return dict(kernel=EDGE_KERNELS.get(out[0], out[0]), atoms_per_chunk=out[1], threads=out[2], grid=out[3], width=out[4])
+
+
+def lsd_measure_fma_peak(kind: int, stream=None) -> float:
+    """Measured FMA peak of the current device in TFLOP/s (kind 0 = fp32, 1 = fp64)."""
+    out = C.c_double()
+    _check(None, load_library().lsd_measure_fma_peak(C.c_int32(kind), _stream(stream), C.byref(out)))
+    return float(out.value)
 
 
 def lsd_tc_enabled(h) -> bool:
