@@ -211,6 +211,14 @@ def transport_step(w, Ft, F, xi, u, p_prev, q_half, par=None):
     return dict(reject=int(rej), S1=S1.value, S2=S2.value, ell=ell.value, q=qo, p=po)
 
 
+def force_slack(Ft, F, eps_F):
+    """App. H: F + clip(-eps_F; Ft - F; eps_F), arrays [N,3]."""
+    a, b = np.ascontiguousarray(Ft, np.float64), np.ascontiguousarray(F, np.float64)
+    out = np.empty_like(b)
+    lib().orc_force_slack(C.c_int32(len(b)), _dp(a), _dp(b), C.c_double(eps_F), _dp(out))
+    return out
+
+
 def lsd_window(w, q, p, n0, K=None, draft=None, target=None, par=None, debug=True, dF=None):
     """One synchronous window (Alg. 1).  Returns dict with new base state, committed trajectory, debug rows.
     dF ([N,3]) switches speculative error correction on (Alg. 3): the cache used by this window; "dF" in the result is the

@@ -585,6 +585,20 @@ int32_t orc_transport_step(const orc_system *sys, const orc_params *par, const d
     return 1;
 }
 
+/* Force slack (App. H): F_(eps) = F + clip(-eps_F; F~ - F; eps_F), component by component: the target force is
+ * pushed towards the draft force inside an L-infinity ball of radius eps_F.  The verification then runs orc_transport_step with
+ * F_(eps) in the place of F (breaks exactness, :781; eps_F = 0 leaves F unchanged).  Ft: the force the draft was drawn around
+ * (F~, or F~ + dF with error correction).  Not on the hot path by default (optional). */
+void orc_force_slack(int32_t n, const double *Ft, const double *F, double eps_F, double *F_out)
+{
+    for (int i = 0; i < 3 * n; ++i) {
+        double x = Ft[i] - F[i];
+        if (x > eps_F) x = eps_F;
+        if (x < -eps_F) x = -eps_F;
+        F_out[i] = F[i] + x;
+    }
+}
+
 /* ------------------------------------------------------------------------------------------
  * O-3: one synchronous window (Alg. 1, L = K; R2, R3, R4).
  * In : base state (q, p) at committed step index n0.
