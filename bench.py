@@ -432,6 +432,62 @@ def acceptance_variant(env, name, precision, target_beta=0.1, windows=6):
     return res
 
 
+def sweep_workload(L, cells, tau_fs, eps):
+    """fcc Cu of cells^3 unit cells at the paper's Fig. 4 conditions (T = 1500 K, dt = 1 fs, friction time scale tau = 1 / gamma,
+    PAPER.md:208-212) with the cfg5 potentials; draft = target with the network's energy scale x (1 + eps) (force error eps F_NN:
+    the same per-atom error scale at every N, which is what Eq. 11 assumes)."""
+    import dataclasses
+    w = L.make_workload("cfg5", cells=(cells, cells, cells))
+    m = dataclasses.replace(w.target.mlip, alpha=w.target.mlip.alpha * (1.0 + eps))
+    return dataclasses.replace(w, draft=dataclasses.replace(w.target, mlip=m), temperature_K=1500.0, dt_fs=1.0, friction_per_fs=1.0 / tau_fs)
+
+
+def run_sweep(args):
+    """the FORM of Fig. 4 (PAPER.md:185 Eq. 11, :208-212): mean rejection rate R(K)/K over a segment of `--sweep-steps`
+    committed steps against N and tau, compared with erf(sqrt(N tau / (N0 tau0)) erfinv(beta0)) where beta0 is the measured rate at
+    (N0 = 500, tau0 = 1 ps) -- the paper's fit of epsilon at that point -- with and without speculative error correction.
+    N starts at 256: the library keeps a single minimum image, i.e. box >= 2 (r_c + skin) = 13 A (R10)."""
+    import torch
+    from scipy.special import erf, erfinv
+    import lsd_inputs as L
+    import paper_2606_02455_b200 as P
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    P.load_library()
+    stream = torch.cuda.Stream()
+    K, nsteps, beta0_target = 8, args.sweep_steps, 0.3
+    # one probe window at (N0, tau0) fixes eps: delta is linear in eps (Eq. 8), beta = erf(|delta| / sqrt 8) (Eq. 9)
+    eps = 1e-2
+    ctx = P.context_from_workload(sweep_workload(L, 5, 1000.0, eps), k_max=K, precision=P.LSD_BF16_TC)
+    ctx.window(K, stream)
+    eps *= float(erfinv(beta0_target)) * np.sqrt(8.0) / float(np.mean(np.sqrt(ctx.debug("S2", K))))
+    ctx.close()
+    rows = []
+    for tau in (1000.0, 100.0):
+        for cells in (4, 5, 6, 7, 8, 10):
+            w = sweep_workload(L, cells, tau, eps)
+            row = dict(N=w.n_atoms, tau_fs=tau)
+            for key, ec in (("no_ec", False), ("ec", True)):
+                ctx = P.context_from_workload(w, k_max=K, precision=P.LSD_BF16_TC)
+                if ec:
+                    P.lsd_set_error_correction(ctx.h, True)
+                P.lsd_run(ctx.h, 5 * K, K, overlap=False, stream=stream)            # equilibrate the EC cache / warm
+                s0 = P.lsd_get_stats(ctx.h)
+                t0 = time.perf_counter()
+                P.lsd_run(ctx.h, nsteps, K, overlap=False, stream=stream)
+                dt = time.perf_counter() - t0
+                s1 = P.lsd_get_stats(ctx.h)
+                nc = s1["committed_steps"] - s0["committed_steps"]
+                row[key] = dict(rejected=int(s1["rejections"] - s0["rejections"]), steps=int(nc), rate=(s1["rejections"] - s0["rejections"]) / nc,
+                                eq9_mean_beta=(s1["beta_sum"] - s0["beta_sum"]) / nc, committed_md_steps_per_s=nc / dt)
+                ctx.close()
+            rows.append(row)
+    b0 = next(r for r in rows if r["N"] == 500 and r["tau_fs"] == 1000.0)["no_ec"]["rate"]
+    for r in rows:
+        r["eq11_prediction"] = float(erf(np.sqrt(r["N"] * r["tau_fs"] / (500 * 1000.0)) * erfinv(b0)))
+    print(json.dumps(dict(sweep="Fig. 4 form (Eq. 11)", T_K=1500.0, dt_fs=1.0, K=K, segment_steps=nsteps, eps=eps, fit_point=dict(N=500, tau_fs=1000.0, beta=b0),
+                          draft="target with network energy scale x (1 + eps)", rows=rows)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -444,9 +500,13 @@ def main():
     ap.add_argument("--no-side", action="store_true", help="skip all_workloads and the acceptance variant (kernel tuning runs)")
     ap.add_argument("--ec", type=int, default=0, help="1: speculative error correction (Alg. 3) on")
     ap.add_argument("--overlap", type=int, default=0, help="1: time lsd_run with the speculative second-stream rollout instead of explicit calls")
+    ap.add_argument("--sweep", action="store_true", help="rejection rate against N and tau (form of Fig. 4 / Eq. 11) instead of the bench line")
+    ap.add_argument("--sweep-steps", type=int, default=1000)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     args.warmup = max(args.warmup, 3)
 
     import torch

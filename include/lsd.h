@@ -188,6 +188,12 @@ lsd_status lsd_set_error_correction(lsd_ctx* ctx, int32_t enable);
 lsd_status lsd_get_ec_cache(lsd_ctx* ctx, double* dF, int32_t where);
 lsd_status lsd_set_ec_cache(lsd_ctx* ctx, const double* dF, int32_t where);
 
+/* Force slack (App. H), OFF by default: with eps_F > 0 the verification replaces the target
+ * force F by F_(eps) = F + clip(-eps_F; F~ - F; eps_F) component by component (F~: the force the draft was drawn around), in the
+ * transport map and in the override.  This BREAKS target exactness (:781; the paper recommends against it, :787); eps_F = 0 restores
+ * the exact method.  Units eV/A.  Synchronises; captured launch sequences are dropped.  Errors: INVALID_ARG (eps_F < 0 or NaN). */
+lsd_status lsd_set_force_slack(lsd_ctx* ctx, double eps_F);
+
 /* Debug rows of that window (parity tests).  `what`: */
 #define LSD_DBG_QHALF    0   /* double [K][3][n]   positions after the first A half-step                */
 #define LSD_DBG_FDRAFT   1   /* double [K][3][n]   F~_j                                                */

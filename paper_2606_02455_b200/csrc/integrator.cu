@@ -118,7 +118,7 @@ constexpr int kTrThreads = 256;
 __global__ void __launch_bounds__(kTrThreads)
 k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, const double* __restrict__ Ft, const double* __restrict__ Fg,
                     const double* __restrict__ sigma, double b, double* __restrict__ partial, double* __restrict__ xi_dbg,
-                    const double* __restrict__ dF)
+                    const double* __restrict__ dF, double slack)
 {
     pdl_sync();
     const int j = blockIdx.y;                      // step j+1 of the window
@@ -132,7 +132,9 @@ k_transport_partial(int n, uint64_t seed, const uint64_t* __restrict__ n0p, cons
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const double Fe = dF ? Ft[base + (size_t)c * n + i] + dF[c * n + i] : Ft[base + (size_t)c * n + i];   // EC: the draft was drawn around F~ + dF
-            const double d = bs * (Fe - Fg[base + (size_t)c * n + i]);
+            double dFo = Fe - Fg[base + (size_t)c * n + i];
+            if (slack > 0.0) dFo -= fmin(fmax(dFo, -slack), slack);       // force slack (App. H :779): F_(eps) = F + clip(-eps; F~ - F; eps) in the place of F
+            const double d = bs * dFo;
             s1 += xi[c] * d;
             s2 += d * d;
             if (xi_dbg) xi_dbg[base + (size_t)c * n + i] = xi[c];
@@ -194,7 +196,7 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
                          const double* __restrict__ Fg, const double* __restrict__ qhalf, const double* __restrict__ pstart,
                          double* __restrict__ yq, double* __restrict__ yp, const double* __restrict__ mass,
                          const double* __restrict__ sigma, double c1, double b, double hdt, double* __restrict__ q_base,
-                         double* __restrict__ p_base, const double* __restrict__ dF, double* __restrict__ dF_out)
+                         double* __restrict__ p_base, const double* __restrict__ dF, double* __restrict__ dF_out, double slack)
 {
     pdl_sync();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -219,8 +221,9 @@ __global__ void k_commit(int n, int K, uint64_t seed, const uint64_t* __restrict
     const double sg = sigma[i], m = mass[i], ratio = S1[l - 1] / S2[l - 1];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double F = Fg[base + (size_t)c * n + i];
+        double F = Fg[base + (size_t)c * n + i];
         const double Fe = dF ? Ft[base + (size_t)c * n + i] + dF[c * n + i] : Ft[base + (size_t)c * n + i];
+        if (slack > 0.0) F += fmin(fmax(Fe - F, -slack), slack);          // F_(eps) of App. H replaces the target force in the override too
         const double d = b / sg * (Fe - F);
         const double ps = c1 * pprev[c * n + i] + b * F + sg * (xi[c] - 2.0 * ratio * d);
         const double qs = qhalf[base + (size_t)c * n + i] + hdt * ps / m;
@@ -301,10 +304,10 @@ void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass
 
 void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const double* Ft, const double* Fg,
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
-                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF)
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF, double slack)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
-    launch_pdl(L, k_transport_partial, dim3(nblk, K), dim3(kTrThreads), 0, n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg, dF);
+    launch_pdl(L, k_transport_partial, dim3(nblk, K), dim3(kTrThreads), 0, n, seed, n0, Ft, Fg, sigma, b, partial, xi_dbg, dF, slack);
     LSD_COUNT(L);
     launch_pdl(L, k_transport_final, dim3(1), dim3(LSD_MAX_K), 0, K, nblk, seed, n0, partial, S1, S2, ell, lnu, reject, flags, result);
     LSD_COUNT(L);
@@ -314,11 +317,11 @@ void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n
 void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0, const TransportResult* result,
                    const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
-                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out)
+                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out, double slack)
 {
     const int pid = prof_begin(L, PROF_TRANSPORT);
     launch_pdl(L, k_commit, dim3((n + 127) / 128), dim3(128), 0, n, K, seed, n0, result, S1, S2, Ft, Fg, qhalf, pstart, yq, yp, mass, sigma,
-                                               c1, b, hdt, q_base, p_base, dF, dF_out);
+                                               c1, b, hdt, q_base, p_base, dF, dF_out, slack);
     LSD_COUNT(L);
     prof_end(L, pid);
 }

@@ -42,6 +42,7 @@ struct lsd_ctx {
     std::vector<void*> allocs;
     std::vector<void*> list_allocs;                          // neighbour-list rows: freed and re-made by setup_lists (lsd_set_skin)
     bool alloc_lists = false;                                // dalloc files under list_allocs
+    double slack = 0.0;                                      // force slack eps_F of App. H (0 = off: exact)
     double cap_growth = 1.0;                                 // extra head room of the rows after an overflow (x 1.5 per retry)
     double c1 = 0, b = 0, hdt = 0, kT = 0;
     double *q = nullptr, *p = nullptr;
@@ -643,9 +644,9 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
     TRY(run_graphed(ctx, st, w.g_transport[K], [&]() -> lsd_status {
         Launcher Lg = mk(ctx, stream);
         launch_transport(Lg, n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk, ctx->S1, ctx->S2,
-                         ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr);
+                         ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr, ctx->slack);
         launch_commit(Lg, n, K, ctx->cfg.seed, w.n0_dev, ctx->result, ctx->S1, ctx->S2, w.Ft, ctx->Fg, w.qhalf, w.pstart, w.yq, w.yp,
-                      ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p, ctx->ec ? w.dF : nullptr, ctx->ec ? ctx->dF : nullptr);
+                      ctx->sys.mass, ctx->sys.sigma, ctx->c1, ctx->b, ctx->hdt, ctx->q, ctx->p, ctx->ec ? w.dF : nullptr, ctx->ec ? ctx->dF : nullptr, ctx->slack);
         return LSD_OK;
     }));
     CK(cudaMemcpyAsync(ctx->result_host, ctx->result, sizeof(TransportResult), cudaMemcpyDeviceToHost, st));
@@ -839,6 +840,15 @@ lsd_status lsd_set_error_correction(lsd_ctx* ctx, int32_t enable)
     return LSD_OK;
 }
 
+lsd_status lsd_set_force_slack(lsd_ctx* ctx, double eps_F)
+{
+    if (!ctx || !(eps_F >= 0.0)) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    ctx->slack = eps_F;
+    drop_graphs(ctx);                                        // the captured kernels take the value by value
+    return LSD_OK;
+}
+
 lsd_status lsd_get_ec_cache(lsd_ctx* ctx, double* dF, int32_t where)
 {
     if (!ctx || !dF) return LSD_ERR_INVALID_ARG;
@@ -919,7 +929,7 @@ lsd_status lsd_get_window_debug(lsd_ctx* ctx, int32_t what, void* out, int32_t w
         case LSD_DBG_XI: {
             if (!ctx->xi_dbg) TRY(dalloc(ctx, &ctx->xi_dbg, (size_t)3 * ctx->sys.n * ctx->cfg.k_max));
             launch_transport(mk(ctx, nullptr), ctx->sys.n, K, ctx->cfg.seed, w.n0_dev, w.Ft, ctx->Fg, ctx->sys.sigma, ctx->b, ctx->partial, ctx->nblk,
-                             ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr);
+                             ctx->S1, ctx->S2, ctx->ell, ctx->lnu, ctx->reject, w.flags, ctx->result, ctx->xi_dbg, ctx->ec ? w.dF : nullptr, ctx->slack);
             CK(cudaDeviceSynchronize());
             return copy_out(ctx, out, ctx->xi_dbg, big, where);
         }

@@ -186,11 +186,11 @@ void launch_initial_momenta(Launcher L, int n, uint64_t seed, const double* mass
 struct TransportResult { int first_reject, n_commit, flags, pad; double beta_sum; };
 void launch_transport(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_dev, const double* Ft, const double* Fg,
                       const double* sigma, double b, double* partial, int nblk, double* S1, double* S2, double* ell,
-                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF);
+                      double* lnu, int* reject, const int* flags, TransportResult* result, double* xi_dbg, const double* dF, double slack = 0.0);
 void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_dev, const TransportResult* result,
                    const double* S1, const double* S2, const double* Ft, const double* Fg, const double* qhalf,
                    const double* pstart, double* yq, double* yp, const double* mass, const double* sigma,
-                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out);
+                   double c1, double b, double hdt, double* q_base, double* p_base, const double* dF, double* dF_out, double slack = 0.0);
 int transport_blocks(int n);
 void launch_obabo(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* p_new,
                   const double* F, const double* mass, double kT, double c1, double ch, double hdt, double* p_mid);
