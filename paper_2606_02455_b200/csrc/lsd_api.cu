@@ -73,6 +73,8 @@ struct lsd_ctx {
     int ec = 0;                                              // speculative error correction (Alg. 3) on / off
     double* dF = nullptr;                                    // [3][n] EC cache: F - F~(bare) of the last committed step
     bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
+    bool tiny = false;                                       // draft rollout as one kernel launch (tiny_rollout.cu; LSD_TINY=0 disables)
+    std::vector<cudaStream_t> busy;                          // caller streams that may still hold work of this context (lsd_get_state / lsd_set_state wait for these only)
     Prof prof;
     lsd_stats stats{};
     std::string err;
@@ -111,6 +113,17 @@ template <typename T> lsd_status upload(lsd_ctx* ctx, T** p, const T* host, size
 #define TRY(expr) do { lsd_status s__ = (expr); if (s__ != LSD_OK) return s__; } while (0)
 
 Launcher mk(lsd_ctx* ctx, void* stream) { return Launcher{(cudaStream_t)stream, &ctx->launches, &ctx->prof}; }
+
+void note_stream(lsd_ctx* ctx, cudaStream_t st) { if (std::find(ctx->busy.begin(), ctx->busy.end(), st) == ctx->busy.end()) ctx->busy.push_back(st); }
+void stream_idle(lsd_ctx* ctx, cudaStream_t st) { ctx->busy.erase(std::remove(ctx->busy.begin(), ctx->busy.end(), st), ctx->busy.end()); }
+// wait for the work this context has enqueued (not for the whole device: a state read-back between windows costs one
+// stream synchronisation, cfg1's end-to-end window is ~0.1 ms)
+lsd_status sync_pending(lsd_ctx* ctx)
+{
+    for (cudaStream_t st : ctx->busy) CK(cudaStreamSynchronize(st));
+    ctx->busy.clear();
+    return LSD_OK;
+}
 
 void drop_graphs(lsd_ctx* ctx)
 {
@@ -412,6 +425,12 @@ lsd_status rollout_body(lsd_ctx* ctx, WindowSlot& w, int K, int which, void* str
     CK(cudaMemsetAsync(w.flags, 0, sizeof(int), st));
     build_lists(ctx, Lg, w.qstart, w.img, w.vl_mlip, w.vl_pair, w.flags);
     const double sh = 0.5 * ctx->cfg.skin, sh2 = sh * sh;
+    if (ctx->tiny && which == LSD_DRAFT) {                                    // one launch for the K steps (the lists above serve the verification)
+        Lg.draft = 1;
+        launch_tiny_rollout(Lg, ctx->sys, ctx->pot[LSD_DRAFT], K, ctx->cfg.seed, w.n0_dev, ctx->c1, ctx->b, ctx->hdt, sh2, w.qstart, w.pstart,
+                            ec ? w.dF : nullptr, w.qhalf, w.Ft, w.yq, w.yp, w.flags);
+        return LSD_OK;
+    }
     for (int j = 1; j <= K; ++j) {                                            // serial in j
         const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
         double* qh = w.qhalf + n3 * (j - 1);
@@ -523,6 +542,17 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
     }
     TRY(upload_potential(ctx, *draft, ctx->pot[LSD_DRAFT]));
     TRY(upload_potential(ctx, *target, ctx->pot[LSD_TARGET]));
+    {   // Tiny systems: the draft rollout is one kernel (tiny_rollout.cu).  Its sums run in another order than the batched kernels,
+        // so it is used only where the draft is a different potential: draft == target must reproduce the target bitwise (R8).
+        auto n_weights = [&](const lsd_mlip& m) { const size_t F = m.width, R = m.n_rbf; return (size_t)m.n_species * F + (size_t)m.n_blocks * (4 * F * F + F * R) + (F / 2) * F + F / 2; };
+        bool same = draft->use_bonded == target->use_bonded && draft->mlip.width == target->mlip.width &&
+                    std::memcmp(draft->pair, target->pair, sizeof(double) * (size_t)sys->n_species * sys->n_species * LSD_PAIR_COLS) == 0;
+        if (same && draft->mlip.width > 0)
+            same = draft->mlip.n_blocks == target->mlip.n_blocks && draft->mlip.cutoff == target->mlip.cutoff && draft->mlip.energy_scale == target->mlip.energy_scale &&
+                   std::memcmp(draft->mlip.weights, target->mlip.weights, sizeof(double) * n_weights(draft->mlip)) == 0;
+        const char* tv = getenv("LSD_TINY");
+        ctx->tiny = !same && !(tv && tv[0] == '0') && tiny_rollout_supported(ctx->sys, ctx->pot[LSD_DRAFT]);
+    }
     ctx->bmax[LSD_DRAFT] = 1; ctx->bmax[LSD_TARGET] = kmax;
 
     const size_t n3 = (size_t)3 * n;
@@ -590,6 +620,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
     WindowSlot& w = ctx->slot[si];
     cudaStream_t st = (cudaStream_t)stream;
     Launcher L = mk(ctx, stream);
+    note_stream(ctx, st);
     if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));          // a discarded rollout into this slot may still run
     if (ctx->pending == 0) {
         CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -621,6 +652,7 @@ lsd_status lsd_verify_window(lsd_ctx* ctx, int32_t K, void* stream)
     if (ctx->pending < 1 || !w.drafted) return fail(ctx, LSD_ERR_STATE, "no drafted window to verify");
     if (K != w.K) return fail(ctx, LSD_ERR_INVALID_ARG, "K differs from the drafted window length");
     cudaStream_t st = (cudaStream_t)stream;
+    note_stream(ctx, st);
     CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
     TRY(run_graphed(ctx, st, w.g_verify[K], [&]() -> lsd_status {
         eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr);
@@ -651,6 +683,7 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
     }));
     CK(cudaMemcpyAsync(ctx->result_host, ctx->result, sizeof(TransportResult), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    stream_idle(ctx, st);
     CK(cudaGetLastError());
     const TransportResult r = *ctx->result_host;
     ctx->last_slot = ctx->verify_idx; ctx->last_K = K;
@@ -772,6 +805,7 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
     if (!ctx || (which != LSD_DRAFT && which != LSD_TARGET) || n_steps < 0) return LSD_ERR_INVALID_ARG;
     if (ctx->pending) return fail(ctx, LSD_ERR_STATE, "a drafted window is pending");
     cudaStream_t st = (cudaStream_t)stream;
+    note_stream(ctx, st);
     const size_t n3 = (size_t)3 * ctx->sys.n;
     WindowSlot& w = ctx->slot[ctx->verify_idx];
     int list_retries = 0;
@@ -807,10 +841,12 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
 lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int32_t where)
 {
     if (!ctx) return LSD_ERR_INVALID_ARG;
-    CK(cudaDeviceSynchronize());
+    TRY(sync_pending(ctx));
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
-    if (q) TRY(copy_out(ctx, q, ctx->q, bytes, where));
-    if (p) TRY(copy_out(ctx, p, ctx->p, bytes, where));
+    const cudaMemcpyKind kind = where == LSD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    if (q) CK(cudaMemcpyAsync(q, ctx->q, bytes, kind, ctx->side));
+    if (p) CK(cudaMemcpyAsync(p, ctx->p, bytes, kind, ctx->side));
+    if (q || p) CK(cudaStreamSynchronize(ctx->side));
     if (step) *step = ctx->step;
     return LSD_OK;
 }
@@ -818,13 +854,14 @@ lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int3
 lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t step, int32_t where)
 {
     if (!ctx || !q || !p) return LSD_ERR_INVALID_ARG;
-    CK(cudaDeviceSynchronize());
+    TRY(sync_pending(ctx));
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
     const cudaMemcpyKind kind = where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-    CK(cudaMemcpy(ctx->q, q, bytes, kind));
-    CK(cudaMemcpy(ctx->p, p, bytes, kind));
+    CK(cudaMemcpyAsync(ctx->q, q, bytes, kind, ctx->side));
+    CK(cudaMemcpyAsync(ctx->p, p, bytes, kind, ctx->side));
     ctx->step = step; ctx->stats.step = step;
-    CK(cudaMemset(ctx->dF, 0, bytes));                        // a new trajectory starts with an empty EC cache
+    if (ctx->ec) CK(cudaMemsetAsync(ctx->dF, 0, bytes, ctx->side));   // a new trajectory starts with an empty EC cache; it is all zeros while EC is off
+    CK(cudaStreamSynchronize(ctx->side));
     ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
     return LSD_OK;
 }
@@ -1024,6 +1061,7 @@ lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t 
     if (!ctx || !start || !n_edges || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
     const CompactList& cl = kind == 0 ? ctx->cl_mlip[which] : ctx->cl_pair[which];
     if (!cl.count || !ctx->cl_img[which]) return fail(ctx, LSD_ERR_STATE, "this potential has no such list (or no evaluation has run yet)");
+    if (ctx->tiny && which == LSD_DRAFT) return fail(ctx, LSD_ERR_STATE, "the one-kernel draft rollout of a tiny system keeps its neighbour rows on chip");
     if (b < 0 || b >= cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "state index out of range");
     CK(cudaDeviceSynchronize());
     const int n = ctx->sys.n;

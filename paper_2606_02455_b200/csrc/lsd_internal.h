@@ -13,6 +13,8 @@
 #define LSD_AMU_EV  103.642696       // eV fs^2 / A^2 per amu
 #define LSD_NRBF    32               // R (M1)
 #define LSD_MAX_K   64
+#define LSD_TINY_MAX_ATOMS 64      // systems up to this size roll their draft out in one kernel launch (tiny_rollout.cu)
+#define LSD_TINY_CLUSTER 8         // ... on one thread-block cluster of this many CTAs
 
 // flags raised on the device during a window
 #define LSD_FLAG_SKIN      1
@@ -194,6 +196,12 @@ void launch_commit(Launcher L, int n, int K, uint64_t seed, const uint64_t* n0_d
 int transport_blocks(int n);
 void launch_obabo(Launcher L, int n, uint64_t seed, const uint64_t* n0_dev, uint64_t j, const double* p_prev, const double* p_new,
                   const double* F, const double* mass, double kT, double c1, double ch, double hdt, double* p_mid);
+
+// ---- tiny_rollout.cu: the K draft steps of a window of a tiny system as one kernel launch
+bool tiny_rollout_supported(const SysDev& sys, const PotDev& pot);
+void launch_tiny_rollout(Launcher L, const SysDev& sys, const PotDev& pot, int K, uint64_t seed, const uint64_t* n0_dev,
+                         double c1, double b, double hdt, double skin_half2, const double* qstart, const double* pstart,
+                         const double* dF /*EC cache or null*/, double* qhalf, double* Ft, double* yq, double* yp, int* flags);
 
 // ---- neighbor.cu
 void cellgrid_setup(CellGrid& g, const SysDev& sys, double rc_skin);
