@@ -252,6 +252,11 @@ const char* lsd_version(void);
 lsd_status lsd_get_edge_launch_info(int32_t pass, int32_t* out);
 /* 1 if the target network's filter contractions run on the bf16 tcgen05 path in this context, else 0. */
 int32_t     lsd_tc_enabled(const lsd_ctx* ctx);
+/* 1 if lsd_draft_rollout drafts a window with ONE kernel launch in this context (a0: the K serial
+ * DRAFT_STEPs of a system of <= 64 atoms on one thread-block cluster), else 0 (one launch sequence
+ * per step).  It is used when the draft is a different potential than the target and is a prior with at most a width-32,
+ * one-block network; the environment variable LSD_TINY=0, read by lsd_init, turns it off (A/B measurements). */
+int32_t     lsd_tiny_rollout_enabled(const lsd_ctx* ctx);
 
 #ifdef __cplusplus
 }

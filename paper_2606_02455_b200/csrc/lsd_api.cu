@@ -466,6 +466,8 @@ int32_t lsd_tc_enabled(const lsd_ctx* ctx)
     return ctx && ctx->cfg.precision == LSD_BF16_TC && ctx->pot[LSD_TARGET].mlip.F > 0 && mlip_tc_supported(ctx->pot[LSD_TARGET].mlip) ? 1 : 0;
 }
 
+int32_t lsd_tiny_rollout_enabled(const lsd_ctx* ctx) { return ctx && ctx->tiny ? 1 : 0; }
+
 void lsd_destroy(lsd_ctx* ctx)
 {
     if (!ctx) return;
