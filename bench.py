@@ -11,7 +11,8 @@ committed ("accepted target-exact") MD steps/s is reported beside it.  One JSON 
 The line of the default run also carries `all_workloads` (the other BASELINE.json workloads, a few windows each, same
 measurement code), `measured_peaks` (fp32 / fp64 FMA peaks measured by a kernel of the library, next to the driver's
 MEASURED_PEAKS.json), a three-term roofline of the batched force evaluation (tensor, HBM, special-function unit) and a
-labelled `acceptance_variant` (draft = target with the gap shrunk until Eq. 9 gives beta ~ 0.1).
+labelled `acceptance_variant` (draft = target with the gap shrunk until Eq. 9 gives beta ~ 0.1), and `async_depth` (committed steps/s
+with 0 / 1 / 3 speculative windows drafted ahead on the second stream, Alg. 2 on one device).
 
 Multi-GPU (weak scaling): every rank runs an independent replica of the workload (its own seed); there is no
 data-path collective.  --impl reference times the CPU oracle (oracle/, fp64, as it stands).
@@ -380,6 +381,38 @@ def build_roofline(env, w, name, precision, prec, ctx, prof, edges, steps, ms_pr
     return roofline, dtype
 
 
+def async_depth_block(env, cases=(("cfg1", None, 0), ("cfg1", None, 1), ("cfg2", "fp32", 1), ("cfg4", "bf16", 1)), depths=(0, 1, 3), slots=4, windows=24):
+    """Labelled side block (SURVEY.md 8(f) rank 3; Alg. 2 on one device, PAPER.md:555-566 Eq. 21 vs Eq. 22, :568-618): committed steps/s of
+    lsd_run at the configuration's K with 0, 1 and 3 speculative windows kept drafted ahead on the second stream (ring of `slots` window
+    slots), on the workloads whose acceptance is high enough for a speculative rollout to survive (EC = error correction, Alg. 3)."""
+    torch, L, P, stream = env["torch"], env["L"], env["P"], env["stream"]
+    out = {}
+    for name, precision, ec in cases:
+        w = L.make_workload(name)
+        K = w.K
+        prec = {"fp32": P.LSD_FP32, "bf16": P.LSD_BF16_TC, None: None}[precision]
+        ctx = P.context_from_workload(w, precision=prec)
+        P.lsd_set_window_slots(ctx.h, slots)
+        if ec:
+            P.lsd_set_error_correction(ctx.h, True)
+        res = dict(window_K=K, window_slots=slots, error_correction=bool(ec), committed_md_steps_per_s={})
+        for d in depths:
+            P.lsd_run(ctx.h, 4 * K, K, overlap=d, stream=stream)           # warm (graph capture of every slot)
+            st0 = P.lsd_get_stats(ctx.h)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            P.lsd_run(ctx.h, windows * K, K, overlap=d, stream=stream)
+            a1.record(stream)
+            torch.cuda.synchronize()
+            st1 = P.lsd_get_stats(ctx.h)
+            nc = st1["committed_steps"] - st0["committed_steps"]
+            res["committed_md_steps_per_s"][str(d)] = nc / (a0.elapsed_time(a1) * 1e-3)
+            res["acceptance_alpha"] = 1.0 - (st1["rejections"] - st0["rejections"]) / max(nc, 1)
+        ctx.close()
+        out[name + ("" if precision is None else "_" + precision) + ("_ec" if ec else "")] = res
+    return out
+
+
 def acceptance_variant(env, name, precision, target_beta=0.1, windows=6):
     """Labelled side block (last paragraph): the same workload with the draft / target gap shrunk until Eq. 9
     (beta = erf(|delta| / sqrt 8)) gives beta ~ target_beta per step, so that 'accepted target-exact MD steps/s' and the
@@ -528,7 +561,7 @@ def main():
 
     m = measure_workload(env, args.workload, args.precision, args.steps, args.warmup, full=True, ec=args.ec, overlap=args.overlap)
 
-    side, variant = None, None
+    side, variant, ring = None, None, None
     if not args.no_side and world == 1 and not args.ec and not args.overlap:
         # the other BASELINE.json workloads, a few windows each, through the same measurement code (the headline is listed again in short form)
         side = {}
@@ -545,6 +578,7 @@ def main():
                                            three_term=rf.get("a2_three_term")),
                              clocks=r["clocks"], steps=SIDE_STEPS if r is not m else args.steps)
         variant = acceptance_variant(env, args.workload, args.precision)
+        ring = async_depth_block(env)
 
     if rank == 0:
         N, K = m["n_atoms"], m["window_K"]
@@ -567,6 +601,8 @@ def main():
             line["all_workloads"] = side
         if variant is not None:
             line["acceptance_variant"] = variant
+        if ring is not None:
+            line["async_depth"] = ring
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = {k: v for k, v in cpu_baseline(args.workload).items() if k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))

@@ -122,7 +122,7 @@ const char* lsd_last_error(const lsd_ctx* ctx);   /* ctx may be NULL: error of t
  * (the base state, or y_K of the previous, still unverified window), storing per step q_half_j,
  * draft forces F~_j and y_j in the next window slot.  Builds the window-shared Verlet lists from the
  * head state first.  Noise xi_j = Philox(seed; step index n + j, atom) (R5).  Asynchronous.
- * Errors: INVALID_ARG (K < 1 or > k_max), STATE (two unverified windows already drafted). */
+ * Errors: INVALID_ARG (K < 1 or > k_max), STATE (every window slot already holds an unverified window). */
 lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream);
 
 /* a1 + a2 (PAPER.md:598-599 VERIFY_STEP): one batched target force evaluation F_j = F(q_half_j) for
@@ -144,10 +144,17 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
  * any speculative window is discarded and the draft head returns to the base state (also for l == K). */
 lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject);
 
-/* Convenience driver: repeat {rollout, verify (+ speculative rollout of the next window on a second
- * internal stream when overlap != 0), transport, rollback} until n_steps more steps are committed
- * (the last window is shortened).  Synchronous. */
+/* Convenience driver: repeat {rollout, verify, transport, rollback} until n_steps more steps are committed (the last
+ * window is shortened).  overlap = d > 0: Alg. 2's asynchronous drafting on one device (Eq. 22 against the
+ * synchronous Eq. 21, :555-566): while a window is verified, up to d speculative windows -- each continuing from y_K of the
+ * one before it -- are kept drafted ahead on a second internal stream, so the drafter never waits for the 8-byte verdict; a
+ * rejection flushes all of them (:611-612).  d is capped at (window slots - 1); the committed trajectory does not depend
+ * on d (R5).  Synchronous. */
 lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, void* stream);
+/* Number of window slots of the context (2 after lsd_init, at most 8): lsd_draft_rollout may hold that many drafted,
+ * unverified windows (Alg. 2's buffers of drafted steps); every slot owns its window rows and its
+ * window-shared neighbour lists.  Synchronises, drops drafted windows.  Errors: INVALID_ARG, OOM. */
+lsd_status lsd_set_window_slots(lsd_ctx* ctx, int32_t n_slots);
 /* lsd_run with K = 0: adaptive lookahead (the window length is the paper's free parameter L): K moves
  * over {1, 2, 4, ..., k_max} by hill climbing on the measured committed steps per second.  With error correction off the
  * committed trajectory does not depend on the K sequence (R5).  lsd_get_adaptive_k: the length it last settled on (0: never). */

@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_roll
                     "lsd_rollback", "lsd_run", "lsd_get_state", "lsd_set_state", "lsd_get_stats", "lsd_get_window_state",
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
                     "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k",
-                    "lsd_get_window_obabo", "lsd_get_edge_launch_info", "lsd_measure_fma_peak", "lsd_set_force_slack", "lsd_tiny_rollout_enabled"]
+                    "lsd_get_window_obabo", "lsd_get_edge_launch_info", "lsd_measure_fma_peak", "lsd_set_force_slack", "lsd_tiny_rollout_enabled", "lsd_set_window_slots"]
 
 
 class LsdError(RuntimeError):
@@ -298,6 +298,10 @@ def lsd_measure_fma_peak(kind: int, stream=None) -> float:
 
 def lsd_tc_enabled(h) -> bool:
     return bool(load_library().lsd_tc_enabled(h))
+
+
+def lsd_set_window_slots(h, n_slots: int):
+    _check(h, load_library().lsd_set_window_slots(h, C.c_int32(n_slots)))
 
 
 def lsd_tiny_rollout_enabled(h) -> bool:

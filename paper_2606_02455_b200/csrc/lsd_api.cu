@@ -47,7 +47,8 @@ struct lsd_ctx {
     double c1 = 0, b = 0, hdt = 0, kT = 0;
     double *q = nullptr, *p = nullptr;
     int64_t step = 0;
-    WindowSlot slot[2];
+    WindowSlot slot[LSD_MAX_SLOTS];                          // ring of window slots: [verify_idx, verify_idx + pending) are drafted and unverified
+    int nslots = 2;                                          // slots in use (lsd_set_window_slots)
     int verify_idx = 0, pending = 0, last_slot = -1, last_K = 0, last_l = 0, last_nc = 0, transported = 0;
     MlipWork work[2];
     CompactList cl_mlip[2], cl_pair[2];
@@ -127,7 +128,7 @@ lsd_status sync_pending(lsd_ctx* ctx)
 
 void drop_graphs(lsd_ctx* ctx)
 {
-    for (int s = 0; s < 2; ++s)
+    for (int s = 0; s < LSD_MAX_SLOTS; ++s)
         for (auto* m : {&ctx->slot[s].g_roll, &ctx->slot[s].g_verify, &ctx->slot[s].g_transport, &ctx->slot[s].g_plain}) {
             for (auto& kv : *m) if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
             m->clear();
@@ -348,7 +349,7 @@ lsd_status setup_lists_impl(lsd_ctx* ctx)
     if (ctx->rc_pair_max > 0) TRY(probe_capacity(ctx, ctx->rc_pair_max + skin, &ctx->cap_pair));
     // equal cutoffs (cfg5: Morse and network both 6 A): one Verlet list serves both, build_lists builds it once
     const bool shared = ctx->cap_mlip && ctx->cap_pair && ctx->rc_mlip_max == ctx->rc_pair_max;
-    for (int s = 0; s < 2; ++s) {
+    for (int s = 0; s < ctx->nslots; ++s) {
         if (ctx->cap_mlip) TRY(alloc_verlet(ctx, ctx->slot[s].vl_mlip, ctx->cap_mlip, ctx->rc_mlip_max));
         if (shared) ctx->slot[s].vl_pair = ctx->slot[s].vl_mlip;
         else if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->slot[s].vl_pair, ctx->cap_pair, ctx->rc_pair_max));
@@ -361,6 +362,26 @@ lsd_status setup_lists_impl(lsd_ctx* ctx)
         if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w], false));
     }
     return LSD_OK;
+}
+
+// state, window rows and event of ring slot s (its neighbour lists are made by setup_lists)
+lsd_status alloc_slot(lsd_ctx* ctx, int s)
+{
+    const size_t n3 = (size_t)3 * ctx->sys.n;
+    const int kmax = ctx->cfg.k_max;
+    WindowSlot& w = ctx->slot[s];
+    if (w.qstart) return LSD_OK;
+    TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
+    TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
+    TRY(dalloc(ctx, &w.img, ctx->sys.n)); TRY(dalloc(ctx, &w.flags, 1)); TRY(dalloc(ctx, &w.n0_dev, 1));
+    TRY(dalloc(ctx, &w.dF, n3)); CK(cudaMemset(w.dF, 0, n3 * sizeof(double)));
+    CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
+    return LSD_OK;
+}
+void reset_slots(lsd_ctx* ctx)                               // nothing drafted, nothing verified
+{
+    ctx->pending = 0; ctx->transported = 0;
+    for (int s = 0; s < LSD_MAX_SLOTS; ++s) { ctx->slot[s].drafted = 0; ctx->slot[s].verified = 0; }
 }
 
 // Window-shared lists from the reference state qref (a1).
@@ -477,7 +498,7 @@ void lsd_destroy(lsd_ctx* ctx)
     for (void* p : ctx->list_allocs) cudaFree(p);
     cudaFree(ctx->grid.cell_count); cudaFree(ctx->grid.cell_start); cudaFree(ctx->grid.cell_cursor);
     cudaFree(ctx->grid.cell_atoms); cudaFree(ctx->grid.atom_cell);
-    for (int s = 0; s < 2; ++s) if (ctx->slot[s].ev_drafted) cudaEventDestroy(ctx->slot[s].ev_drafted);
+    for (int s = 0; s < LSD_MAX_SLOTS; ++s) if (ctx->slot[s].ev_drafted) cudaEventDestroy(ctx->slot[s].ev_drafted);
     for (cudaEvent_t e : ctx->prof.ev) cudaEventDestroy(e);
     if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->result_host) cudaFreeHost(ctx->result_host);
@@ -563,14 +584,7 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
     if (p0) CK(cudaMemcpy(ctx->p, p0, n3 * sizeof(double), cudaMemcpyHostToDevice));
     else launch_initial_momenta(mk(ctx, nullptr), n, cfg->seed, S.mass, ctx->kT, ctx->p);
     TRY(setup_lists(ctx));
-    for (int s = 0; s < 2; ++s) {
-        WindowSlot& w = ctx->slot[s];
-        TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
-        TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
-        TRY(dalloc(ctx, &w.img, n)); TRY(dalloc(ctx, &w.flags, 1)); TRY(dalloc(ctx, &w.n0_dev, 1));
-        TRY(dalloc(ctx, &w.dF, n3)); CK(cudaMemset(w.dF, 0, n3 * sizeof(double)));
-        CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
-    }
+    for (int s = 0; s < ctx->nslots; ++s) TRY(alloc_slot(ctx, s));
     for (int w = 0; w < 2; ++w) if (ctx->pot[w].mlip.F > 0) TRY(alloc_work(ctx, ctx->pot[w].mlip, ctx->work[w], ctx->bmax[w]));
     TRY(dalloc(ctx, &ctx->Fg, n3 * kmax));
     TRY(dalloc(ctx, &ctx->dF, n3)); CK(cudaMemset(ctx->dF, 0, n3 * sizeof(double)));
@@ -607,30 +621,44 @@ lsd_status lsd_set_skin(lsd_ctx* ctx, double skin)
     CK(cudaDeviceSynchronize());
     ctx->cfg.skin = skin;
     drop_graphs(ctx);                                        // captured pointers and the skin value change
-    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
+    reset_slots(ctx);
     return setup_lists(ctx);      // frees the superseded rows
+}
+
+lsd_status lsd_set_window_slots(lsd_ctx* ctx, int32_t n_slots)
+{
+    if (!ctx || n_slots < 2 || n_slots > LSD_MAX_SLOTS) return LSD_ERR_INVALID_ARG;
+    CK(cudaDeviceSynchronize());
+    drop_graphs(ctx);
+    reset_slots(ctx);
+    ctx->verify_idx = 0; ctx->last_slot = -1;
+    ctx->nslots = n_slots;
+    for (int s = 0; s < n_slots; ++s) TRY(alloc_slot(ctx, s));
+    return setup_lists(ctx);                                 // every slot owns its window-shared Verlet lists
 }
 
 lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
 {
     if (!ctx) return LSD_ERR_INVALID_ARG;
     if (K < 1 || K > ctx->cfg.k_max) return fail(ctx, LSD_ERR_INVALID_ARG, "K must be in 1..k_max");
-    if (ctx->pending >= 2) return fail(ctx, LSD_ERR_STATE, "two unverified windows are already drafted");
+    if (ctx->pending >= ctx->nslots) return fail(ctx, LSD_ERR_STATE, "every window slot holds an unverified window (lsd_set_window_slots)");
     const int n = ctx->sys.n;
     const size_t n3 = (size_t)3 * n;
-    const int si = (ctx->verify_idx + ctx->pending) & 1;
+    const int si = (ctx->verify_idx + ctx->pending) % ctx->nslots;
     WindowSlot& w = ctx->slot[si];
     cudaStream_t st = (cudaStream_t)stream;
     Launcher L = mk(ctx, stream);
     note_stream(ctx, st);
     if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));          // a discarded rollout into this slot may still run
     if (ctx->pending == 0) {
+        // flushed speculative rollouts may still run on another stream: they share the draft's work buffers
+        for (int s = 0; s < ctx->nslots; ++s) if (s != si && ctx->slot[s].ev_drafted) CK(cudaStreamWaitEvent(st, ctx->slot[s].ev_drafted, 0));
         CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         CK(cudaMemcpyAsync(w.pstart, ctx->p, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         if (ctx->ec) CK(cudaMemcpyAsync(w.dF, ctx->dF, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         w.n0 = (uint64_t)ctx->step;
     } else {                                                                  // speculative: continue from y_K of the unverified window
-        WindowSlot& pv = ctx->slot[si ^ 1];
+        WindowSlot& pv = ctx->slot[(si + ctx->nslots - 1) % ctx->nslots];
         CK(cudaStreamWaitEvent(st, pv.ev_drafted, 0));
         CK(cudaMemcpyAsync(w.qstart, pv.yq + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         CK(cudaMemcpyAsync(w.pstart, pv.yp + n3 * (pv.K - 1), n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -690,8 +718,7 @@ lsd_status lsd_transport_accept(lsd_ctx* ctx, int32_t K, void* stream, int32_t* 
     const TransportResult r = *ctx->result_host;
     ctx->last_slot = ctx->verify_idx; ctx->last_K = K;
     if (r.flags) {                                             // nothing committed: drop every drafted window
-        ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0;
-        ctx->transported = 0;
+        reset_slots(ctx);
         return flags_to_status(ctx, r.flags);
     }
     ctx->last_l = r.first_reject; ctx->last_nc = r.n_commit; ctx->transported = 1;
@@ -709,9 +736,9 @@ lsd_status lsd_rollback(lsd_ctx* ctx, int32_t first_reject)
     ctx->step += ctx->last_nc;
     ctx->stats.windows++; ctx->stats.committed_steps += ctx->last_nc; ctx->stats.rejections += first_reject ? 1 : 0; ctx->stats.step = ctx->step;
     w.drafted = 0; w.verified = 0;
-    ctx->verify_idx ^= 1; ctx->pending--;
-    if (first_reject != 0 && ctx->pending > 0) {              // flush the speculative window
-        ctx->slot[ctx->verify_idx].drafted = 0;
+    ctx->verify_idx = (ctx->verify_idx + 1) % ctx->nslots; ctx->pending--;
+    if (first_reject != 0 && ctx->pending > 0) {              // flush every speculative window
+        for (int s = 0; s < LSD_MAX_SLOTS; ++s) ctx->slot[s].drafted = 0;
         ctx->pending = 0;
     }
     ctx->transported = 0;
@@ -743,14 +770,25 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
     auto rate = [&](int i) { return a_t[i] > 0 ? a_nc[i] / a_t[i] : -1.0; };
     std::chrono::steady_clock::time_point t_win = std::chrono::steady_clock::now();
     int64_t remaining = n_steps;
+    const int depth = std::min(std::max((int)overlap, 0), ctx->nslots - 1);   // speculative windows kept in flight
     constexpr int kMaxListRetries = 6;                        // per call: a window that still fails returns its error
     int list_retries = 0;
     while (remaining > 0) {
         if (ctx->pending == 0) TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining), stream));
         const int k = ctx->slot[ctx->verify_idx].K;
         TRY(lsd_verify_window(ctx, k, stream));
-        if (overlap && remaining - k > 0 && ctx->pending == 1)
-            TRY(lsd_draft_rollout(ctx, (int32_t)std::min<int64_t>(K, remaining - k), ctx->side));   // speculative, second stream
+        if (depth > 0) {
+            // Alg. 2 semantics on one device: the drafter does not wait for the verdict of the window being
+            // verified; up to `depth` speculative windows stay drafted ahead on the second stream, each continuing from y_K of the
+            // one before it, all flushed by a rejection (:611-612)
+            int64_t ahead = 0;
+            for (int i = 0; i < ctx->pending; ++i) ahead += ctx->slot[(ctx->verify_idx + i) % ctx->nslots].K;
+            while (ctx->pending < 1 + depth && remaining - ahead > 0) {
+                const int kw = (int)std::min<int64_t>(K, remaining - ahead);
+                TRY(lsd_draft_rollout(ctx, kw, ctx->side));
+                ahead += kw;
+            }
+        }
         int32_t l = 0, nc = 0;
         lsd_status ts = lsd_transport_accept(ctx, k, stream, &l, &nc);
         if ((ts == LSD_ERR_SKIN_VIOLATED || ts == LSD_ERR_NBR_OVERFLOW) && list_retries < kMaxListRetries) {
@@ -791,12 +829,12 @@ lsd_status lsd_run(lsd_ctx* ctx, int64_t n_steps, int32_t K, int32_t overlap, vo
                 ctx->adaptive_k = 1 << a_home;
             }
         }
-        if (ctx->pending == 1 && ctx->slot[ctx->verify_idx].K > remaining) {   // cannot happen with the K choice above; defensive
+        if (ctx->pending >= 1 && ctx->slot[ctx->verify_idx].K > remaining) {   // cannot happen with the K choice above; defensive
             CK(cudaStreamSynchronize(ctx->side));
-            ctx->pending = 0; ctx->slot[ctx->verify_idx].drafted = 0;
+            reset_slots(ctx);
         }
     }
-    if (ctx->pending) { CK(cudaStreamSynchronize(ctx->side)); ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; }
+    if (ctx->pending) { CK(cudaStreamSynchronize(ctx->side)); reset_slots(ctx); }
     return LSD_OK;
 }
 
@@ -864,7 +902,7 @@ lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t
     ctx->step = step; ctx->stats.step = step;
     if (ctx->ec) CK(cudaMemsetAsync(ctx->dF, 0, bytes, ctx->side));   // a new trajectory starts with an empty EC cache; it is all zeros while EC is off
     CK(cudaStreamSynchronize(ctx->side));
-    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
+    reset_slots(ctx);
     return LSD_OK;
 }
 
@@ -875,7 +913,7 @@ lsd_status lsd_set_error_correction(lsd_ctx* ctx, int32_t enable)
     ctx->ec = enable ? 1 : 0;
     CK(cudaMemset(ctx->dF, 0, (size_t)3 * ctx->sys.n * sizeof(double)));
     drop_graphs(ctx);                                        // the captured kernels take the cache pointer (or null) by value
-    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0; ctx->slot[0].verified = ctx->slot[1].verified = 0; ctx->transported = 0;
+    reset_slots(ctx);
     return LSD_OK;
 }
 
@@ -901,7 +939,7 @@ lsd_status lsd_set_ec_cache(lsd_ctx* ctx, const double* dF, int32_t where)
     if (!ctx->ec) return fail(ctx, LSD_ERR_STATE, "error correction is off (lsd_set_error_correction)");
     CK(cudaDeviceSynchronize());
     CK(cudaMemcpy(ctx->dF, dF, (size_t)3 * ctx->sys.n * sizeof(double), where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice));
-    ctx->pending = 0; ctx->slot[0].drafted = ctx->slot[1].drafted = 0;
+    reset_slots(ctx);
     return LSD_OK;
 }
 

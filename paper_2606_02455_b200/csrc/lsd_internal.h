@@ -13,6 +13,7 @@
 #define LSD_AMU_EV  103.642696       // eV fs^2 / A^2 per amu
 #define LSD_NRBF    32               // R (M1)
 #define LSD_MAX_K   64
+#define LSD_MAX_SLOTS 8             // window slots of a context (lsd_set_window_slots)
 #define LSD_TINY_MAX_ATOMS 64      // systems up to this size roll their draft out in one kernel launch (tiny_rollout.cu)
 #define LSD_TINY_CLUSTER 8         // ... on one thread-block cluster of this many CTAs
 
