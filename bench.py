@@ -561,7 +561,7 @@ def main():
 
     m = measure_workload(env, args.workload, args.precision, args.steps, args.warmup, full=True, ec=args.ec, overlap=args.overlap)
 
-    side, variant, ring = None, None, None
+    side, variant, ring, design = None, None, None, None
     if not args.no_side and world == 1 and not args.ec and not args.overlap:
         # the other BASELINE.json workloads, a few windows each, through the same measurement code (the headline is listed again in short form)
         side = {}
@@ -579,6 +579,19 @@ def main():
                              clocks=r["clocks"], steps=SIDE_STEPS if r is not m else args.steps)
         variant = acceptance_variant(env, args.workload, args.precision)
         ring = async_depth_block(env)
+        # two design measurements DESIGN.md cites (section 4.1, section 7): tensor-memory bandwidth of an SM, and the second delivery of a
+        # half-list schedule at the headline workload's sizes (rows = half of the mean directed neighbour count)
+        wl = L.make_workload(args.workload)
+        nb_half = max(1, int(round(0.5 * m["roofline"].get("directed_edges_per_window", 0) / max(wl.K * wl.n_atoms, 1)))) if m["roofline"] else 0
+        design = dict(tmem_bytes_per_clk_per_sm={"ld_x16_%dw" % nw: P.lsd_measure_tmem_bandwidth(nw, False, stream) for nw in (1, 4, 8, 16)})
+        design["tmem_bytes_per_clk_per_sm"].update({"st_x16_%dw" % nw: P.lsd_measure_tmem_bandwidth(nw, True, stream) for nw in (4, 8, 16)})
+        if nb_half > 0 and wl.target.mlip is not None and wl.target.mlip.width == 128:
+            sc, ga = P.lsd_measure_half_list_delivery(wl.n_atoms, wl.K, nb_half, stream)
+            rows_gb = wl.n_atoms * wl.K * nb_half * 256e-9
+            design["half_list_delivery"] = dict(rows_per_atom=nb_half, rows_GB=rows_gb, scatter_ms=sc, ordered_gather_sum_ms=ga, total_ms=sc + ga,
+                                                edge_backward_launch_ms=m["roofline"].get("avg_launch_ms"),
+                                                note="one 256-byte bf16 row per undirected pair written to the partner's slot, then summed per atom in slot order: what a "
+                                                     "deterministic half-list schedule adds per edge pass; it replaces at most half of the edge kernel's launch time")
 
     if rank == 0:
         N, K = m["n_atoms"], m["window_K"]
@@ -603,6 +616,8 @@ def main():
             line["acceptance_variant"] = variant
         if ring is not None:
             line["async_depth"] = ring
+        if design is not None:
+            line["design_measurements"] = design
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = {k: v for k, v in cpu_baseline(args.workload).items() if k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))
