@@ -294,7 +294,7 @@ lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
         w.y16.resize(net.T);
         for (int t = 0; t < net.T; ++t) TRY(dalloc(ctx, &w.y16[t], e));
         TRY(dalloc(ctx, &w.mbar16, e));
-        if (net.F == 128) TRY(dalloc(ctx, &w.ym16, e));
+        TRY(dalloc(ctx, &w.ym16, e));
     }
     return LSD_OK;
 }

@@ -249,7 +249,7 @@ inline int lsd_sm_count()
 
 // which tcgen05 edge kernel the last forward / backward launch of this process used (parity tests assert that the timed
 // instantiation is the one they compared with the oracle): kernel 1 = k_edge_tc (mlip_tc.cu), 2 = k_edge_tc128, 3 = k_edge_er128_fwd,
-// 4 = k_edge_rows, 5 = k_edge_pipe
+// 4 = k_edge_rows, 5 = k_edge_pipe, 7 = k_edge_rows (narrow widths)
 struct EdgeLaunchInfo { int kernel = 0, atoms_per_chunk = 0, threads = 0, grid = 0, width = 0; };
 inline EdgeLaunchInfo g_edge_last[2];
 inline void note_edge_launch(bool backward, int kernel, int atoms_per_chunk, int threads, int grid, int width)
@@ -269,6 +269,7 @@ void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // ml
 void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
 void launch_edge_pipe(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_pipe.cu: width 128, warp-specialised pipeline of the same tile algebra
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_rows.cu: width 128, edges-as-rows, activations in TMEM
+void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward);   // mlip_edge_rows_narrow.cu: the same kernel, width-generic, for widths 32 / 64 (fp32 rows out)
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);
 void mlip_forward_backward_bf16tc(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,

@@ -13,6 +13,7 @@
 //                      F_a   += sum_j [ sum_f (mbar_a y_j + mbar_j y_a)_f w'_aj,f ] rhat_aj ;   xbar += W_in^T ybar
 #include <cuda_bf16.h>
 #include <algorithm>
+#include <cstdlib>
 #include "lsd_internal.h"
 
 namespace {
@@ -185,12 +186,17 @@ k_dense(int total, const float* __restrict__ in, const float* __restrict__ W0, c
                 } else {
                     stv<CPT>(out + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
                     if (out16) st16(out16 + (size_t)(g0 + r) * F + lane * CPT, acc2[r]);
-                    if (outpair) {                                         // (y, mbar) bf16 pairs for the width-128 backward edge kernel
+                    if (outpair) {
+                        // rows gathered by the edges-as-rows backward kernel (mlip_edge_rows.cu), pair layout: per channel pair
+                        // (f, f+1) the words (y_f | y_f+1 << 16), (mbar_f | mbar_f+1 << 16)
                         const size_t o = (size_t)(g0 + r) * F + lane * CPT;
+                        if constexpr (CPT >= 2) {
 #pragma unroll
-                        for (int c = 0; c < CPT; ++c) {
-                            const __nv_bfloat16 hb = __float2bfloat16_rn(acc2[r][c]);
-                            outpair[o + c] = (uint32_t)pair16[o + c] | ((uint32_t)*reinterpret_cast<const uint16_t*>(&hb) << 16);
+                            for (int c = 0; c < CPT; c += 2)
+                                *reinterpret_cast<uint2*>(outpair + o + c) = make_uint2(*reinterpret_cast<const uint32_t*>(pair16 + o + c), bf16x2(acc2[r][c], acc2[r][c + 1]));
+                        } else {
+                            const float nxt = __shfl_down_sync(0xffffffffu, acc2[r][0], 1);
+                            if ((lane & 1) == 0) *reinterpret_cast<uint2*>(outpair + o) = make_uint2(*reinterpret_cast<const uint32_t*>(pair16 + o), bf16x2(acc2[r][0], nxt));
                         }
                     }
                 }
@@ -376,6 +382,9 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         configured = true;
     }
     const int sms = num_sms();
+    // widths 32 / 64 on the tcgen05 path: the edges-as-rows kernel of mlip_edge_rows.cu (LSD_EDGE_NARROW=0: k_edge_tc of mlip_tc.cu)
+    static const bool narrow_env = [] { const char* v = getenv("LSD_EDGE_NARROW"); return !(v && v[0] == '0'); }();
+    const bool narrow_rows = use_tc && F < 128 && narrow_env;
     // 16 warps per CTA once every SM has at least 16 atoms to work on (occupancy: +8 % at cfg4 fp32); 8 for small batches,
     // whose kernels are latency-bound (a bigger CTA only adds to the weight-load and barrier time).  Same arithmetic either way.
     const int kWarps = total >= sms * kMaxWarps ? kMaxWarps : 8;
@@ -397,7 +406,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         pid = prof_begin(L, PROF_EDGE_FWD);
         if (use_tc) {
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t];
-            if (F == 128) launch_edge_tc128(L, ea, false); else launch_edge_tc(L, ea, F, false);
+            if (F == 128) launch_edge_tc128(L, ea, false); else if (narrow_rows) launch_edge_rows_narrow(L, ea, F, false); else launch_edge_tc(L, ea, F, false);
         }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
@@ -410,7 +419,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     prof_end(L, pidr);
     for (int t = net.T - 1; t >= 0; --t) {
         int pid = prof_begin(L, PROF_DENSE);
-        const bool pairs = use_tc && F == 128;
+        const bool pairs = use_tc && narrow_rows;               // (y, mbar) pair rows for k_edge_rows
         k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc && !pairs ? w.mbar16 : nullptr,
                                                                                  pairs ? w.y16[t] : nullptr, pairs ? w.ym16 : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
@@ -418,7 +427,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         pid = prof_begin(L, PROF_EDGE_BWD);
         if (use_tc) {
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; ea.ym16 = w.ym16;
-            if (F == 128) launch_edge_tc128(L, ea, true); else launch_edge_tc(L, ea, F, true);
+            if (F == 128) launch_edge_tc128(L, ea, true); else if (narrow_rows) launch_edge_rows_narrow(L, ea, F, true); else launch_edge_tc(L, ea, F, true);
         }
         else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
