@@ -57,6 +57,7 @@ struct lsd_ctx {
     CellGrid grid;
     double rc_mlip_max = 0, rc_pair_max = 0;
     int cap_mlip = 0, cap_pair = 0;
+    double* pair_rcs2 = nullptr;                             // [ns][ns] (largest pair cutoff of draft / target + skin)^2, 0 = the species pair has no pair term
     double* Fg = nullptr;
     double* obabo_p = nullptr;                               // scratch of lsd_get_window_obabo
     double *partial = nullptr, *S1 = nullptr, *S2 = nullptr, *ell = nullptr, *lnu = nullptr, *xi_dbg = nullptr;
@@ -257,6 +258,7 @@ lsd_status upload_potential(lsd_ctx* ctx, const lsd_potential& p, PotDev& d)
     }
     for (int s = 0; s < ns; ++s) { tether[s] = p.pair[((size_t)s * ns + s) * LSD_PAIR_COLS + 7]; if (tether[s] != 0.0) d.has_tether = 1; }
     TRY(upload(ctx, &d.pair_rc2, rc2.data(), rc2.size()));
+    d.pair_rc2_host = rc2;
     TRY(upload(ctx, &d.tether, tether.data(), tether.size()));
     if (p.mlip.width > 0) TRY(upload_mlip(ctx, p.mlip, d.mlip));
     return LSD_OK;
@@ -347,6 +349,19 @@ lsd_status setup_lists_impl(lsd_ctx* ctx)
     ctx->cap_mlip = ctx->cap_pair = 0;
     if (ctx->rc_mlip_max > 0) TRY(probe_capacity(ctx, ctx->rc_mlip_max + skin, &ctx->cap_mlip));
     if (ctx->rc_pair_max > 0) TRY(probe_capacity(ctx, ctx->rc_pair_max + skin, &ctx->cap_pair));
+    {   // pair-prior list: only the species pairs that interact, each with its own cutoff (cfg3: O-O only, a ninth of the candidates)
+        const int ns = ctx->sys.ns;
+        std::vector<double> t((size_t)ns * ns, 0.0);
+        for (int w = 0; w < 2; ++w) {
+            if (!ctx->pot[w].pair_rc2_host.size()) continue;
+            for (int a = 0; a < ns * ns; ++a) {
+                const double rc2 = ctx->pot[w].pair_rc2_host[a];
+                if (rc2 > 0.0) { const double r = std::sqrt(rc2) + skin; t[a] = std::max(t[a], r * r); }
+            }
+        }
+        ctx->pair_rcs2 = nullptr;
+        if (ctx->rc_pair_max > 0) TRY(upload(ctx, &ctx->pair_rcs2, t.data(), t.size()));
+    }
     // equal cutoffs (cfg5: Morse and network both 6 A): one Verlet list serves both, build_lists builds it once
     const bool shared = ctx->cap_mlip && ctx->cap_pair && ctx->rc_mlip_max == ctx->rc_pair_max;
     for (int s = 0; s < ctx->nslots; ++s) {
@@ -394,7 +409,7 @@ void build_lists(lsd_ctx* ctx, Launcher L, const double* qref, int* img, VerletL
     }
     if (ctx->cap_pair && vp.keys != vm.keys) {                   // (shared list when the cutoffs are equal, setup_lists)
         cellgrid_setup(ctx->grid, ctx->sys, ctx->rc_pair_max + ctx->cfg.skin);
-        launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_pair_max + ctx->cfg.skin, vp, flags);
+        launch_build_verlet(L, ctx->sys, ctx->grid, qref, img, ctx->rc_pair_max + ctx->cfg.skin, vp, flags, ctx->pair_rcs2);
     }
 }
 

@@ -56,6 +56,7 @@ struct PotDev {
     int ns = 0, use_bonded = 0;
     double* pair = nullptr;          // [ns*ns*8]
     double* pair_rc2 = nullptr;      // [ns*ns] squared cutoff of the pair term (0 = none)
+    std::vector<double> pair_rc2_host;
     double* tether = nullptr;        // [ns]
     double pair_rcmax = 0.0;
     int has_tether = 0;
@@ -208,7 +209,8 @@ void launch_tiny_rollout(Launcher L, const SysDev& sys, const PotDev& pot, int K
 void cellgrid_setup(CellGrid& g, const SysDev& sys, double rc_skin);
 void launch_pack_ref(Launcher L, const SysDev& sys, const double* qref, int* img);
 void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const double* qref, const int* img,
-                         double rc_skin, VerletList& vl, int* flags);
+                         double rc_skin, VerletList& vl, int* flags,
+                         const double* pair_rcs2 = nullptr /*[ns][ns] per-species-pair (cutoff + skin)^2 of a pair-prior list, 0 = pair does not interact*/);
 void launch_compact(Launcher L, const SysDev& sys, int B, const double* q /*[B][3][n]*/, const int* img,
                     const VerletList& vl, double rc2_single, const double* pair_rc2 /*or null*/, CompactList& cl, int* flags,
                     float rc_records = 0.f /* > 0: also write cl.recs with the cutoff function of this radius */);

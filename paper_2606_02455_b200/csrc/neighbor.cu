@@ -123,7 +123,8 @@ constexpr int kVlMaxRow = 512;
 __global__ void __launch_bounds__(kVlWarps * 32)
 k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int* __restrict__ img,
                const int* __restrict__ atom_cell, const int* __restrict__ cell_start, const int* __restrict__ cell_atoms,
-               double rcs2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags)
+               double rcs2, int cap, int* __restrict__ count, uint32_t* __restrict__ keys, int* flags,
+               const int* __restrict__ species, int ns, const double* __restrict__ pair_rcs2 /*or null: [ns][ns] (r_c(s_i, s_j) + skin)^2, 0 = no pair term*/)
 {
     pdl_sync();
     __shared__ uint32_t rows[kVlWarps][kVlMaxRow];
@@ -135,6 +136,7 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
     const int ci = atom_cell[i];
     const int cz = ci % g.nc[2], cy = (ci / g.nc[2]) % g.nc[1], cx = ci / (g.nc[2] * g.nc[1]);
     int iix, iiy, iiz; img_unpack(img[i], iix, iiy, iiz);
+    const double* const lim_row = pair_rcs2 ? pair_rcs2 + species[i] * ns : nullptr;
     const int lox = g.nc[0] >= 3 ? -1 : 0, hix = g.nc[0] >= 3 ? 1 : g.nc[0] - 1;   // < 3 cells: visit each cell once (R10)
     const int loy = g.nc[1] >= 3 ? -1 : 0, hiy = g.nc[1] >= 3 ? 1 : g.nc[1] - 1;
     const int loz = g.nc[2] >= 3 ? -1 : 0, hiz = g.nc[2] >= 3 ? 1 : g.nc[2] - 1;
@@ -152,7 +154,7 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
                 if (j != i) {
                     int sx, sy, sz;
                     const double r2 = pair_r2(box, q, n, i, j, sx, sy, sz);
-                    if (r2 < rcs2) {
+                    if (r2 < (lim_row ? lim_row[species[j]] : rcs2)) {   // pair-prior list: candidates of the species pairs that interact only
                         int jx, jy, jz; img_unpack(img[j], jx, jy, jz);
                         const int wx = sx - iix + jx, wy = sy - iiy + jy, wz = sz - iiz + jz;   // s_w = s - img_i + img_j
                         keep = true;
@@ -291,7 +293,7 @@ void launch_pack_ref(Launcher L, const SysDev& sys, const double* qref, int* img
 }
 
 void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const double* qref, const int* img,
-                         double rc_skin, VerletList& vl, int* flags)
+                         double rc_skin, VerletList& vl, int* flags, const double* pair_rcs2)
 {
     const int n = sys.n;
     const int pid = prof_begin(L, PROF_NBR);
@@ -301,7 +303,8 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
     launch_pdl(L, k_cell_scan, dim3(1), dim3(1024), 0, g.ncell, g.cell_count, g.cell_start, g.cell_cursor); LSD_COUNT(L);
     launch_pdl(L, k_cell_fill, dim3((n + 255) / 256), dim3(256), 0, n, g.atom_cell, g.cell_cursor, g.cell_atoms); LSD_COUNT(L);
     launch_pdl(L, k_build_verlet, dim3((n + kVlWarps - 1) / kVlWarps), dim3(kVlWarps * 32), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_start,
-                                                                             g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags);
+                                                                             g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags,
+                                                                             sys.species, sys.ns, pair_rcs2);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
