@@ -116,6 +116,7 @@ struct MlipWork {                    // activations of one batched evaluation (k
     uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
     uint32_t* ym16 = nullptr;        // width 128 only: rows of (y, mbar) bf16 pairs gathered by the backward tcgen05 kernel
     double* e_atom = nullptr;        // [bmax*n]
+    int y0_rows = 0;                 // one-block networks: rows of y[0] / y16[0] (species-only) already written
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline numbers)

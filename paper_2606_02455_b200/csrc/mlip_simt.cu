@@ -246,6 +246,66 @@ k_readout(int total, float alpha, const float* __restrict__ x, const float* __re
     }
 }
 
+// ------------------------------------------------------------------------------------------------ one-block networks (the drafts)
+// With T = 1 everything between the two edge kernels is local to an atom: h = W_o1 m; x = Emb + W_o2 ssp(h); readout
+// z = W_r1 x, e = alpha w_r2 . ssp(z); xbar = alpha W_r1^T (logistic(z) . w_r2); hbar = logistic(h) . W_o2^T xbar; mbar = W_o1^T hbar
+// (M5, M6, M9).  One warp per atom, lane = channel (F = 32), the six small matrices resident in shared memory: one launch
+// instead of k_dense<DENSE_OUT>, k_readout and k_dense<BWD_OUT>, and nothing but mbar leaves the kernel.
+// out[lane] = sum_k in[k] W[k][lane], in[k] held by lane k; four interleaved chains, summed in a fixed order
+__device__ __forceinline__ float warp_matvec32(float in, const float* __restrict__ W, int lane, int K = 32)
+{
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 8
+    for (int k = 0; k < K; k += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc[u] = fmaf(__shfl_sync(0xffffffffu, in, k + u), W[(k + u) * 32 + lane], acc[u]);
+    }
+    return (acc[0] + acc[1]) + (acc[2] + acc[3]);
+}
+
+__global__ void __launch_bounds__(512)
+k_atom_chain1(int total, int n, const int* __restrict__ species, float alpha, const float* __restrict__ m, const float* __restrict__ emb,
+              const float* __restrict__ Wo1T, const float* __restrict__ Wo2T, const float* __restrict__ Wo2, const float* __restrict__ Wo1,
+              const float* __restrict__ Wr1, const float* __restrict__ wr2, float* __restrict__ mbar, uint16_t* __restrict__ mbar16,
+              const uint16_t* __restrict__ y16, uint32_t* __restrict__ ympair, double* __restrict__ e_atom)
+{
+    constexpr int F = 32, H = F / 2;
+    __shared__ __align__(16) float W[4 * F * F + H * F + H];
+    float* const sWo1T = W; float* const sWo2T = W + F * F; float* const sWo2 = W + 2 * F * F; float* const sWo1 = W + 3 * F * F;
+    float* const sWr1 = W + 4 * F * F; float* const sw2 = sWr1 + H * F;
+    for (int i = threadIdx.x; i < F * F; i += blockDim.x) { sWo1T[i] = Wo1T[i]; sWo2T[i] = Wo2T[i]; sWo2[i] = Wo2[i]; sWo1[i] = Wo1[i]; }
+    for (int i = threadIdx.x; i < H * F; i += blockDim.x) sWr1[i] = Wr1[i];
+    if (threadIdx.x < H) sw2[threadIdx.x] = wr2[threadIdx.x];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int g = blockIdx.x * nw + warp; g < total; g += gridDim.x * nw) {
+        const float h = warp_matvec32(m[(size_t)g * F + lane], sWo1T, lane);
+        const float x = emb[species[g % n] * F + lane] + warp_matvec32(ssp(h), sWo2T, lane);
+        float z0 = 0.f, z1 = 0.f;
+#pragma unroll 8
+        for (int f = 0; f < F; f += 2) {
+            const float x0 = __shfl_sync(0xffffffffu, x, f), x1 = __shfl_sync(0xffffffffu, x, f + 1);
+            if (lane < H) { z0 = fmaf(sWr1[lane * F + f], x0, z0); z1 = fmaf(sWr1[lane * F + f + 1], x1, z1); }
+        }
+        const float z = z0 + z1;
+        float e = lane < H ? sw2[lane] * ssp(z) : 0.f;
+        const float s = lane < H ? logistic(z) * sw2[lane] : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        const float xb = alpha * warp_matvec32(s, sWr1, lane, H);
+        const float hb = logistic(h) * warp_matvec32(xb, sWo2, lane);
+        const float mb = warp_matvec32(hb, sWo1, lane);
+        const size_t o = (size_t)g * F + lane;
+        if (mbar) mbar[o] = mb;
+        if (mbar16) { const __nv_bfloat16 b = __float2bfloat16_rn(mb); mbar16[o] = *reinterpret_cast<const uint16_t*>(&b); }
+        if (ympair) {                                  // pair rows of the edges-as-rows backward kernel (see k_dense)
+            const float nxt = __shfl_down_sync(0xffffffffu, mb, 1);
+            if ((lane & 1) == 0) *reinterpret_cast<uint2*>(ympair + o) = make_uint2(*reinterpret_cast<const uint32_t*>(y16 + o), bf16x2(mb, nxt));
+        }
+        if (lane == 0 && e_atom) e_atom[g] = (double)(alpha * e);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ continuous-filter convolution
 
 template <int F, bool BWD>
@@ -391,7 +451,16 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
     const int kThreads = kWarps * 32;
     const int grid_tiles = std::max(1, std::min(sms, (total + kWarps * 8 - 1) / (kWarps * 8)));
     const int grid_atoms = std::max(1, std::min(sms, (total + kWarps - 1) / kWarps));
-    k_embed_y<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, net.ytab0, w.x, w.y[0], use_tc ? w.y16[0] : nullptr); LSD_COUNT(L);
+    // one-block width-32 network of a small system: k_atom_chain1 between the two edge kernels (three launches less per evaluation;
+    // cfg4: draft network 2.32 -> 1.76 ms per window).  Large systems keep the tiled kernels, which are faster there (cfg5: 6.1 vs
+    // 6.5 ms).  The choice depends on the atoms of ONE state, never on the batch: the same network gives the same bits alone and batched.
+    const bool chain1 = F == 32 && net.T == 1 && sys.n <= 16384;
+    // y of the first block depends on the species only (M4, M5): for a one-block network nothing else is read from the embedding
+    // kernel's outputs, so its rows are written once per context (and again when a larger batch needs more of them)
+    if (!chain1 || w.y0_rows < total) {
+        k_embed_y<<<(int)(((size_t)total * F + 255) / 256), 256, 0, L.s>>>(total, sys.n, F, sys.species, net.emb, net.ytab0, w.x, w.y[0], use_tc ? w.y16[0] : nullptr); LSD_COUNT(L);
+        if (chain1) w.y0_rows = total;
+    }
     EdgeArgs ea{};
     ea.total = total; ea.n = sys.n; ea.cap = cl.cap; ea.count = cl.count; ea.keys = cl.keys; ea.recs = cl.recs; ea.rec_zero = cl.rec_zero;
     ea.rc = net.rc; ea.inv_rc = 1.f / net.rc; ea.delta = net.rc / (float)(net.R - 1); ea.inv_delta2 = 1.f / (ea.delta * ea.delta);
@@ -410,19 +479,31 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
+        if (chain1) continue;
         pid = prof_begin(L, PROF_DENSE);
         k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x, nullptr); LSD_COUNT(L);
         prof_end(L, pid);
     }
-    int pidr = prof_begin(L, PROF_DENSE);
-    k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(kWarps), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
-    prof_end(L, pidr);
+    const bool pairs = use_tc && narrow_rows;                   // (y, mbar) pair rows for k_edge_rows
+    if (chain1) {
+        const int pidc = prof_begin(L, PROF_DENSE);
+        const int cw = 16, grid_c = std::max(1, std::min(sms * 2, (total + cw - 1) / cw));
+        k_atom_chain1<<<grid_c, cw * 32, 0, L.s>>>(total, sys.n, sys.species, net.alpha, w.m, net.emb, net.Wo1T[0], net.Wo2T[0], net.Wo2[0], net.Wo1[0], net.Wr1, net.wr2,
+                                                   w.mbar, use_tc && !pairs ? w.mbar16 : nullptr, pairs ? w.y16[0] : nullptr, pairs ? w.ym16 : nullptr, e_atom); LSD_COUNT(L);
+        prof_end(L, pidc);
+    } else {
+        int pidr = prof_begin(L, PROF_DENSE);
+        k_readout<F><<<grid_atoms, kThreads, smem_readout<F>(kWarps), L.s>>>(total, net.alpha, w.x, net.Wr1, net.wr2, w.xbar, e_atom); LSD_COUNT(L);
+        prof_end(L, pidr);
+    }
     for (int t = net.T - 1; t >= 0; --t) {
-        int pid = prof_begin(L, PROF_DENSE);
-        const bool pairs = use_tc && narrow_rows;               // (y, mbar) pair rows for k_edge_rows
+        int pid = -1;
+        if (!chain1) {
+        pid = prof_begin(L, PROF_DENSE);
         k_dense<F, BWD_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.xbar, net.Wo2[t], net.Wo1[t], w.h[t], w.mbar, use_tc && !pairs ? w.mbar16 : nullptr,
                                                                                  pairs ? w.y16[t] : nullptr, pairs ? w.ym16 : nullptr); LSD_COUNT(L);
         prof_end(L, pid);
+        }
         ea.Wf1 = net.Wf1T[t]; ea.Wf2 = net.Wf2T[t]; ea.y = w.y[t]; ea.m_out = nullptr; ea.mbar = w.mbar; ea.ybar = t > 0 ? w.ybar : nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
         if (use_tc) {
