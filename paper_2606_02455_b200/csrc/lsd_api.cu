@@ -52,6 +52,7 @@ struct lsd_ctx {
     int verify_idx = 0, pending = 0, last_slot = -1, last_K = 0, last_l = 0, last_nc = 0, transported = 0;
     MlipWork work[2];
     CompactList cl_mlip[2], cl_pair[2];
+    bool pair_is_mlip[2] = {false, false};                   // every pair term has the network's cutoff: the network's per-state list serves the prior too
     const int* cl_img[2] = {nullptr, nullptr};
     int bmax[2] = {1, 1};
     CellGrid grid;
@@ -374,7 +375,14 @@ lsd_status setup_lists_impl(lsd_ctx* ctx)
     else if (ctx->cap_pair) TRY(alloc_verlet(ctx, ctx->vl_eval_pair, ctx->cap_pair, ctx->rc_pair_max));
     for (int w = 0; w < 2; ++w) {
         if (ctx->pot[w].mlip.F > 0) TRY(alloc_compact(ctx, ctx->cl_mlip[w], ctx->cap_mlip, ctx->bmax[w], true));
-        if (ctx->pot[w].pair_rcmax > 0) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w], false));
+        {   // the same directed edge set for the prior and the network: every species pair has a pair term, all with the network's cutoff
+            const PotDev& pd = ctx->pot[w];
+            bool same = pd.mlip.F > 0 && pd.pair_rcmax > 0;
+            const double rc2 = (double)pd.mlip.rc * (double)pd.mlip.rc;
+            for (double v : pd.pair_rc2_host) same = same && v == rc2;
+            ctx->pair_is_mlip[w] = same;
+        }
+        if (ctx->pot[w].pair_rcmax > 0 && !ctx->pair_is_mlip[w]) TRY(alloc_compact(ctx, ctx->cl_pair[w], ctx->cap_pair, ctx->bmax[w], false));
     }
     return LSD_OK;
 }
@@ -421,14 +429,19 @@ void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, co
     L.draft = which == LSD_DRAFT;
     ctx->cl_img[which] = img;
     CompactList* pl = nullptr;
-    if (pot.pair_rcmax > 0) {
+    const bool one_list = ctx->pair_is_mlip[which];              // cfg5: Morse and network both 6 A: one per-state list, one launch less
+    if (pot.mlip.F > 0 && one_list) {
+        const double rc = (double)pot.mlip.rc;
+        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
+        pl = &ctx->cl_mlip[which];
+    } else if (pot.pair_rcmax > 0) {
         launch_compact(L, ctx->sys, B, q, img, vp, 0.0, pot.pair_rc2, ctx->cl_pair[which], flags);
         pl = &ctx->cl_pair[which];
     }
     launch_prior_forces(L, ctx->sys, pot, B, q, img, pl, F);
     if (pot.mlip.F > 0) {
         const double rc = (double)pot.mlip.rc;
-        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
+        if (!one_list) launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
         if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(pot.mlip))
             mlip_forward_backward_bf16tc(L, ctx->sys, pot.mlip, ctx->work[which], B, q, img, ctx->cl_mlip[which], F, e_atom);
         else
@@ -1069,7 +1082,7 @@ lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const 
 lsd_status lsd_get_edge_count(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t n_states, int64_t* total)
 {
     if (!ctx || !total || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
-    const CompactList& cl = kind == 0 ? ctx->cl_mlip[which] : ctx->cl_pair[which];
+    const CompactList& cl = (kind == 0 || ctx->pair_is_mlip[which]) ? ctx->cl_mlip[which] : ctx->cl_pair[which];
     *total = 0;
     if (!cl.count) return LSD_OK;
     if (n_states < 1 || n_states > cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "n_states out of range");
@@ -1114,7 +1127,7 @@ lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t 
                              int8_t* shifts, int64_t* n_edges)
 {
     if (!ctx || !start || !n_edges || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
-    const CompactList& cl = kind == 0 ? ctx->cl_mlip[which] : ctx->cl_pair[which];
+    const CompactList& cl = (kind == 0 || ctx->pair_is_mlip[which]) ? ctx->cl_mlip[which] : ctx->cl_pair[which];
     if (!cl.count || !ctx->cl_img[which]) return fail(ctx, LSD_ERR_STATE, "this potential has no such list (or no evaluation has run yet)");
     if (ctx->tiny && which == LSD_DRAFT) return fail(ctx, LSD_ERR_STATE, "the one-kernel draft rollout of a tiny system keeps its neighbour rows on chip");
     if (b < 0 || b >= cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "state index out of range");
