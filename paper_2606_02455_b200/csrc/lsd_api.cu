@@ -27,6 +27,8 @@ struct WindowSlot {
     std::map<int, GraphEntry> g_roll, g_verify, g_transport, g_plain; // by K (g_plain: by 2 K + which)
     double *qstart = nullptr, *pstart = nullptr;             // [3][n]
     double *qhalf = nullptr, *Ft = nullptr, *yq = nullptr, *yp = nullptr;   // [kmax][3][n]
+    double* Fprior = nullptr;                                // [kmax][3][n] prior part of the draft forces (kept when the target has the same prior)
+    int prior_valid = 0;
     int* img = nullptr;                                      // [n] images of the reference (start) state
     VerletList vl_mlip, vl_pair;
     int* flags = nullptr;
@@ -76,6 +78,7 @@ struct lsd_ctx {
     int ec = 0;                                              // speculative error correction (Alg. 3) on / off
     double* dF = nullptr;                                    // [3][n] EC cache: F - F~(bare) of the last committed step
     bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
+    bool same_prior = false;                                 // draft and target share the classical prior: the verification re-uses the rollout's prior forces
     bool tiny = false;                                       // draft rollout as one kernel launch (tiny_rollout.cu; LSD_TINY=0 disables)
     std::vector<cudaStream_t> busy;                          // caller streams that may still hold work of this context (lsd_get_state / lsd_set_state wait for these only)
     Prof prof;
@@ -396,6 +399,7 @@ lsd_status alloc_slot(lsd_ctx* ctx, int s)
     if (w.qstart) return LSD_OK;
     TRY(dalloc(ctx, &w.qstart, n3)); TRY(dalloc(ctx, &w.pstart, n3));
     TRY(dalloc(ctx, &w.qhalf, n3 * kmax)); TRY(dalloc(ctx, &w.Ft, n3 * kmax)); TRY(dalloc(ctx, &w.yq, n3 * kmax)); TRY(dalloc(ctx, &w.yp, n3 * kmax));
+    if (ctx->same_prior) TRY(dalloc(ctx, &w.Fprior, n3 * kmax));
     TRY(dalloc(ctx, &w.img, ctx->sys.n)); TRY(dalloc(ctx, &w.flags, 1)); TRY(dalloc(ctx, &w.n0_dev, 1));
     TRY(dalloc(ctx, &w.dF, n3)); CK(cudaMemset(w.dF, 0, n3 * sizeof(double)));
     CK(cudaEventCreateWithFlags(&w.ev_drafted, cudaEventDisableTiming));
@@ -422,26 +426,35 @@ void build_lists(lsd_ctx* ctx, Launcher L, const double* qref, int* img, VerletL
 }
 
 // One batched force evaluation of potential `which` on B <= bmax[which] states (a0 / a2).
+// prior_out: also keep the prior part of the forces; prior_in: the prior part is known (same positions, same prior, computed by the
+// same batch-invariant kernel: identical bits), only the network is evaluated
 void eval_forces(lsd_ctx* ctx, Launcher L, int which, int B, const double* q, const int* img, const VerletList& vm,
-                 const VerletList& vp, double* F, int* flags, double* e_atom)
+                 const VerletList& vp, double* F, int* flags, double* e_atom, double* prior_out = nullptr, const double* prior_in = nullptr)
 {
     PotDev& pot = ctx->pot[which];
     L.draft = which == LSD_DRAFT;
     ctx->cl_img[which] = img;
     CompactList* pl = nullptr;
     const bool one_list = ctx->pair_is_mlip[which];              // cfg5: Morse and network both 6 A: one per-state list, one launch less
-    if (pot.mlip.F > 0 && one_list) {
-        const double rc = (double)pot.mlip.rc;
-        launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
-        pl = &ctx->cl_mlip[which];
-    } else if (pot.pair_rcmax > 0) {
-        launch_compact(L, ctx->sys, B, q, img, vp, 0.0, pot.pair_rc2, ctx->cl_pair[which], flags);
-        pl = &ctx->cl_pair[which];
+    const size_t fbytes = (size_t)B * 3 * ctx->sys.n * sizeof(double);
+    bool mlip_list_done = false;
+    if (prior_in) cudaMemcpyAsync(F, prior_in, fbytes, cudaMemcpyDeviceToDevice, L.s);
+    else {
+        if (pot.mlip.F > 0 && one_list) {
+            const double rc = (double)pot.mlip.rc;
+            launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
+            pl = &ctx->cl_mlip[which];
+            mlip_list_done = true;
+        } else if (pot.pair_rcmax > 0) {
+            launch_compact(L, ctx->sys, B, q, img, vp, 0.0, pot.pair_rc2, ctx->cl_pair[which], flags);
+            pl = &ctx->cl_pair[which];
+        }
+        launch_prior_forces(L, ctx->sys, pot, B, q, img, pl, F);
+        if (prior_out) cudaMemcpyAsync(prior_out, F, fbytes, cudaMemcpyDeviceToDevice, L.s);
     }
-    launch_prior_forces(L, ctx->sys, pot, B, q, img, pl, F);
     if (pot.mlip.F > 0) {
         const double rc = (double)pot.mlip.rc;
-        if (!one_list) launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
+        if (!mlip_list_done) launch_compact(L, ctx->sys, B, q, img, vm, rc * rc, nullptr, ctx->cl_mlip[which], flags, pot.mlip.rc);
         if (ctx->cfg.precision == LSD_BF16_TC && mlip_tc_supported(pot.mlip))
             mlip_forward_backward_bf16tc(L, ctx->sys, pot.mlip, ctx->work[which], B, q, img, ctx->cl_mlip[which], F, e_atom);
         else
@@ -484,7 +497,8 @@ lsd_status rollout_body(lsd_ctx* ctx, WindowSlot& w, int K, int which, void* str
         const double* pp = j == 1 ? w.pstart : w.yp + n3 * (j - 2);
         double* qh = w.qhalf + n3 * (j - 1);
         if (j == 1) launch_half_a(Lg, n, w.qstart, w.pstart, ctx->sys.mass, ctx->hdt, qh, w.qstart, sh2, w.flags);
-        eval_forces(ctx, Lg, which, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr);
+        eval_forces(ctx, Lg, which, 1, qh, w.img, w.vl_mlip, w.vl_pair, w.Ft + n3 * (j - 1), w.flags, nullptr,
+                    (ctx->same_prior && which == LSD_DRAFT) ? w.Fprior + n3 * (j - 1) : nullptr);
         launch_bob_a(Lg, n, ctx->cfg.seed, w.n0_dev, (uint64_t)j, pp, w.Ft + n3 * (j - 1), qh, ctx->sys.mass, ctx->sys.sigma,
                      ctx->c1, ctx->b, ctx->hdt, w.yq + n3 * (j - 1), w.yp + n3 * (j - 1), ec ? w.dF : nullptr,
                      j < K ? w.qhalf + n3 * j : nullptr, w.qstart, sh2, w.flags);       // + the first A(1/2) of step j + 1
@@ -601,6 +615,9 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
         if (same && draft->mlip.width > 0)
             same = draft->mlip.n_blocks == target->mlip.n_blocks && draft->mlip.cutoff == target->mlip.cutoff && draft->mlip.energy_scale == target->mlip.energy_scale &&
                    std::memcmp(draft->mlip.weights, target->mlip.weights, sizeof(double) * n_weights(draft->mlip)) == 0;
+        const char* pv = getenv("LSD_PRIOR_REUSE");
+        ctx->same_prior = !same && !(pv && pv[0] == '0') && draft->use_bonded == target->use_bonded &&
+                          std::memcmp(draft->pair, target->pair, sizeof(double) * (size_t)sys->n_species * sys->n_species * LSD_PAIR_COLS) == 0;
         const char* tv = getenv("LSD_TINY");
         ctx->tiny = !same && !(tv && tv[0] == '0') && tiny_rollout_supported(ctx->sys, ctx->pot[LSD_DRAFT]);
     }
@@ -698,6 +715,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
     ctx->cl_img[LSD_DRAFT] = w.img;                                           // (set by eval_forces only when the body runs)
     CK(cudaEventRecord(w.ev_drafted, st));
     w.K = K; w.drafted = 1; w.verified = 0;
+    w.prior_valid = ctx->same_prior && !ctx->tiny;               // (the one-kernel rollout keeps its prior forces on chip)
     ctx->pending++;
     CK(cudaGetLastError());
     return LSD_OK;
@@ -713,7 +731,8 @@ lsd_status lsd_verify_window(lsd_ctx* ctx, int32_t K, void* stream)
     note_stream(ctx, st);
     CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
     TRY(run_graphed(ctx, st, w.g_verify[K], [&]() -> lsd_status {
-        eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr);
+        eval_forces(ctx, mk(ctx, stream), LSD_TARGET, K, w.qhalf, w.img, w.vl_mlip, w.vl_pair, ctx->Fg, w.flags, nullptr, nullptr,
+                    (ctx->same_prior && w.prior_valid) ? w.Fprior : nullptr);
         return LSD_OK;
     }));
     ctx->cl_img[LSD_TARGET] = w.img;
