@@ -570,13 +570,13 @@ def main():
             if name == args.workload and (precn or "") == (args.precision or ("bf16" if m["dtype"] == "bf16" else "fp32" if m["dtype"] == "f32" else "")):
                 r = m
             else:
-                r = measure_workload(env, name, precn, SIDE_STEPS, 3, full=False)
+                r = measure_workload(env, name, precn, SIDE_STEPS * (5 if name in ("cfg1", "cfg2") else 1), 3, full=False)   # (0.1-0.5 ms windows: more of them)
             rf = r["roofline"]
             side[key] = dict(ms_per_step=r["ms_per_step"], value=r["value"], unit=UNIT, dtype=r["dtype"], committed_md_steps_per_s=r["committed_md_steps_per_s"],
                              committed_per_window=r["committed_per_window"], e2e_value=r["e2e"]["value"], gpu_launches=r["gpu_launches"],
                              roofline=dict(bound=rf["bound"], frac=rf["frac"], achieved=rf["achieved"], peak=rf["peak"], unit=rf["unit"], kernel=rf["kernel"],
                                            three_term=rf.get("a2_three_term")),
-                             clocks=r["clocks"], steps=SIDE_STEPS if r is not m else args.steps)
+                             clocks=r["clocks"], steps=r["windows_timed"])
         variant = acceptance_variant(env, args.workload, args.precision)
         ring = async_depth_block(env)
         # two design measurements DESIGN.md cites (section 4.1, section 7): tensor-memory bandwidth of an SM, and the second delivery of a
