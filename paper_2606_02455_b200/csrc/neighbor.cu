@@ -133,7 +133,7 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
     if (i >= n) return;
     uint32_t* row = rows[warp];
     int cnt = 0;
-    const int ci = atom_cell[i];
+    const int ci = atom_cell ? atom_cell[i] : 0;            // (no cell tables: the whole system is one cell, launch_build_verlet)
     const int cz = ci % g.nc[2], cy = (ci / g.nc[2]) % g.nc[1], cx = ci / (g.nc[2] * g.nc[1]);
     int iix, iiy, iiz; img_unpack(img[i], iix, iiy, iiz);
     const double* const lim_row = pair_rcs2 ? pair_rcs2 + species[i] * ns : nullptr;
@@ -145,12 +145,12 @@ k_build_verlet(int n, BoxC box, GridC g, const double* __restrict__ q, const int
         const int oy = g.nc[1] >= 3 ? (cy + dy + g.nc[1]) % g.nc[1] : dy;
         const int oz = g.nc[2] >= 3 ? (cz + dz + g.nc[2]) % g.nc[2] : dz;
         const int c = (ox * g.nc[1] + oy) * g.nc[2] + oz;
-        const int beg = cell_start[c], end = cell_start[c + 1];
+        const int beg = cell_start ? cell_start[c] : 0, end = cell_start ? cell_start[c + 1] : n;
         for (int t0 = beg; t0 < end; t0 += 32) {
             const int t = t0 + lane;
             bool keep = false; uint32_t key = 0;
             if (t < end) {
-                const int j = cell_atoms[t];
+                const int j = cell_atoms ? cell_atoms[t] : t;
                 if (j != i) {
                     int sx, sy, sz;
                     const double r2 = pair_r2(box, q, n, i, j, sx, sy, sz);
@@ -298,13 +298,16 @@ void launch_build_verlet(Launcher L, const SysDev& sys, CellGrid& g, const doubl
     const int n = sys.n;
     const int pid = prof_begin(L, PROF_NBR);
     GridC gc; gc.nc[0] = g.nc[0]; gc.nc[1] = g.nc[1]; gc.nc[2] = g.nc[2];
-    cudaMemsetAsync(g.cell_count, 0, sizeof(int) * g.ncell, L.s);
-    launch_pdl(L, k_cell_count, dim3((n + 255) / 256), dim3(256), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_count); LSD_COUNT(L);
-    launch_pdl(L, k_cell_scan, dim3(1), dim3(1024), 0, g.ncell, g.cell_count, g.cell_start, g.cell_cursor); LSD_COUNT(L);
-    launch_pdl(L, k_cell_fill, dim3((n + 255) / 256), dim3(256), 0, n, g.atom_cell, g.cell_cursor, g.cell_atoms); LSD_COUNT(L);
-    launch_pdl(L, k_build_verlet, dim3((n + kVlWarps - 1) / kVlWarps), dim3(kVlWarps * 32), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_start,
-                                                                             g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags,
-                                                                             sys.species, sys.ns, pair_rcs2);
+    const bool one_cell = g.ncell == 1;                      // small boxes / vacuum: every atom is a candidate, no binning (three launches less)
+    if (!one_cell) {
+        cudaMemsetAsync(g.cell_count, 0, sizeof(int) * g.ncell, L.s);
+        launch_pdl(L, k_cell_count, dim3((n + 255) / 256), dim3(256), 0, n, make_box(sys), gc, qref, img, g.atom_cell, g.cell_count); LSD_COUNT(L);
+        launch_pdl(L, k_cell_scan, dim3(1), dim3(1024), 0, g.ncell, g.cell_count, g.cell_start, g.cell_cursor); LSD_COUNT(L);
+        launch_pdl(L, k_cell_fill, dim3((n + 255) / 256), dim3(256), 0, n, g.atom_cell, g.cell_cursor, g.cell_atoms); LSD_COUNT(L);
+    }
+    launch_pdl(L, k_build_verlet, dim3((n + kVlWarps - 1) / kVlWarps), dim3(kVlWarps * 32), 0, n, make_box(sys), gc, qref, img,
+               one_cell ? (const int*)nullptr : (const int*)g.atom_cell, one_cell ? (const int*)nullptr : (const int*)g.cell_start,
+               one_cell ? (const int*)nullptr : (const int*)g.cell_atoms, rc_skin * rc_skin, vl.cap, vl.count, vl.keys, flags, sys.species, sys.ns, pair_rcs2);
     LSD_COUNT(L);
     prof_end(L, pid);
 }
