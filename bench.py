@@ -38,7 +38,11 @@ UNIT = "atom-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from one `ncu --set full` capture of this
 # command (per workload and arithmetic type; null where no capture is committed).  Not measured by this run: a run under a
 # profiler is never a bench run; `roofline.traffic_source` names the committed capture the figure comes from.
-NCU_TRAFFIC = {("cfg5", "bf16"): (1.652183e9 + 0.145999872e9, "profiles/r2_edge_rows_bwd_cfg5.md (k_edge_rows<1,2>)")}
+NCU_TRAFFIC = {("cfg5", "bf16"): (1.6515e9 + 0.1405e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)"),
+               ("cfg4", "bf16"): (0.2073e9 + 0.0250e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)"),
+               ("cfg4", "f32"): (0.2750e9 + 0.0565e9, "profiles/r2_traffic.md (k_edge<128,bwd>)"),
+               ("cfg3", "bf16"): (0.0572e9 + 0.0004e9, "profiles/r2_traffic.md (k_edge_rows<64,1,2>)"),
+               ("cfg3", "f32"): (0.0635e9 + 0.0002e9, "profiles/r2_traffic.md (k_edge<64,bwd>)")}
 
 # the workloads of BASELINE.json with the arithmetic types it lists for them (north_star: "report throughput on the five synthetic
 # workloads"): the default run times --workload in full and the others for a few windows each (`all_workloads`)
