@@ -35,7 +35,7 @@ sys.path.insert(0, ROOT)
 METRIC = "batched force-eval atom-steps/s (whole verified window; accepted target-exact MD steps/s beside it)"
 UNIT = "atom-steps/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from one `ncu --set full` capture of this
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from one ncu capture of this
 # command (per workload and arithmetic type; null where no capture is committed).  Not measured by this run: a run under a
 # profiler is never a bench run; `roofline.traffic_source` names the committed capture the figure comes from.
 NCU_TRAFFIC = {("cfg5", "bf16"): (1.6515e9 + 0.1405e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)"),
