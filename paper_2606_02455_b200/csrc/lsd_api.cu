@@ -80,6 +80,9 @@ struct lsd_ctx {
     bool use_graphs = true;                                  // LSD_GRAPHS=0 disables graph replay
     bool same_prior = false;                                 // draft and target share the classical prior: the verification re-uses the rollout's prior forces
     bool tiny = false;                                       // draft rollout as one kernel launch (tiny_rollout.cu; LSD_TINY=0 disables)
+    double* state_host = nullptr;                            // pinned [2][3][n] staging of lsd_set_state / lsd_get_state (small systems: one copy each way, no wait on upload)
+    cudaEvent_t ev_state = nullptr;                          // the staged upload has reached q, p
+    bool state_in_flight = false;
     std::vector<cudaStream_t> busy;                          // caller streams that may still hold work of this context (lsd_get_state / lsd_set_state wait for these only)
     Prof prof;
     lsd_stats stats{};
@@ -128,6 +131,7 @@ lsd_status sync_pending(lsd_ctx* ctx)
 {
     for (cudaStream_t st : ctx->busy) CK(cudaStreamSynchronize(st));
     ctx->busy.clear();
+    ctx->state_in_flight = false;
     return LSD_OK;
 }
 
@@ -544,6 +548,8 @@ void lsd_destroy(lsd_ctx* ctx)
     for (cudaEvent_t e : ctx->prof.ev) cudaEventDestroy(e);
     if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->result_host) cudaFreeHost(ctx->result_host);
+    if (ctx->state_host) cudaFreeHost(ctx->state_host);
+    if (ctx->ev_state) cudaEventDestroy(ctx->ev_state);
     delete ctx;
 }
 
@@ -624,8 +630,13 @@ static lsd_status init_impl(lsd_ctx* ctx, const lsd_config* cfg, const lsd_syste
     ctx->bmax[LSD_DRAFT] = 1; ctx->bmax[LSD_TARGET] = kmax;
 
     const size_t n3 = (size_t)3 * n;
-    TRY(upload(ctx, &ctx->q, q0, n3));
-    TRY(dalloc(ctx, &ctx->p, n3));
+    TRY(dalloc(ctx, &ctx->q, 2 * n3));                       // q and p are one allocation: a state moves with one copy
+    ctx->p = ctx->q + n3;
+    CK(cudaMemcpy(ctx->q, q0, n3 * sizeof(double), cudaMemcpyHostToDevice));
+    if (n3 * 2 * sizeof(double) <= (size_t)512 * 1024) {
+        CK(cudaMallocHost(&ctx->state_host, 2 * n3 * sizeof(double)));
+        CK(cudaEventCreateWithFlags(&ctx->ev_state, cudaEventDisableTiming));
+    }
     if (p0) CK(cudaMemcpy(ctx->p, p0, n3 * sizeof(double), cudaMemcpyHostToDevice));
     else launch_initial_momenta(mk(ctx, nullptr), n, cfg->seed, S.mass, ctx->kT, ctx->p);
     TRY(setup_lists(ctx));
@@ -694,6 +705,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
     cudaStream_t st = (cudaStream_t)stream;
     Launcher L = mk(ctx, stream);
     note_stream(ctx, st);
+    if (ctx->state_in_flight) CK(cudaStreamWaitEvent(st, ctx->ev_state, 0));  // a staged lsd_set_state upload
     if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));          // a discarded rollout into this slot may still run
     if (ctx->pending == 0) {
         // flushed speculative rollouts may still run on another stream: they share the draft's work buffers
@@ -893,6 +905,7 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
     if (ctx->pending) return fail(ctx, LSD_ERR_STATE, "a drafted window is pending");
     cudaStream_t st = (cudaStream_t)stream;
     note_stream(ctx, st);
+    if (ctx->state_in_flight) CK(cudaStreamWaitEvent(st, ctx->ev_state, 0));
     const size_t n3 = (size_t)3 * ctx->sys.n;
     WindowSlot& w = ctx->slot[ctx->verify_idx];
     int list_retries = 0;
@@ -930,6 +943,14 @@ lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int3
     if (!ctx) return LSD_ERR_INVALID_ARG;
     TRY(sync_pending(ctx));
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
+    if (where == LSD_HOST && ctx->state_host && q && p) {     // small system: one device-to-host copy of (q, p) through the pinned staging
+        CK(cudaMemcpyAsync(ctx->state_host, ctx->q, 2 * bytes, cudaMemcpyDeviceToHost, ctx->side));
+        CK(cudaStreamSynchronize(ctx->side));
+        std::memcpy(q, ctx->state_host, bytes);
+        std::memcpy(p, ctx->state_host + 3 * ctx->sys.n, bytes);
+        if (step) *step = ctx->step;
+        return LSD_OK;
+    }
     const cudaMemcpyKind kind = where == LSD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     if (q) CK(cudaMemcpyAsync(q, ctx->q, bytes, kind, ctx->side));
     if (p) CK(cudaMemcpyAsync(p, ctx->p, bytes, kind, ctx->side));
@@ -943,6 +964,20 @@ lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t
     if (!ctx || !q || !p) return LSD_ERR_INVALID_ARG;
     TRY(sync_pending(ctx));
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
+    if (where == LSD_HOST && ctx->state_host) {
+        // small system: the caller's buffers are copied into the pinned staging (they are free again on return), ONE upload is
+        // enqueued on the internal stream and the call does not wait for it: whatever reads q, p next waits for ev_state
+        std::memcpy(ctx->state_host, q, bytes);
+        std::memcpy(ctx->state_host + 3 * ctx->sys.n, p, bytes);
+        CK(cudaMemcpyAsync(ctx->q, ctx->state_host, 2 * bytes, cudaMemcpyHostToDevice, ctx->side));
+        if (ctx->ec) CK(cudaMemsetAsync(ctx->dF, 0, bytes, ctx->side));
+        CK(cudaEventRecord(ctx->ev_state, ctx->side));
+        note_stream(ctx, ctx->side);
+        ctx->state_in_flight = true;
+        ctx->step = step; ctx->stats.step = step;
+        reset_slots(ctx);
+        return LSD_OK;
+    }
     const cudaMemcpyKind kind = where == LSD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
     CK(cudaMemcpyAsync(ctx->q, q, bytes, kind, ctx->side));
     CK(cudaMemcpyAsync(ctx->p, p, bytes, kind, ctx->side));
