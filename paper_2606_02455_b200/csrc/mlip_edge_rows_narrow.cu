@@ -6,7 +6,8 @@
 // the per-atom sums written as fp32 rows for the fp32 atom-wise layers of this path.  The segment-sum contraction always
 // reads 128 operand rows, so the stage keeps its full size (unused cells stay zero) and accumulator lanes >= F are ignored.
 // Replaces k_edge_tc (mlip_tc.cu: channels are rows, 64 edges per tile and three round trips) for these widths:
-// cfg3 bf16 window 2.45 -> 2.00 ms, draft network at cfg5 7.5 -> 6.1 ms per window; LSD_EDGE_NARROW=0 selects k_edge_tc.
+// cfg3 bf16 window 2.45 -> 2.00 ms, draft network at cfg5 7.5 -> 6.1 ms per window (4.35 ms with the four teams of width 32,
+// below); LSD_EDGE_NARROW=0 selects k_edge_tc.
 // The width-128 instantiation lives in mlip_edge_rows.cu: generated from this generic source the dominant kernel came out
 // 2.3 % slower (44.6 vs 43.6 ms per cfg5 window, same instruction counts in the tile loop), so its tuned translation unit is kept.
 // Determinism / batch invariance: as in mlip_edge_rows.cu.
@@ -21,7 +22,9 @@ namespace {
 using namespace tcp;
 
 constexpr int kR = LSD_NRBF;
-constexpr int kTeams = 2;
+// teams per SM: the width-32 kernels are pure round-trip latency (2 teams of 4 warps are as fast as 2 teams of 8), so they run 4
+// teams of ONE thread per edge in 128 TMEM columns each; width 64 keeps 2 teams of two threads per edge in 256 columns
+template <int F> struct Teams { static constexpr int N = F == 32 ? 4 : 2; };
 constexpr int kTT = 128;                               // edge slots of a tile
 constexpr int kCH = 16;                                // atoms per chunk = columns of D3
 constexpr int kGE = 16;                                // edge slots per record group
@@ -35,16 +38,23 @@ constexpr int kSTBytes = kCH * kTT * 2;
 // keeps its full size (the unused cells stay zero) and the accumulator lanes >= F are ignored.
 template <int F, bool BWD> struct Lay {
     static constexpr int NSLAB = BWD ? F / 4 : F / 8;  // 16-byte pieces of a gathered row (bwd: 4 channels x (y, y, mbar, mbar); fwd: 8 channels)
-    static constexpr int NSLAB_ALLOC = BWD ? 32 : 16;
+    static constexpr int kTeams = Teams<F>::N;
+    static constexpr int NSLAB_READ = BWD ? 32 : 16;   // slabs the segment-sum contraction reads (128 operand rows whatever the width)
+    // The stages of all teams come first, the other team buffers behind them.  Width 64 keeps full-size stages.  Width 32 has
+    // room for 4 teams only with stages of the slabs it uses: the contraction then reads on past a stage into the stages and
+    // buffers behind it -- allocated shared memory (asserted below) whose contents land in accumulator lanes >= F, which are ignored.
+    static constexpr int NSLAB_ALLOC = F == 32 ? NSLAB : NSLAB_READ;
     static constexpr int StageBytes = ((NSLAB_ALLOC * kSlab + 127) / 128) * 128;
     static constexpr int OwnBytes = BWD ? kCH * 4 * F : 0;
     static constexpr int W1Bytes = F * kR * 2, W2Bytes = F * F * 2;
     static constexpr int AccBytes = BWD ? kTT * kCH * 4 : 0;    // bwd: per (channel, atom) sums over the chunk's tiles (D3 is per tile there)
     static constexpr int MiscBytes = kMaxGroups + 128 /*pref*/ + 128 /*gpart*/ + 1024 /*gx*/ + AccBytes + 5 * kTT * 4 /*recS*/ + 256 /*fsum*/;
-    static constexpr int TeamBytes = StageBytes + OwnBytes + kSTBytes + MiscBytes;
+    static constexpr int RestBytes = OwnBytes + kSTBytes + MiscBytes;          // own rows, S, book-keeping of a team
+    static constexpr int TeamBytes = StageBytes + RestBytes;
     static constexpr int Smem = W1Bytes + W2Bytes + kTeams * TeamBytes;
     static_assert(Smem + 1024 <= 227 * 1024, "shared memory budget");
-    static_assert(TeamBytes % 16 == 0, "regions stay 16-byte aligned");
+    static_assert(StageBytes % 128 == 0 && RestBytes % 16 == 0, "regions stay aligned");
+    static_assert((kTeams - 1) * StageBytes + NSLAB_READ * kSlab <= kTeams * TeamBytes, "the last team's operand reads stay inside the allocation");
 };
 
 constexpr float kLog2e = 1.44269504088896340736f;
@@ -55,7 +65,12 @@ constexpr float kP0 = -0.49872449040412903f, kP1 = 0.2356506735086441f, kP2 = -0
 // bwd: D = [Dv 0..63 | Dt 64..127], A2v 128..191, A2t 192..255; G aliases A2v's second half (160..175), G' A2t's (224..239):
 //      they are dead when the activation of the second channel half overwrites them.  D3 of a tile lands in D (0..15).
 // fwd: D 0..127, A2 128..191, G 192..207, D3 208..223 (accumulated over the tiles of a chunk)
-constexpr uint32_t kColA2v = 128, kColA2t = 192, kColGb = 160, kColGtb = 224, kColGf = 192, kColD3f = 208;
+// width 32 (128 columns per team): bwd D = [Dv 0..31 | Dt 32..63], A2v 64..79, A2t 80..95, G 96..111, G' 112..127;
+//                                  fwd D 0..31, A2 32..47, G 48..63, D3 64..79
+template <int F> struct Cols {
+    static constexpr uint32_t A2v = F == 32 ? 64 : 128, A2t = F == 32 ? 80 : 192, Gb = F == 32 ? 96 : 160, Gtb = F == 32 ? 112 : 224;
+    static constexpr uint32_t A2f = F == 32 ? 32 : 128, Gf = F == 32 ? 48 : 192, D3f = F == 32 ? 64 : 208;
+};
 
 template <int TT> __device__ __forceinline__ void team_bar(int team) { asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(TT) : "memory"); }
 
@@ -81,14 +96,17 @@ __device__ __forceinline__ void act_pair(uint32_t h0u, uint32_t h1u, uint32_t hp
 }
 
 template <int F, bool BWD, int SPLIT>
-__global__ void __launch_bounds__(kTeams * kTT * SPLIT, 1)
+__global__ void __launch_bounds__(Teams<F>::N * kTT * SPLIT, 1)
 k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
 {
     using L = Lay<F, BWD>;
     constexpr int kF = F, HC = F >= 64 ? 64 : F, NH = F / HC;      // channels per contraction round, rounds per layer
     constexpr int kW1Bytes = L::W1Bytes, kW2Bytes = L::W2Bytes;
+    constexpr int kTeams = Teams<F>::N;
+    constexpr uint32_t kColA2v = BWD ? Cols<F>::A2v : Cols<F>::A2f, kColA2t = Cols<F>::A2t, kColGb = Cols<F>::Gb, kColGtb = Cols<F>::Gtb,
+                       kColGf = Cols<F>::Gf, kColD3f = Cols<F>::D3f;
     static_assert(F == 64 || F == 32, "narrow widths");
-    static_assert(F == 128 || SPLIT == 2, "narrow widths: two threads per edge");
+    static_assert((F == 32 && SPLIT == 1) || (F == 64 && SPLIT == 2), "width 32: one thread per edge, width 64: two");
     constexpr int TT = kTT * SPLIT;                    // threads of a team
     constexpr int TW = TT / 32;                        // warps of a team
     constexpr int kThreads = kTeams * TT;
@@ -126,26 +144,27 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
     tc_fence_after();
 
     const int team = __shfl_sync(0xffffffffu, warp, 0) / TW;     // warp-uniform (kept in uniform registers)
-    uint8_t* const tbuf = smem + kW1Bytes + kW2Bytes + team * L::TeamBytes;
+    uint8_t* const stage_buf = smem + kW1Bytes + kW2Bytes + team * L::StageBytes;                       // stages of all teams first
+    uint8_t* const tbuf = smem + kW1Bytes + kW2Bytes + kTeams * L::StageBytes + team * L::RestBytes;   // then the other buffers of a team
     const uint32_t sW1 = smem_u32(smem), sW2 = sW1 + kW1Bytes;
-    const uint32_t sStage = smem_u32(tbuf), sST = sStage + L::StageBytes + L::OwnBytes;
+    const uint32_t sStage = smem_u32(stage_buf), sST = smem_u32(tbuf) + L::OwnBytes;
     const uint32_t rdy = smem_u32(&mbar[2 * team]), done = rdy + 8;
-    const uint32_t tb = tmem_base_s + (uint32_t)(team * 256);
+    const uint32_t tb = tmem_base_s + (uint32_t)(team * (512 / kTeams));
     const bool need_sum = BWD ? (a.ybar16_out != nullptr || (F < 128 && a.ybar != nullptr)) : true;     // the adjoint of the first block needs the forces only
 
     {
         const int tt = tid - team * TT;                            // thread of the team
         const int e = tt & (kTT - 1), part = tt >> 7, wq = warp & 3;   // edge slot, channel part, TMEM lane quarter (warp % 4)
-        uint8_t* const stage = tbuf;
-        uint8_t* const own = stage + L::StageBytes;                // bwd: [16 atoms][512 B] (y, mbar) rows of the chunk's atoms
+        uint8_t* const stage = stage_buf;
+        uint8_t* const own = tbuf;                // bwd: [16 atoms][512 B] (y, mbar) rows of the chunk's atoms
         uint8_t* const ST = own + L::OwnBytes;
         uint8_t* const gatom = ST + kSTBytes;                      // group -> atom of the chunk
         int* const pref = reinterpret_cast<int*>(gatom + kMaxGroups);             // first group of every atom (17 entries)
         float* const gx = reinterpret_cast<float*>(gatom + kMaxGroups + 128) + 32;
         float* const gpart = gx;                                   // bwd: [2 tile parities][SPLIT parts][8 groups][4] force sums of the tile's groups
         float4* const accs = reinterpret_cast<float4*>(gx + 256);  // bwd: [4][128] float4: sums of channel e for atoms 4 j .. 4 j + 3
-        float* const fsum = reinterpret_cast<float*>(tbuf + L::TeamBytes - 256);      // bwd: [16 atoms][4] force sums of the chunk
-        float* const recS = reinterpret_cast<float*>(tbuf + L::TeamBytes - 256 - 5 * kTT * 4);   // [5 fields][128]: fc, fc', ux, uy, uz of the tile's slots
+        float* const fsum = reinterpret_cast<float*>(tbuf + L::RestBytes - 256);      // bwd: [16 atoms][4] force sums of the chunk
+        float* const recS = reinterpret_cast<float*>(tbuf + L::RestBytes - 256 - 5 * kTT * 4);   // [5 fields][128]: fc, fc', ux, uy, uz of the tile's slots
         const uint32_t lsel = (uint32_t)(wq * 32) << 16;
         const uint32_t tl = tb + lsel;
         const int n = a.n;
@@ -234,10 +253,11 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         const uint8_t* const rows = reinterpret_cast<const uint8_t*>(BWD ? (const void*)a.ym16 : (const void*)a.y16);
         constexpr int ROWB = BWD ? 4 * F : 2 * F;
 
-        for (int chunk = blockIdx.x * kTeams + team; chunk < nchunks; chunk += gridDim.x * kTeams) {
+        // team-major: a small batch (fewer chunks than teams on the device) still spreads over every SM
+        for (int chunk = blockIdx.x + team * (int)gridDim.x; chunk < nchunks; chunk += gridDim.x * kTeams) {
             const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
             const int g0 = b * n + ci * kCH;                       // first feature row of the chunk
-            tr_on = a.trace != nullptr && blockIdx.x == 0 && tt == 0 && chunk == blockIdx.x * kTeams + team + 3 * (int)gridDim.x * kTeams;
+            tr_on = a.trace != nullptr && blockIdx.x == 0 && tt == 0 && chunk == (int)blockIdx.x + team * (int)gridDim.x + 3 * (int)gridDim.x * kTeams;
             const int natoms = min(kCH, n - ci * kCH);
             if (tt < 32) {                                         // groups per atom, exclusive scan over the 16 atoms
                 const int c = tt < natoms ? a.count[g0 + tt] : 0;
@@ -290,12 +310,12 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
             auto issue_gathers = [&](int jrow) {
                 // runs of SL consecutive slabs this part consumes: SPLIT == 1 the whole row in runs of 8; SPLIT == 2 backward one run per
                 // channel round (slabs of 4 channels), forward one run (slabs of 8 channels)
-                constexpr int SL = SPLIT == 1 ? 8 : (BWD ? HC / 8 : F / 16);
-                constexpr int NRUN = SPLIT == 1 ? NSLAB / 8 : (BWD ? NH : 1);
+                constexpr int SL = SPLIT == 1 ? (NSLAB < 8 ? NSLAB : 8) : (BWD ? HC / 8 : F / 16);
+                constexpr int NRUN = SPLIT == 1 ? NSLAB / SL : (BWD ? NH : 1);
                 constexpr int EPI = 32 / SL;                       // edges per instruction: SL lanes = SL x 16 contiguous bytes of one row
 #pragma unroll
                 for (int gq = 0; gq < NRUN; ++gq) {
-                    const int s0 = SPLIT == 1 ? 8 * gq : (BWD ? (HC / 4) * gq + SL * part : SL * part);
+                    const int s0 = SPLIT == 1 ? SL * gq : (BWD ? (HC / 4) * gq + SL * part : SL * part);
 #pragma unroll
                     for (int i = 0; i < SL; ++i) {
                         const int el = EPI * i + lane / SL, s = s0 + lane % SL;
@@ -585,11 +605,12 @@ int device_sm_count()
 
 template <int F, bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
 {
+    constexpr int kTeams = Teams<F>::N;
     constexpr int threads = kTeams * kTT * SPLIT;
     cudaFuncSetAttribute(k_edge_rows<F, BWD, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lay<F, BWD>::Smem);
     const int cps = (a.n + kCH - 1) / kCH;
     const int nchunks = cps * (a.total / a.n);
-    const int grid = std::max(1, std::min(device_sm_count(), (nchunks + kTeams - 1) / kTeams));
+    const int grid = std::max(1, std::min(device_sm_count(), nchunks));
     static const bool trace_on = [] { const char* v = getenv("LSD_EDGE_TRACE"); return v && v[0] == '1'; }();
     static int trace_launch[2] = {0, 0};
     if (trace_on && ++trace_launch[BWD] == 8) {                    // debug: time stamps of one chunk, printed once per direction
@@ -626,5 +647,5 @@ template <int F, bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArg
 void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward)
 {
     if (F == 64) { if (backward) launch_rows<64, true, 2>(L, a); else launch_rows<64, false, 2>(L, a); }
-    else if (F == 32) { if (backward) launch_rows<32, true, 2>(L, a); else launch_rows<32, false, 2>(L, a); }
+    else if (F == 32) { if (backward) launch_rows<32, true, 1>(L, a); else launch_rows<32, false, 1>(L, a); }
 }
