@@ -272,6 +272,7 @@ void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // ml
 void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
 void launch_edge_pipe(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_pipe.cu: width 128, warp-specialised pipeline of the same tile algebra
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_rows.cu: width 128, edges-as-rows, activations in TMEM
+void launch_edge_fwd4(Launcher L, const EdgeArgs& a);                      // mlip_edge_fwd4.cu: width 128, forward, four tiles in flight per SM
 void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward);   // mlip_edge_rows_narrow.cu: the same kernel, width-generic, for widths 32 / 64 (fp32 rows out)
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout
 void tc_pack_weights(const double* Wf1, const double* Wf2, int F, int R, std::vector<uint16_t>& out1, std::vector<uint16_t>& out2);

@@ -379,6 +379,9 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     // LSD_EDGE_PIPE: which passes use the warp-specialised pipeline (mlip_edge_pipe.cu); same bits; takes precedence
     static const int pipe_sel = [] { const char* v = getenv("LSD_EDGE_PIPE"); return v ? atoi(v) : 0; }();
     const bool use_pipe_f = (pipe_sel & 1) != 0, use_pipe_b = (pipe_sel & 2) != 0;
+    // LSD_EDGE_FWD4: forward pass with four tiles in flight per SM (mlip_edge_fwd4.cu; default, measured 2.9 vs 3.9 ms per cfg5
+    // launch); 0 falls back to the selection above
+    static const bool use_fwd4 = [] { const char* v = getenv("LSD_EDGE_FWD4"); return v == nullptr || v[0] != '0'; }();
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
     uint16_t* const xbar16 = reinterpret_cast<uint16_t*>(w.mbar);
@@ -392,7 +395,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_pipe_f) launch_edge_pipe(L, ea, false); else if (use_rows_f) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
+        if (use_fwd4) launch_edge_fwd4(L, ea); else if (use_pipe_f) launch_edge_pipe(L, ea, false); else if (use_rows_f) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
         prof_end(L, pid);
         AtomArgs aa{};
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;

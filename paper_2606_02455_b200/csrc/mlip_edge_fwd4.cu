@@ -1,0 +1,312 @@
+// bf16 tcgen05 filter path, width F = 128, FORWARD pass  m_i = sum_j y_j . w_ij  (M5, section 4.1) with FOUR tiles in
+// flight per SM.  Same tile algebra as mlip_edge_rows.cu (a tile is 128 edge slots, TMEM lane = edge = thread, radial basis and
+// activations are A operands in tensor memory, the gathered rows y_j sit in a slab-layout stage that the segment-sum operand
+// P = bf16(lin) . y_j overwrites in place, D3 = P^T S with the cutoff riding on S).  Measured in round 2: these kernels are
+// bound by the serial latency of a team's contraction round trips, not by any pipe -- one thread per edge (4 warps per team) is
+// as fast as two (8 warps) -- so the lever is the number of tiles in flight, and tensor memory is what limits it.  Here a
+// team needs 128 columns instead of 224: the contractions run as channel halves (D = 64 columns, A2 = 64 columns of bf16
+// pairs, G aliased into A2's second half, which is dead until the second half is activated) and the per-tile D3 lands in D
+// and is summed over the chunk's tiles in shared memory.  Five round trips per tile instead of three, four teams instead of
+// two.  Determinism / batch invariance: as in mlip_edge_rows.cu (every sum has a fixed order that depends only on the atom's
+// sorted neighbour row and on the 16-atom chunking of its state).
+#include <algorithm>
+#include <cstdlib>
+#include "lsd_internal.h"
+#include "tc_ptx.cuh"
+
+namespace {
+using namespace tcp;
+
+constexpr int kF = 128;
+constexpr int kR = LSD_NRBF;
+constexpr int kTeams = 4;
+constexpr int kTT = 128;                               // threads of a team = edge slots of a tile
+constexpr int kThreads = kTeams * kTT;
+constexpr int kCH = 16;                                // atoms per chunk = columns of D3
+constexpr int kGE = 16;                                // edge slots per record group
+constexpr int kGPT = kTT / kGE;                        // groups per tile
+constexpr int kMaxGroups = kCH * (512 / kGE);
+constexpr int kW1Bytes = kF * kR * 2, kW2Bytes = kF * kF * 2;
+constexpr int kSlab = 2048 + 16;                       // bytes between slabs of the stage (16 B x 128 edges + one bank group)
+constexpr int kNSlab = 16;                             // 16-byte pieces (8 channels) of a gathered row
+constexpr int kStageBytes = ((kNSlab * kSlab + 127) / 128) * 128;
+constexpr int kSTBytes = kCH * kTT * 2;
+constexpr int kAccBytes = kTT * kCH * 4;               // per (channel, atom) sums over the chunk's tiles
+constexpr int kTeamBytes = kStageBytes + kSTBytes + kAccBytes + kMaxGroups + 128 /*pref*/ + kTT * 4 /*fc of the tile's slots*/;
+constexpr int kSmem = kW1Bytes + kW2Bytes + kTeams * kTeamBytes;
+static_assert(kSmem + 1024 <= 227 * 1024, "shared memory budget");
+static_assert(kTeamBytes % 16 == 0, "regions stay 16-byte aligned");
+
+constexpr float kLog2e = 1.44269504088896340736f;
+// -ln(1 + a) / (2 a) on [0, 1] (weighted minimax fit of a P(a), |error| < 3.6e-5)
+constexpr float kP0 = -0.49872449040412903f, kP1 = 0.2356506735086441f, kP2 = -0.11284290254116058f, kP3 = 0.02937859483063221f;
+
+// TMEM columns of a team (128 per team): D 0..63 (one channel half; D3 of a tile in 0..15), A2 64..127, G 96..111
+constexpr uint32_t kColA2 = 64, kColG = 96;
+
+__device__ __forceinline__ void team_bar(int team) { asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTT) : "memory"); }
+
+// ssp(2h)/2 for a pair of channels; h = x/2 comes out of the first contraction because W_f1 is packed halved (and W_f2 doubled):
+// ssp(x)/2 = max(h, 0) + a P(a), a = tanh|h|
+__device__ __forceinline__ uint32_t act_pair(uint32_t h0u, uint32_t h1u)
+{
+    const float h0 = __uint_as_float(h0u), h1 = __uint_as_float(h1u);
+    const f32x2 a2 = pk2(tanhf_approx(fabsf(h0)), tanhf_approx(fabsf(h1)));
+    f32x2 r2 = fma2(pk2(kP3, kP3), a2, pk2(kP2, kP2));
+    r2 = fma2(r2, a2, pk2(kP1, kP1));
+    r2 = fma2(r2, a2, pk2(kP0, kP0));
+    return pack_bf16(fma2(r2, a2, pk2(fmaxf(h0, 0.f), fmaxf(h1, 0.f))));
+}
+
+enum { R_G1H0 = 0, R_G1H1 = 1, R_G2O0 = 2, R_G2O1 = 3, R_G3 = 4 };
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_edge_fwd4(EdgeArgs a, int chunks_per_state, int nchunks)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t mbar[2 * kTeams];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    {   // resident B operand images (K-major): W_f1 / 2 [128 x 32], 2 W_f2 [128 x 128]; every other buffer starts as zeros
+        const uint4* s1 = reinterpret_cast<const uint4*>(a.Wf1_tc);
+        const uint4* s2 = reinterpret_cast<const uint4*>(a.Wf2_tc);
+        uint4* d1 = reinterpret_cast<uint4*>(smem);
+        uint4* d2 = reinterpret_cast<uint4*>(smem + kW1Bytes);
+        for (int i = tid; i < kW1Bytes / 16; i += kThreads) d1[i] = s1[i];
+        for (int i = tid; i < kW2Bytes / 16; i += kThreads) d2[i] = s2[i];
+        uint4* z = reinterpret_cast<uint4*>(smem + kW1Bytes + kW2Bytes);
+        for (int i = tid; i < kTeams * kTeamBytes / 16; i += kThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    if (tid == 0) {
+        for (int t = 0; t < kTeams; ++t) {
+            mbar_init(smem_u32(&mbar[2 * t]), kTT / 32);   // "operand published / accumulator consumed": one arrival per warp of the team
+            mbar_init(smem_u32(&mbar[2 * t + 1]), 1);      // "contractions of the round complete" (tcgen05.commit)
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+
+    const int team = __shfl_sync(0xffffffffu, warp, 0) >> 2;       // warp-uniform
+    uint8_t* const stage = smem + kW1Bytes + kW2Bytes + team * kTeamBytes;
+    uint8_t* const ST = stage + kStageBytes;
+    float4* const accs = reinterpret_cast<float4*>(ST + kSTBytes);  // [4][128] float4: sums of channel e for atoms 4 j .. 4 j + 3
+    uint8_t* const gatom = reinterpret_cast<uint8_t*>(accs) + kAccBytes;   // group -> atom of the chunk
+    int* const pref = reinterpret_cast<int*>(gatom + kMaxGroups);   // first group of every atom (17 entries)
+    float* const fcS = reinterpret_cast<float*>(gatom + kMaxGroups + 128);   // cutoff of the tile's slots
+    const uint32_t sW1 = smem_u32(smem), sW2 = sW1 + kW1Bytes, sStage = smem_u32(stage), sST = smem_u32(ST);
+    const uint32_t rdy = smem_u32(&mbar[2 * team]), done = rdy + 8;
+    const uint32_t tb = tmem_base_s + (uint32_t)(team * 128);
+    const int e = tid & (kTT - 1), wq = warp & 3;                  // edge slot = channel of the final sums; TMEM lane quarter
+    const uint32_t tl = tb + ((uint32_t)(wq * 32) << 16);
+    const int n = a.n;
+    const float c2 = -0.5f * kLog2e * a.inv_delta2;
+    const int my_g = e >> 4, my_s = e & 15;
+    const uint8_t* const rows = reinterpret_cast<const uint8_t*>(a.y16);
+
+    // ---- round protocol (as in mlip_edge_rows.cu): every warp publishes what it wrote / that it is done reading the accumulator
+    // (one arrival per warp on `rdy`); the team's last warp waits for all arrivals, one elected lane of it issues the
+    // contractions of the round and commits them to `done`; then every warp waits for `done`.
+    uint32_t ph = 0, phr = 0;
+    const bool issuer = wq == 3;
+    const uint32_t id64 = make_idesc(128, 64, 0), id3 = make_idesc(128, kCH, 0) | (1u << 15);
+    const uint64_t dW1 = make_desc(sW1, 128, 512), dW2 = make_desc(sW2, 128, 2048);
+    const uint64_t dP = make_desc(sStage, 128, kSlab), dS = make_desc(sST, 128, 2048);
+    auto publish = [&](int kind) {
+        tc_fence_before();
+        warp_arrive(rdy, lane);
+        if (issuer) {
+            mbar_wait(rdy, phr); phr ^= 1u;
+            tc_fence_after();
+            if (elect_one()) {
+                if (kind == R_G1H0 || kind == R_G1H1) {            // x of channel half h
+                    const int h = kind - R_G1H0;
+#pragma unroll
+                    for (int k16 = 0; k16 < kR / 16; ++k16)
+                        umma_ts(tb, tb + kColG + 8 * k16, dW1 + (uint64_t)((h * 4096 + k16 * 256) >> 4), id64, k16 > 0);
+                } else if (kind == R_G2O0 || kind == R_G2O1) {     // lin of output channel half o
+                    const int o = kind - R_G2O0;
+#pragma unroll
+                    for (int k16 = 0; k16 < kF / 16; ++k16)
+                        umma_ts(tb, tb + kColA2 + 8 * k16, dW2 + (uint64_t)((o * 16384 + k16 * 256) >> 4), id64, k16 > 0);
+                } else {                                           // D3 (this tile) = P^T S
+#pragma unroll
+                    for (int k16 = 0; k16 < kTT / 16; ++k16) umma(tb, dP + (uint64_t)(k16 * 16), dS + (uint64_t)(k16 * 16), id3, k16 > 0);
+                }
+                umma_commit(done);
+            }
+            __syncwarp();
+        }
+    };
+    auto await = [&]() { mbar_wait(done, ph); ph ^= 1u; tc_fence_after(); };
+
+    // team-major chunk assignment: a small batch still spreads over every SM
+    for (int chunk = blockIdx.x + team * (int)gridDim.x; chunk < nchunks; chunk += gridDim.x * kTeams) {
+        const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
+        const int g0 = b * n + ci * kCH;                           // first feature row of the chunk
+        const int natoms = min(kCH, n - ci * kCH);
+        if (e < 32) {                                              // groups per atom, exclusive scan over the 16 atoms
+            const int c = e < natoms ? a.count[g0 + e] : 0;
+            int v = (c + kGE - 1) / kGE;
+#pragma unroll
+            for (int o = 1; o < 16; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, v, o); if (e >= o) v += u; }
+            if (e < kCH) pref[e + 1] = v;
+            if (e == 0) pref[0] = 0;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) accs[j * kTT + e] = make_float4(0.f, 0.f, 0.f, 0.f);
+        team_bar(team);
+        const int G = pref[kCH];
+        if (e < kCH) for (int g = pref[e]; g < pref[e + 1]; ++g) gatom[g] = (uint8_t)e;
+        const int ntiles = (G + kGPT - 1) / kGPT;
+        team_bar(team);
+
+        // record of this thread's edge slot in tile t (the zero group behind the chunk's last group), fetched one tile ahead
+        float r_n; int jrow_n, at_n; const float* rp_n;
+        auto load_record = [&](int t) {
+            const int gl = t * kGPT + my_g;
+            at_n = -1; rp_n = a.rec_zero + my_s;
+            if (gl < G) {
+                at_n = gatom[gl];
+                rp_n = a.recs + lsd_rec_index((size_t)(g0 + at_n), a.cap, (gl - pref[at_n]) * kGE + my_s, 0);
+            }
+            r_n = rp_n[LSD_REC_R * 16];
+            jrow_n = at_n >= 0 ? __float_as_int(rp_n[LSD_REC_JROW * 16]) : g0;
+        };
+        if (ntiles > 0) load_record(0);
+        for (int t = 0; t < ntiles; ++t) {
+            const int at = at_n;
+            // ---- gathers: this warp's pieces of the rows y_j of its own 32 edges -> slabs (8 lanes = 128 contiguous bytes of a row)
+#pragma unroll
+            for (int gq = 0; gq < kNSlab / 8; ++gq) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int el = 4 * i + (lane >> 3), s = 8 * gq + (lane & 7);
+                    const int jr = __shfl_sync(0xffffffffu, jrow_n, el);
+                    cp_async16_ca(sStage + (uint32_t)(s * kSlab + (32 * wq + el) * 16), rows + (size_t)jr * (kF * 2) + s * 16);
+                }
+            }
+            cp_async4(smem_u32(fcS) + (uint32_t)e * 4, rp_n + LSD_REC_FC * 16);
+            cp_async_commit();
+            {   // ---- radial basis (M1) of the thread's edge -> TMEM, packed bf16 pairs along k
+                uint32_t gv[kR / 2];
+                const f32x2 c22 = pk2(c2, c2);
+#pragma unroll
+                for (int k = 0; k < kR; k += 2) {
+                    const float x0 = r_n - (float)k * a.delta, x1 = x0 - a.delta;
+                    const f32x2 x2 = pk2(x0, x1);
+                    float e0, e1;
+                    un2(mul2(mul2(x2, x2), c22), e0, e1);
+                    gv[k >> 1] = pack_bf16(ex2f(e0), ex2f(e1));
+                }
+                tmem_st16(tl + kColG, gv);
+                tmem_wait_st();
+            }
+            publish(R_G1H0);
+            if (t + 1 < ntiles) load_record(t + 1);                // lands under the round trips
+            // ---- activation (M3) of channel half h: D -> A2 (32 columns of bf16 pairs)
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {
+                await();
+#pragma unroll
+                for (int c0 = 0; c0 < 64; c0 += 32) {
+                    uint32_t pv[16];
+#pragma unroll
+                    for (int c1 = 0; c1 < 32; c1 += 16) {
+                        uint32_t v[16];
+                        tmem_ld16(tl + c0 + c1, v);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int c = 0; c < 16; c += 2) pv[(c1 + c) >> 1] = act_pair(v[c], v[c + 1]);
+                    }
+                    tmem_st16(tl + kColA2 + 32 * h + c0 / 2, pv);
+                }
+                tmem_wait_st();
+                publish(h == 0 ? R_G1H1 : R_G2O0);
+            }
+            // ---- epilogue of output half o: P = bf16(lin) . y_j, in place (8 channels = one 16-byte cell)
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+#pragma unroll 1
+            for (int o = 0; o < 2; ++o) {
+                await();
+#pragma unroll
+                for (int c0 = 0; c0 < 64; c0 += 16) {
+                    uint32_t v[16];
+                    tmem_ld16(tl + c0, v);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int q8 = 0; q8 < 2; ++q8) {
+                        uint8_t* cell = stage + ((64 * o + c0 + 8 * q8) >> 3) * kSlab + e * 16;
+                        const uint4 y = *reinterpret_cast<const uint4*>(cell);
+                        uint4 p;
+                        p.x = bmul2(pack_bf16(__uint_as_float(v[8 * q8]), __uint_as_float(v[8 * q8 + 1])), y.x);
+                        p.y = bmul2(pack_bf16(__uint_as_float(v[8 * q8 + 2]), __uint_as_float(v[8 * q8 + 3])), y.y);
+                        p.z = bmul2(pack_bf16(__uint_as_float(v[8 * q8 + 4]), __uint_as_float(v[8 * q8 + 5])), y.z);
+                        p.w = bmul2(pack_bf16(__uint_as_float(v[8 * q8 + 6]), __uint_as_float(v[8 * q8 + 7])), y.w);
+                        *reinterpret_cast<uint4*>(cell) = p;
+                    }
+                }
+                if (o == 0) { fence_async_smem(); publish(R_G2O1); }
+            }
+            uint16_t* const st_e = reinterpret_cast<uint16_t*>(ST + ((at >= 0 ? at : 0) >> 3) * 2048 + (e >> 3) * 128 + ((at >= 0 ? at : 0) & 7) * 16 + (e & 7) * 2);
+            if (at >= 0) {                                         // S^T[e][at] = fc
+                const __nv_bfloat16 fb = __float2bfloat16_rn(fcS[e]);
+                *st_e = *reinterpret_cast<const uint16_t*>(&fb);
+            }
+            fence_async_smem();
+            publish(R_G3);                                         // -> D3 = P^T S
+            await();                                               // the stage (P) and S are free again
+            {   // thread = channel e: this tile's sums of the 16 atoms
+                uint32_t v[16];
+                tmem_ld16(tl, v);
+                tmem_wait_ld();
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    float4 s4 = accs[j * kTT + e];
+                    s4.x += __uint_as_float(v[4 * j]); s4.y += __uint_as_float(v[4 * j + 1]); s4.z += __uint_as_float(v[4 * j + 2]); s4.w += __uint_as_float(v[4 * j + 3]);
+                    accs[j * kTT + e] = s4;
+                }
+            }
+            if (at >= 0) *st_e = 0;
+        }
+        // ---- sums of the chunk -> bf16 rows (thread = channel e)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 s4 = accs[j * kTT + e];
+            const float acc[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int at = 4 * j + i;
+                if (at < natoms) { const __nv_bfloat16 pb = __float2bfloat16_rn(acc[i]); a.m16_out[(size_t)(g0 + at) * kF + e] = *reinterpret_cast<const uint16_t*>(&pb); }
+            }
+        }
+        tc_fence_before();
+        team_bar(team);                                            // pref / gatom / sums are rewritten by the next chunk
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
+}
+
+}  // namespace
+
+void launch_edge_fwd4(Launcher L, const EdgeArgs& a)
+{
+    static bool configured_dev[64] = {};
+    bool& configured = configured_dev[lsd_current_device()];
+    if (!configured) { cudaFuncSetAttribute(k_edge_fwd4, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem); configured = true; }
+    const int cps = (a.n + kCH - 1) / kCH;
+    const int nchunks = cps * (a.total / a.n);
+    const int grid = std::max(1, std::min(lsd_sm_count(), nchunks));
+    k_edge_fwd4<<<grid, kThreads, kSmem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(false, 8, kCH, kThreads, grid, kF);
+    LSD_COUNT(L);
+}

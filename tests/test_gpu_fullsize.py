@@ -138,7 +138,7 @@ def test_full_size_forces_match_oracle(P, orc, name, prec, states):
         assert fwd["width"] == w.target.mlip.width and bwd["width"] == w.target.mlip.width     # the target's launches were the last ones
         if w.target.mlip.width == 128:
             # the kernels the cfg5 / cfg4 bench lines time, with a grid that fills the device
-            assert bwd["kernel"] in ("k_edge_rows", "k_edge_pipe", "k_edge_tc128") and fwd["kernel"] in ("k_edge_er128_fwd", "k_edge_rows", "k_edge_pipe")
+            assert bwd["kernel"] in ("k_edge_rows", "k_edge_pipe", "k_edge_tc128") and fwd["kernel"] in ("k_edge_er128_fwd", "k_edge_rows", "k_edge_pipe", "k_edge_fwd4")
             assert bwd["grid"] >= 148 and fwd["grid"] >= 148
             if bwd["kernel"] == "k_edge_tc128":
                 assert bwd["atoms_per_chunk"] == 64                # not the small-batch instantiation
