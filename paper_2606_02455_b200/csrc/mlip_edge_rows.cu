@@ -287,10 +287,11 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                 jrow_n = at_n >= 0 ? __float_as_int(rp_n[LSD_REC_JROW * 16]) : g0;
             };
             // this warp's pieces of the neighbour rows of its 32 edges -> slabs (8 lanes = 128 contiguous bytes of one row)
-            auto issue_gathers = [&](int jrow) {
-                constexpr int NGRP = NSLAB / 8 / SPLIT;            // groups of 8 slabs this part consumes
+            constexpr int NGRP = NSLAB / 8 / SPLIT;                // groups of 8 slabs this part consumes
+            auto issue_gathers = [&](int jrow, int g_begin, int g_end) {
 #pragma unroll
                 for (int gq = 0; gq < NGRP; ++gq) {
+                    if (gq < g_begin || gq >= g_end) continue;
                     // bwd: output half o = gq covers slabs 16 o + (16 / SPLIT) part ...; fwd: part owns channels [64 part, +64)
                     const int s0 = BWD ? (SPLIT == 2 ? 16 * gq + 8 * part : 8 * gq) : (SPLIT == 2 ? 8 * part : 8 * gq);
 #pragma unroll
@@ -335,7 +336,12 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
             load_record(0);
             for (int t = 0; t < ntiles; ++t) {
                 TRACE(1);
-                issue_gathers(jrow_n);
+                // first contraction first: its round trip runs under the issue of this tile's gathers
+                stage_basis(r_n);
+                TRACE(2);
+                publish(BWD ? R_G1H0 : R_F1);
+                TRACE(3);
+                issue_gathers(jrow_n, 0, BWD ? NGRP / 2 : NGRP);   // bwd: the rows' first channel half (the second: under the next round trip)
                 if (part == 0) {                                   // cutoff (slope, unit vector) of the slot: asynchronous 4-byte copies, read at the tile's end
                     const uint32_t d = smem_u32(recS) + (uint32_t)e * 4;
                     cp_async4(d, rp_n + LSD_REC_FC * 16);
@@ -345,10 +351,6 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                     }
                 }
                 cp_async_commit();
-                TRACE(2);
-                stage_basis(r_n);
-                TRACE(3);
-                publish(BWD ? R_G1H0 : R_F1);                      // -> first contraction
 
                 if (BWD) {
                     constexpr int NC = 64 / SPLIT;                 // channels of a half this thread handles
@@ -383,6 +385,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         tmem_wait_st();
                         TRACE(6);
                         publish(h == 0 ? R_G1H1 : R_G2O0);
+                        if (h == 0) { issue_gathers(jrow_n, NGRP / 2, NGRP); cp_async_commit(); }
                     }
                     TRACE(7);
                     // ---- epilogue of output half o: P = bf16(lin) . mbar_j (in place), A = sum_f c_f lin'_f, B = sum_f c_f lin_f,
