@@ -305,6 +305,15 @@ lsd_status alloc_work(lsd_ctx* ctx, const MlipDev& net, MlipWork& w, int bmax)
         for (int t = 0; t < net.T; ++t) TRY(dalloc(ctx, &w.y16[t], e));
         TRY(dalloc(ctx, &w.mbar16, e));
         TRY(dalloc(ctx, &w.ym16, e));
+        if (net.F == 128) {                                            // TMA tensor map over the pair rows (gather4 of the backward edge kernel)
+            alignas(64) unsigned char hm[128];
+            if (lsd_encode_row_tmap(hm, w.ym16, rows, 512)) {
+                unsigned char* dm = nullptr;
+                TRY(dalloc(ctx, &dm, (size_t)128));
+                CK(cudaMemcpy(dm, hm, 128, cudaMemcpyHostToDevice));
+                w.ym_tmap = dm;
+            }
+        }
     }
     return LSD_OK;
 }

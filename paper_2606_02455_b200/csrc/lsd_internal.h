@@ -115,6 +115,7 @@ struct MlipWork {                    // activations of one batched evaluation (k
     std::vector<uint16_t*> y16;      // [T] bf16 copies of y gathered by the tcgen05 edge kernels (LSD_BF16_TC only)
     uint16_t* mbar16 = nullptr;      // bf16 copy of mbar
     uint32_t* ym16 = nullptr;        // width 128 only: rows of (y, mbar) bf16 pairs gathered by the backward tcgen05 kernel
+    void* ym_tmap = nullptr;         // device copy of the TMA tensor map over ym16 (rows of 512 B, boxes of 128 B x 1 row, 128-byte swizzle)
     double* e_atom = nullptr;        // [bmax*n]
     int y0_rows = 0;                 // one-block networks: rows of y[0] / y16[0] (species-only) already written
 };
@@ -232,6 +233,7 @@ struct EdgeArgs {
     const float* y;                   // [total][F]
     const uint16_t *y16 = nullptr, *mbar16 = nullptr;   // bf16 rows gathered by the tcgen05 kernels
     const uint32_t* ym16 = nullptr;   // [total][F] (y | mbar << 16) bf16 pairs, width-128 backward kernel
+    const void* ym_tmap = nullptr;    // TMA tensor map over ym16 (global memory); null: cp.async gathers
     float* m_out;                     // FWD: m
     uint16_t* m16_out = nullptr;      // FWD, width 128: m as bf16 rows instead of m_out
     uint16_t* ybar16_out = nullptr;   // BWD, width 128: ybar as bf16 rows instead of ybar
@@ -272,6 +274,7 @@ void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // ml
 void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
 void launch_edge_pipe(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_pipe.cu: width 128, warp-specialised pipeline of the same tile algebra
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_rows.cu: width 128, edges-as-rows, activations in TMEM
+bool lsd_encode_row_tmap(void* host_map_128B, const void* base, size_t rows, int row_bytes);   // mlip_edge_rows.cu: false if the driver lacks the entry point
 void launch_edge_fwd4(Launcher L, const EdgeArgs& a);                      // mlip_edge_fwd4.cu: width 128, forward, four tiles in flight per SM
 void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward);   // mlip_edge_rows_narrow.cu: the same kernel, width-generic, for widths 32 / 64 (fp32 rows out)
 // host: pack W_f1 [F][R] / W_f2 [F][F] (row-major fp64) as bf16 in the no-swizzle K-major UMMA layout

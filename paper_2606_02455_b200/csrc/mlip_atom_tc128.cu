@@ -417,7 +417,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
             aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t]; aa.ym_pairs = use_rows || use_pipe_b;
             launch_atom<BWD2>(L, aa);
         }
-        ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.ym16 = w.ym16;
+        ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.ym16 = w.ym16; ea.ym_tmap = w.ym_tmap;
         ea.ybar16_out = t > 0 ? ybar16 : nullptr; ea.ybar = nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
         if (use_pipe_b) launch_edge_pipe(L, ea, true); else if (use_rows) launch_edge_rows(L, ea, true); else launch_edge_tc128(L, ea, true);

@@ -23,6 +23,7 @@
 //   * 2 threads per edge (SPLIT = 2): a team is 8 warps, 16 compute warps per SM.
 // Determinism / batch invariance: every sum has a fixed order that depends only on the atom's own sorted neighbour row and
 // on the chunking of its state (16 consecutive atoms), never on the batch or on the grid.
+#include <cuda.h>
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -45,14 +46,17 @@ constexpr int kW1Bytes = kF * kR * 2, kW2Bytes = kF * kF * 2;
 constexpr int kSlab = 2048 + 16;                       // bytes between slabs of the gather stage (16 B x 128 edges + shift by one bank group)
 constexpr int kSTBytes = kCH * kTT * 2;
 
-template <bool BWD> struct Lay {
+// TMA (backward only): the stage is four 1024-byte aligned regions [128 edges][128 B] with the 128-byte swizzle (region s =
+// bytes 128 s .. 128 s + 127 of the gathered rows), written by cp.async.bulk.tensor gather4 instead of per-lane cp.async
+template <bool BWD, bool TMA = false> struct Lay {
     static constexpr int NSLAB = BWD ? 32 : 16;        // 16-byte pieces of a gathered row (bwd: 4 channels x (y, y, mbar, mbar); fwd: 8 channels)
-    static constexpr int StageBytes = ((NSLAB * kSlab + 127) / 128) * 128;
+    static constexpr int StageBytes = TMA ? kTT * 512 : ((NSLAB * kSlab + 127) / 128) * 128;
     static constexpr int OwnBytes = BWD ? kCH * 512 : 0;
     static constexpr int AccBytes = BWD ? kTT * kCH * 4 : 0;    // bwd: per (channel, atom) sums over the chunk's tiles (D3 is per tile there)
-    static constexpr int MiscBytes = kMaxGroups + 128 /*pref*/ + 128 /*gpart*/ + 1024 /*gx*/ + AccBytes + 5 * kTT * 4 /*recS*/ + 256 /*fsum*/;
+    static constexpr int MiscBytes = kMaxGroups + 128 /*pref*/ + 128 /*gpart*/ + 1024 /*gx*/ + AccBytes + 5 * kTT * 4 /*recS*/ + 256 /*fsum*/ + (TMA ? 512 : 0);
     static constexpr int TeamBytes = StageBytes + OwnBytes + kSTBytes + MiscBytes;
-    static constexpr int Smem = kW1Bytes + kW2Bytes + kTeams * TeamBytes;
+    static constexpr int Smem = kW1Bytes + kW2Bytes + kTeams * TeamBytes + (TMA ? 1024 : 0);
+    static_assert(!TMA || (TeamBytes % 1024 == 0 && (kW1Bytes + kW2Bytes) % 1024 == 0), "swizzled regions stay 1024-byte aligned");
     static_assert(Smem + 1024 <= 227 * 1024, "shared memory budget");
     static_assert(TeamBytes % 16 == 0, "regions stay 16-byte aligned");
 };
@@ -90,19 +94,22 @@ __device__ __forceinline__ void act_pair(uint32_t h0u, uint32_t h1u, uint32_t hp
     }
 }
 
-template <bool BWD, int SPLIT>
+template <bool BWD, int SPLIT, bool TMA = false>
 __global__ void __launch_bounds__(kTeams * kTT * SPLIT, 1)
 k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
 {
-    using L = Lay<BWD>;
+    static_assert(!TMA || (BWD && SPLIT == 2), "the TMA gather is implemented for the two-part backward");
+    using L = Lay<BWD, TMA>;
     constexpr int TT = kTT * SPLIT;                    // threads of a team
     constexpr int TW = TT / 32;                        // warps of a team
     constexpr int kThreads = kTeams * TT;
     constexpr int NSLAB = L::NSLAB;
-    extern __shared__ __align__(128) uint8_t smem[];
+    extern __shared__ __align__(128) uint8_t smem_raw[];
     __shared__ __align__(8) uint64_t mbar[2 * kTeams];
+    __shared__ __align__(8) uint64_t gbar_s[kTeams];    // TMA: "the tile's gathered rows have landed" (transaction count)
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    uint8_t* const smem = TMA ? smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) : smem_raw;
 
     {   // resident B operand images (K-major): W_f1 / 2 [128 x 32], 2 W_f2 [128 x 128]; every other buffer starts as zeros
         const uint4* s1 = reinterpret_cast<const uint4*>(a.Wf1_tc);
@@ -118,6 +125,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         for (int t = 0; t < kTeams; ++t) {
             mbar_init(smem_u32(&mbar[2 * t]), TW);     // "operand published / accumulator consumed": one arrival per warp of the team
             mbar_init(smem_u32(&mbar[2 * t + 1]), 1);  // "contractions of the round complete" (tcgen05.commit)
+            if (TMA) mbar_init(smem_u32(&gbar_s[t]), 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
     }
@@ -161,11 +169,15 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         // elected lane of it issues the contractions of the round and commits them to `done`; then every warp waits for `done`.
         // No dedicated MMA warps: 16 warps per SM leave 128 registers per thread (a spilled register costs an L2 round trip here,
         // the L1 cache is what the 200 KB of shared memory leave over).
-        uint32_t ph = 0, phr = 0;
+        uint32_t ph = 0, phr = 0, gph = 0;
+        const uint32_t gbar = smem_u32(&gbar_s[team]);
         const bool issuer = (warp % TW) == TW - 1;
         const uint32_t id64 = make_idesc(128, 64, 0), id128 = make_idesc(128, 128, 0), id3 = make_idesc(128, kCH, 0) | (1u << 15);
         const uint64_t dW1 = make_desc(sW1, 128, 512), dW2 = make_desc(sW2, 128, 2048);
-        const uint64_t dP = make_desc(sStage, 128, BWD ? 2 * kSlab : kSlab), dS = make_desc(sST, 128, 2048);
+        // P^T (MN-major): slab layout, or (TMA) two 128-byte swizzled atoms of 64 channel slots [region 0 | region 1]
+        const uint64_t dP = TMA ? make_desc_sw128(sStage, kTT * 128, 1024) : make_desc(sStage, 128, BWD ? 2 * kSlab : kSlab);
+        const uint64_t dS = make_desc(sST, 128, 2048);
+        constexpr uint32_t kPStep = TMA ? 128 : 16;                // descriptor units (16 B) per 16 edges of K
         enum { R_G1H0 = 0, R_G1H1 = 1, R_G2O0 = 2, R_G2O1 = 3, R_G3 = 4, R_F1 = 5, R_F2 = 6, R_F3NEW = 7, R_F3ACC = 8, R_SYNC = 9 };
         int tile_in_chunk = 0;
         auto publish = [&](int kind) {
@@ -193,7 +205,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         }
                     } else if (kind == R_G3) {                     // D3 (this tile) = P^T S
 #pragma unroll
-                        for (int k16 = 0; k16 < kTT / 16; ++k16) umma(tb, dP + (uint64_t)(k16 * 16), dS + (uint64_t)(k16 * 16), id3, k16 > 0);
+                        for (int k16 = 0; k16 < kTT / 16; ++k16) umma(tb, dP + (uint64_t)(k16 * kPStep), dS + (uint64_t)(k16 * 16), id3, k16 > 0);
                     } else if (kind == R_F1) {
 #pragma unroll
                         for (int k16 = 0; k16 < kR / 16; ++k16) umma_ts(tb, tb + kColGf + 8 * k16, dW1 + (uint64_t)(k16 * 16), id128, k16 > 0);
@@ -336,12 +348,22 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
             load_record(0);
             for (int t = 0; t < ntiles; ++t) {
                 TRACE(1);
+                // TMA: the tile's 128 rows of 512 B by 128 gather4 copies (4 edges x 128 B each): the thread of every fourth edge
+                // issues the two segments its part consumes (part p: segments p and 2 + p = channel halves o = 0, 1); a gather4
+                // costs its issuing warp ~90 cycles, so they too are issued under the first two round trips
+                [[maybe_unused]] const int j1 = TMA ? __shfl_down_sync(0xffffffffu, jrow_n, 1) : 0, j2 = TMA ? __shfl_down_sync(0xffffffffu, jrow_n, 2) : 0,
+                                           j3 = TMA ? __shfl_down_sync(0xffffffffu, jrow_n, 3) : 0;
+                auto tma_half = [&](int o) {
+                    if ((e & 3) == 0) tma_gather4(sStage + (uint32_t)((2 * o + part) * (kTT * 128) + e * 128), a.ym_tmap, (2 * o + part) * 64, jrow_n, j1, j2, j3, gbar);
+                };
+                if constexpr (TMA) { if (tt == 0) mbar_expect_tx(gbar, (uint32_t)(kTT * 512)); }
                 // first contraction first: its round trip runs under the issue of this tile's gathers
                 stage_basis(r_n);
                 TRACE(2);
                 publish(BWD ? R_G1H0 : R_F1);
                 TRACE(3);
-                issue_gathers(jrow_n, 0, BWD ? NGRP / 2 : NGRP);   // bwd: the rows' first channel half (the second: under the next round trip)
+                if constexpr (TMA) tma_half(0);
+                else issue_gathers(jrow_n, 0, BWD ? NGRP / 2 : NGRP);   // bwd: the rows' first channel half (the second: under the next round trip)
                 if (part == 0) {                                   // cutoff (slope, unit vector) of the slot: asynchronous 4-byte copies, read at the tile's end
                     const uint32_t d = smem_u32(recS) + (uint32_t)e * 4;
                     cp_async4(d, rp_n + LSD_REC_FC * 16);
@@ -385,13 +407,14 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         tmem_wait_st();
                         TRACE(6);
                         publish(h == 0 ? R_G1H1 : R_G2O0);
-                        if (h == 0) { issue_gathers(jrow_n, NGRP / 2, NGRP); cp_async_commit(); }
+                        if (h == 0) { if constexpr (TMA) tma_half(1); else { issue_gathers(jrow_n, NGRP / 2, NGRP); cp_async_commit(); } }
                     }
                     TRACE(7);
                     // ---- epilogue of output half o: P = bf16(lin) . mbar_j (in place), A = sum_f c_f lin'_f, B = sum_f c_f lin_f,
                     //      c = mbar_a y_j + mbar_j y_a (bf16 pairs)
                     asm volatile("cp.async.wait_group 0;" ::: "memory");
                     __syncwarp();
+                    if constexpr (TMA) { mbar_wait(gbar, gph); gph ^= 1u; }
                     f32x2 A2 = 0, B2 = 0;
                     const int gl_t = t * kGPT + my_g;
                     const int at = gl_t < G ? (int)gatom[gl_t] : -1;
@@ -412,8 +435,11 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
 #pragma unroll
                             for (int q8 = 0; q8 < 2; ++q8) {       // 8 channels = two stage cells -> one P cell
                                 const int slab = (ch0 + c0 + 8 * q8) >> 2;
-                                const uint4 s0v = *reinterpret_cast<const uint4*>(stage + slab * kSlab + e * 16);
-                                const uint4 s1v = *reinterpret_cast<const uint4*>(stage + (slab + 1) * kSlab + e * 16);
+                                // TMA: row e of segment 2 o + part, 16-byte chunks s and s + 1 (swizzled by the row)
+                                const int sseg = (c0 + 8 * q8) >> 2;
+                                const uint8_t* const srow = stage + (2 * o + part) * (kTT * 128) + e * 128;
+                                const uint4 s0v = *reinterpret_cast<const uint4*>(TMA ? srow + ((sseg ^ (e & 7)) << 4) : stage + slab * kSlab + e * 16);
+                                const uint4 s1v = *reinterpret_cast<const uint4*>(TMA ? srow + (((sseg + 1) ^ (e & 7)) << 4) : stage + (slab + 1) * kSlab + e * 16);
                                 const uint4 o0v = *reinterpret_cast<const uint4*>(ownrow + slab * 16);
                                 const uint4 o1v = *reinterpret_cast<const uint4*>(ownrow + (slab + 1) * 16);
                                 const uint32_t yj[4] = {s0v.x, s0v.z, s1v.x, s1v.z}, mj[4] = {s0v.y, s0v.w, s1v.y, s1v.w};
@@ -427,7 +453,11 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                                     B2 = fma2(cf, pk2u(v[c], v[c + 1]), B2);
                                     pw[i] = bmul2(pack_bf16(__uint_as_float(v[c]), __uint_as_float(v[c + 1])), mj[i]);
                                 }
-                                if (need_sum) *reinterpret_cast<uint4*>(stage + slab * kSlab + e * 16) = make_uint4(pw[0], pw[1], pw[2], pw[3]);
+                                // P cell of these 8 channels: in place (TMA: chunk 4 o + .. of the part's atom = region `part`, whose
+                                // chunks this thread has consumed already: o = 0 reads region `part` itself, ahead of the writes)
+                                uint8_t* const pcell = TMA ? stage + part * (kTT * 128) + e * 128 + (((4 * o + ((c0 + 8 * q8) >> 3)) ^ (e & 7)) << 4)
+                                                           : stage + slab * kSlab + e * 16;
+                                if (need_sum) *reinterpret_cast<uint4*>(pcell) = make_uint4(pw[0], pw[1], pw[2], pw[3]);
                             }
                         }
                         TRACE(10);
@@ -552,7 +582,9 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         const int at = part * NA + i;
                         if (at < natoms2) {
                             const __nv_bfloat16 pb = __float2bfloat16_rn(acc[i]);
-                            out16[(size_t)(g02 + at) * kF + e] = *reinterpret_cast<const uint16_t*>(&pb);
+                            // TMA: contraction row e = 64 part + 8 chunk + i holds channel 64 (chunk >> 2) + 32 part + 8 (chunk & 3) + i
+                            const int ch = TMA ? 64 * ((e >> 5) & 1) + 32 * (e >> 6) + (e & 31) : e;
+                            out16[(size_t)(g02 + at) * kF + ch] = *reinterpret_cast<const uint16_t*>(&pb);
                         }
                     }
                 }
@@ -572,6 +604,25 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
 }
 
+}  // namespace
+
+// TMA tensor map over rows of `row_bytes` bytes of 16-bit elements: boxes of 64 elements (128 B) x 1 row (what tile::gather4
+// takes), 128-byte swizzle.  The driver entry point is looked up through the runtime (no link against libcuda).
+bool lsd_encode_row_tmap(void* host_map_128B, const void* base, size_t rows, int row_bytes)
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                 const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
+    EncodeFn enc = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &q) != cudaSuccess || enc == nullptr) { cudaGetLastError(); return false; }
+    const cuuint64_t dims[2] = {(cuuint64_t)(row_bytes / 2), (cuuint64_t)rows}, strides[1] = {(cuuint64_t)row_bytes};
+    const cuuint32_t box[2] = {64, 1}, es[2] = {1, 1};
+    return enc(reinterpret_cast<CUtensorMap*>(host_map_128B), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+namespace {
 int device_sm_count()
 {
     int dev = 0, sms = 0;
@@ -580,10 +631,10 @@ int device_sm_count()
     return sms > 0 ? sms : 148;
 }
 
-template <bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
+template <bool BWD, int SPLIT, bool TMA = false> void launch_rows(Launcher L, const EdgeArgs& a)
 {
     constexpr int threads = kTeams * kTT * SPLIT;
-    cudaFuncSetAttribute(k_edge_rows<BWD, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lay<BWD>::Smem);
+    cudaFuncSetAttribute(k_edge_rows<BWD, SPLIT, TMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lay<BWD, TMA>::Smem);
     const int cps = (a.n + kCH - 1) / kCH;
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(device_sm_count(), (nchunks + kTeams - 1) / kTeams));
@@ -593,7 +644,7 @@ template <bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
         unsigned long long* dbuf = nullptr;
         cudaMalloc(&dbuf, 2048 * 8); cudaMemsetAsync(dbuf, 0, 2048 * 8, L.s);
         EdgeArgs at = a; at.trace = dbuf;
-        k_edge_rows<BWD, SPLIT><<<grid, threads, Lay<BWD>::Smem, L.s>>>(at, cps, nchunks);
+        k_edge_rows<BWD, SPLIT, TMA><<<grid, threads, Lay<BWD, TMA>::Smem, L.s>>>(at, cps, nchunks);
         cudaStreamSynchronize(L.s);
         std::vector<unsigned long long> h(2048);
         cudaMemcpy(h.data(), dbuf, 2048 * 8, cudaMemcpyDeviceToHost); cudaFree(dbuf);
@@ -610,8 +661,8 @@ template <bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
         LSD_COUNT(L);
         return;
     }
-    k_edge_rows<BWD, SPLIT><<<grid, threads, Lay<BWD>::Smem, L.s>>>(a, cps, nchunks);
-    note_edge_launch(BWD, 4, kCH, threads, grid, kF);
+    k_edge_rows<BWD, SPLIT, TMA><<<grid, threads, Lay<BWD, TMA>::Smem, L.s>>>(a, cps, nchunks);
+    note_edge_launch(BWD, TMA ? 9 : 4, kCH, threads, grid, kF);
     LSD_COUNT(L);
 }
 
@@ -621,6 +672,9 @@ template <bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward)
 {
     static const int split = [] { const char* v = getenv("LSD_EDGE_SPLIT"); return (v && v[0] == '1') ? 1 : 2; }();
+    // LSD_EDGE_TMA: the backward gathers its rows with TMA gather4 (needs the tensor map of alloc_work)
+    static const bool tma = [] { const char* v = getenv("LSD_EDGE_TMA"); return v != nullptr && v[0] != '0'; }();
+    if (backward && split == 2 && tma && a.ym_tmap) { launch_rows<true, 2, true>(L, a); return; }
     if (backward) { if (split == 2) launch_rows<true, 2>(L, a); else launch_rows<true, 1>(L, a); }
     else { if (split == 2) launch_rows<false, 2>(L, a); else launch_rows<false, 1>(L, a); }
 }

@@ -37,6 +37,18 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo, uint
     d |= (uint64_t)1 << 46;
     return d;
 }
+// the same for the 128-byte swizzled canonical layouts (rows of 128 bytes, 16-byte chunk c of row r stored at chunk c ^ (r & 7);
+// what a TMA tensor map with CU_TENSOR_MAP_SWIZZLE_128B writes); the buffer is 1024-byte aligned
+__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    return make_desc(saddr, lbo, sbo) | ((uint64_t)2 << 61);
+}
+// TMA gather: four rows (r0..r3) x one box of columns starting at `col` of a 2-D tensor map -> four consecutive box rows at dst
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const void* tmap, int col, int r0, int r1, int r2, int r3, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cta.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+                 ::"r"(dst), "l"(tmap), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3), "r"(bar) : "memory");
+}
 // instruction descriptor, kind::f16: D = fp32, A = B = bf16, A K-major, B K-major or MN-major, M x N
 __device__ __forceinline__ uint32_t make_idesc(int M, int N, int b_mn_major)
 {
