@@ -234,7 +234,8 @@ k_compact(int n, int B, BoxC box, const double* __restrict__ q, const int* __res
                     }
                     float* o = recs + lsd_rec_index((size_t)warp, cap, pos, 0);
                     o[LSD_REC_R * 16] = rf; o[LSD_REC_FC * 16] = fc; o[LSD_REC_FCP * 16] = fcp;
-                    o[LSD_REC_UX * 16] = (float)(d[0] / rd); o[LSD_REC_UY * 16] = (float)(d[1] / rd); o[LSD_REC_UZ * 16] = (float)(d[2] / rd);
+                    const double rinv = 1.0 / rd;                           // one fp64 division per edge; the unit vector is rounded to fp32
+                    o[LSD_REC_UX * 16] = (float)(d[0] * rinv); o[LSD_REC_UY * 16] = (float)(d[1] * rinv); o[LSD_REC_UZ * 16] = (float)(d[2] * rinv);
                     o[LSD_REC_JROW * 16] = __int_as_float(b * n + j);
                 }
             }
