@@ -23,8 +23,9 @@ using namespace tcp;
 
 constexpr int kR = LSD_NRBF;
 // teams per SM: the width-32 kernels are pure round-trip latency (2 teams of 4 warps are as fast as 2 teams of 8), so they run 4
-// teams of ONE thread per edge in 128 TMEM columns each; width 64 keeps 2 teams of two threads per edge in 256 columns
-template <int F> struct Teams { static constexpr int N = F == 32 ? 4 : 2; };
+// teams of ONE thread per edge in 128 TMEM columns each; so does the width-64 FORWARD (D 64 + A2 32 + G 16 + D3 16 = 128 columns);
+// the width-64 backward (192 columns) keeps 2 teams of two threads per edge
+template <int F, bool BWD> struct Teams { static constexpr int N = (F == 32 || !BWD) ? 4 : 2; };
 constexpr int kTT = 128;                               // edge slots of a tile
 constexpr int kCH = 16;                                // atoms per chunk = columns of D3
 constexpr int kGE = 16;                                // edge slots per record group
@@ -38,7 +39,7 @@ constexpr int kSTBytes = kCH * kTT * 2;
 // keeps its full size (the unused cells stay zero) and the accumulator lanes >= F are ignored.
 template <int F, bool BWD> struct Lay {
     static constexpr int NSLAB = BWD ? F / 4 : F / 8;  // 16-byte pieces of a gathered row (bwd: 4 channels x (y, y, mbar, mbar); fwd: 8 channels)
-    static constexpr int kTeams = Teams<F>::N;
+    static constexpr int kTeams = Teams<F, BWD>::N;
     static constexpr int NSLAB_READ = BWD ? 32 : 16;   // slabs the segment-sum contraction reads (128 operand rows whatever the width)
     // The stages of all teams come first, the other team buffers behind them.  Width 64 keeps full-size stages.  Width 32 has
     // room for 4 teams only with stages of the slabs it uses: the contraction then reads on past a stage into the stages and
@@ -69,7 +70,7 @@ constexpr float kP0 = -0.49872449040412903f, kP1 = 0.2356506735086441f, kP2 = -0
 //                                  fwd D 0..31, A2 32..47, G 48..63, D3 64..79
 template <int F> struct Cols {
     static constexpr uint32_t A2v = F == 32 ? 64 : 128, A2t = F == 32 ? 80 : 192, Gb = F == 32 ? 96 : 160, Gtb = F == 32 ? 112 : 224;
-    static constexpr uint32_t A2f = F == 32 ? 32 : 128, Gf = F == 32 ? 48 : 192, D3f = F == 32 ? 64 : 208;
+    static constexpr uint32_t A2f = F == 32 ? 32 : 64, Gf = F == 32 ? 48 : 96, D3f = F == 32 ? 64 : 112;   // width 64 fwd: D 0..63, A2 64..95, G 96..111, D3 112..127
 };
 
 template <int TT> __device__ __forceinline__ void team_bar(int team) { asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(TT) : "memory"); }
@@ -96,17 +97,17 @@ __device__ __forceinline__ void act_pair(uint32_t h0u, uint32_t h1u, uint32_t hp
 }
 
 template <int F, bool BWD, int SPLIT>
-__global__ void __launch_bounds__(Teams<F>::N * kTT * SPLIT, 1)
+__global__ void __launch_bounds__(Teams<F, BWD>::N * kTT * SPLIT, 1)
 k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
 {
     using L = Lay<F, BWD>;
     constexpr int kF = F, HC = F >= 64 ? 64 : F, NH = F / HC;      // channels per contraction round, rounds per layer
     constexpr int kW1Bytes = L::W1Bytes, kW2Bytes = L::W2Bytes;
-    constexpr int kTeams = Teams<F>::N;
+    constexpr int kTeams = Teams<F, BWD>::N;
     constexpr uint32_t kColA2v = BWD ? Cols<F>::A2v : Cols<F>::A2f, kColA2t = Cols<F>::A2t, kColGb = Cols<F>::Gb, kColGtb = Cols<F>::Gtb,
                        kColGf = Cols<F>::Gf, kColD3f = Cols<F>::D3f;
     static_assert(F == 64 || F == 32, "narrow widths");
-    static_assert((F == 32 && SPLIT == 1) || (F == 64 && SPLIT == 2), "width 32: one thread per edge, width 64: two");
+    static_assert((F == 32 && SPLIT == 1) || (F == 64 && SPLIT == (BWD ? 2 : 1)), "one thread per edge, the width-64 backward: two");
     constexpr int TT = kTT * SPLIT;                    // threads of a team
     constexpr int TW = TT / 32;                        // warps of a team
     constexpr int kThreads = kTeams * TT;
@@ -605,7 +606,7 @@ int device_sm_count()
 
 template <int F, bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArgs& a)
 {
-    constexpr int kTeams = Teams<F>::N;
+    constexpr int kTeams = Teams<F, BWD>::N;
     constexpr int threads = kTeams * kTT * SPLIT;
     cudaFuncSetAttribute(k_edge_rows<F, BWD, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lay<F, BWD>::Smem);
     const int cps = (a.n + kCH - 1) / kCH;
@@ -646,6 +647,6 @@ template <int F, bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArg
 // rows (a.m_out / a.ybar) for the fp32 atom-wise layers of that path
 void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward)
 {
-    if (F == 64) { if (backward) launch_rows<64, true, 2>(L, a); else launch_rows<64, false, 2>(L, a); }
+    if (F == 64) { if (backward) launch_rows<64, true, 2>(L, a); else launch_rows<64, false, 1>(L, a); }
     else if (F == 32) { if (backward) launch_rows<32, true, 1>(L, a); else launch_rows<32, false, 1>(L, a); }
 }
