@@ -1,13 +1,15 @@
 // bf16 tcgen05 filter path for the NARROW widths F = 32 and F = 64 (cfg3's target, the draft networks of cfg4 / cfg5): the
 // edges-as-rows kernel of mlip_edge_rows.cu in its width-generic form (M5, M9, section 4.1).  Same tile algebra -- a tile
 // is 128 edge slots, TMEM lane = edge, radial basis and activations are A operands in tensor memory, the gathered neighbour rows
-// sit in a slab-layout stage that the segment-sum operand P overwrites in place, D3 = P^T S -- with ONE contraction round per
-// layer instead of two channel halves (HC = min(F, 64) channels per round: three round trips per tile in the backward pass), and
-// the per-atom sums written as fp32 rows for the fp32 atom-wise layers of this path.  The segment-sum contraction always
-// reads 128 operand rows, so the stage keeps its full size (unused cells stay zero) and accumulator lanes >= F are ignored.
+// sit in a slab-layout stage that the segment-sum operand P overwrites in place, D3 = P^T S -- with the contraction rounds cut
+// so that a team fits 128 tensor-memory columns and FOUR teams of one thread per edge share the SM (these kernels are bound by
+// the latency of a team's round trips, so tiles in flight are the lever): one round per layer at width 32 and in the width-64
+// forward, channel halves of 32 in the width-64 backward; the per-atom sums go out as fp32 rows for the fp32 atom-wise
+// layers of this path.  The segment-sum contraction always reads 128 operand rows: past the slabs a stage holds it reads on
+// into allocated shared memory whose contents land in accumulator lanes >= F, which are ignored.
 // Replaces k_edge_tc (mlip_tc.cu: channels are rows, 64 edges per tile and three round trips) for these widths:
-// cfg3 bf16 window 2.45 -> 2.00 ms, draft network at cfg5 7.5 -> 6.1 ms per window (4.35 ms with the four teams of width 32,
-// below); LSD_EDGE_NARROW=0 selects k_edge_tc.
+// cfg3 bf16 window 2.45 -> 2.00 ms (1.43 ms with four teams), draft network at cfg5 7.5 -> 6.1 ms per window (4.35 ms with four
+// teams); LSD_EDGE_NARROW=0 selects k_edge_tc.
 // The width-128 instantiation lives in mlip_edge_rows.cu: generated from this generic source the dominant kernel came out
 // 2.3 % slower (44.6 vs 43.6 ms per cfg5 window, same instruction counts in the tile loop), so its tuned translation unit is kept.
 // Determinism / batch invariance: as in mlip_edge_rows.cu.
@@ -24,8 +26,8 @@ using namespace tcp;
 constexpr int kR = LSD_NRBF;
 // teams per SM: the width-32 kernels are pure round-trip latency (2 teams of 4 warps are as fast as 2 teams of 8), so they run 4
 // teams of ONE thread per edge in 128 TMEM columns each; so does the width-64 FORWARD (D 64 + A2 32 + G 16 + D3 16 = 128 columns);
-// the width-64 backward (192 columns) keeps 2 teams of two threads per edge
-template <int F, bool BWD> struct Teams { static constexpr int N = (F == 32 || !BWD) ? 4 : 2; };
+// the width-64 backward runs its contractions as channel halves of 32 to fit them too (D 32 + 32, A2v 32, A2t 32)
+template <int F, bool BWD> struct Teams { static constexpr int N = 4; };
 constexpr int kTT = 128;                               // edge slots of a tile
 constexpr int kCH = 16;                                // atoms per chunk = columns of D3
 constexpr int kGE = 16;                                // edge slots per record group
@@ -44,7 +46,7 @@ template <int F, bool BWD> struct Lay {
     // The stages of all teams come first, the other team buffers behind them.  Width 64 keeps full-size stages.  Width 32 has
     // room for 4 teams only with stages of the slabs it uses: the contraction then reads on past a stage into the stages and
     // buffers behind it -- allocated shared memory (asserted below) whose contents land in accumulator lanes >= F, which are ignored.
-    static constexpr int NSLAB_ALLOC = F == 32 ? NSLAB : NSLAB_READ;
+    static constexpr int NSLAB_ALLOC = (F == 32 || BWD) ? NSLAB : NSLAB_READ;
     static constexpr int StageBytes = ((NSLAB_ALLOC * kSlab + 127) / 128) * 128;
     static constexpr int OwnBytes = BWD ? kCH * 4 * F : 0;
     static constexpr int W1Bytes = F * kR * 2, W2Bytes = F * F * 2;
@@ -69,7 +71,8 @@ constexpr float kP0 = -0.49872449040412903f, kP1 = 0.2356506735086441f, kP2 = -0
 // width 32 (128 columns per team): bwd D = [Dv 0..31 | Dt 32..63], A2v 64..79, A2t 80..95, G 96..111, G' 112..127;
 //                                  fwd D 0..31, A2 32..47, G 48..63, D3 64..79
 template <int F> struct Cols {
-    static constexpr uint32_t A2v = F == 32 ? 64 : 128, A2t = F == 32 ? 80 : 192, Gb = F == 32 ? 96 : 160, Gtb = F == 32 ? 112 : 224;
+    // width 64 bwd (halves of 32): D = [Dv 0..31 | Dt 32..63], A2v 64..95, A2t 96..127, G / G' alias their second halves (80.., 112..)
+    static constexpr uint32_t A2v = 64, A2t = F == 32 ? 80 : 96, Gb = F == 32 ? 96 : 80, Gtb = 112;
     static constexpr uint32_t A2f = F == 32 ? 32 : 64, Gf = F == 32 ? 48 : 96, D3f = F == 32 ? 64 : 112;   // width 64 fwd: D 0..63, A2 64..95, G 96..111, D3 112..127
 };
 
@@ -101,13 +104,13 @@ __global__ void __launch_bounds__(Teams<F, BWD>::N * kTT * SPLIT, 1)
 k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
 {
     using L = Lay<F, BWD>;
-    constexpr int kF = F, HC = F >= 64 ? 64 : F, NH = F / HC;      // channels per contraction round, rounds per layer
+    constexpr int kF = F, HC = (F == 64 && BWD) ? 32 : (F >= 64 ? 64 : F), NH = F / HC;   // channels per contraction round, rounds per layer
     constexpr int kW1Bytes = L::W1Bytes, kW2Bytes = L::W2Bytes;
     constexpr int kTeams = Teams<F, BWD>::N;
     constexpr uint32_t kColA2v = BWD ? Cols<F>::A2v : Cols<F>::A2f, kColA2t = Cols<F>::A2t, kColGb = Cols<F>::Gb, kColGtb = Cols<F>::Gtb,
                        kColGf = Cols<F>::Gf, kColD3f = Cols<F>::D3f;
     static_assert(F == 64 || F == 32, "narrow widths");
-    static_assert((F == 32 && SPLIT == 1) || (F == 64 && SPLIT == (BWD ? 2 : 1)), "one thread per edge, the width-64 backward: two");
+    static_assert(SPLIT == 1, "four teams of one thread per edge");
     constexpr int TT = kTT * SPLIT;                    // threads of a team
     constexpr int TW = TT / 32;                        // warps of a team
     constexpr int kThreads = kTeams * TT;
@@ -194,7 +197,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         const int h = kind - R_G1H0;
 #pragma unroll
                         for (int k16 = 0; k16 < kR / 16; ++k16) {
-                            const uint64_t db = dW1 + (uint64_t)((h * 4096 + k16 * 256) >> 4);
+                            const uint64_t db = dW1 + (uint64_t)((h * HC * 64 + k16 * 256) >> 4);      // HC rows = HC / 8 groups of 512 bytes
                             umma_ts(tb, tb + kColGb + 8 * k16, db, id64, k16 > 0);
                             umma_ts(tb + HC, tb + kColGtb + 8 * k16, db, id64, k16 > 0);
                         }
@@ -202,7 +205,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                         const int o = kind - R_G2O0;
 #pragma unroll
                         for (int k16 = 0; k16 < kF / 16; ++k16) {
-                            const uint64_t db = dW2 + (uint64_t)((o * 128 * F + k16 * 256) >> 4);       // 64 output rows = 8 groups of F * 16 bytes
+                            const uint64_t db = dW2 + (uint64_t)((o * HC * 2 * F + k16 * 256) >> 4);   // HC output rows = HC / 8 groups of F * 16 bytes
                             umma_ts(tb, tb + kColA2v + 8 * k16, db, id64, k16 > 0);
                             umma_ts(tb + HC, tb + kColA2t + 8 * k16, db, id64, k16 > 0);
                         }
@@ -647,6 +650,6 @@ template <int F, bool BWD, int SPLIT> void launch_rows(Launcher L, const EdgeArg
 // rows (a.m_out / a.ybar) for the fp32 atom-wise layers of that path
 void launch_edge_rows_narrow(Launcher L, const EdgeArgs& a, int F, bool backward)
 {
-    if (F == 64) { if (backward) launch_rows<64, true, 2>(L, a); else launch_rows<64, false, 1>(L, a); }
+    if (F == 64) { if (backward) launch_rows<64, true, 1>(L, a); else launch_rows<64, false, 1>(L, a); }
     else if (F == 32) { if (backward) launch_rows<32, true, 1>(L, a); else launch_rows<32, false, 1>(L, a); }
 }
