@@ -254,7 +254,7 @@ k_edge_fwd4(EdgeArgs a, int chunks_per_state, int nchunks)
                         *reinterpret_cast<uint4*>(cell) = p;
                     }
                 }
-                if (o == 0) { fence_async_smem(); publish(R_G2O1); }
+                if (o == 0) publish(R_G2O1);                           // (P becomes visible to the contraction by the fence before G3)
             }
             uint16_t* const st_e = reinterpret_cast<uint16_t*>(ST + ((at >= 0 ? at : 0) >> 3) * 2048 + (e >> 3) * 128 + ((at >= 0 ? at : 0) & 7) * 16 + (e & 7) * 2);
             if (at >= 0) {                                         // S^T[e][at] = fc

@@ -461,7 +461,7 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
                             }
                         }
                         TRACE(10);
-                        if (o == 0) { if (need_sum) fence_async_smem(); publish(R_G2O1); }
+                        if (o == 0) publish(R_G2O1);                   // (P becomes visible to the contraction by the fence before G3)
                     }
                     // ---- force term of the edge, summed over the 16 edges of its group
                     float Al, Ah, Bl, Bh;
