@@ -275,6 +275,45 @@ int32_t     lsd_tc_enabled(const lsd_ctx* ctx);
  * one-block network; the environment variable LSD_TINY=0, read by lsd_init, turns it off (A/B measurements). */
 int32_t     lsd_tiny_rollout_enabled(const lsd_ctx* ctx);
 
+/* ---- The one entry point that allocates nothing ----------------------------------------------------------------------------
+ * lsd_transport_window_noalloc: steps a3 + a4 (PAPER.md:108-111 Eq. 8 REFLECTIONVERIFY, :424 l = min{j : x_j != y_j}) for a window
+ * whose draft and target forces the caller already holds in device memory.  No context, and no cudaMalloc / cudaFree / other
+ * allocating call, ever.
+ *
+ * It exists for callers that are not allowed to allocate GPU memory: a host program (an MD engine, a PyTorch job) whose own
+ * pool already owns almost all of the device, so that a cudaMalloc made by this library would fail or fragment the pool; and a
+ * force / acceptance callback inside another program's step loop, where the device-wide synchronisation that cudaMalloc and
+ * cudaFree imply would stall that program's other streams.  Every other call of this header needs an lsd_ctx, and lsd_init
+ * allocates.
+ *
+ * The per-block partial sums of S1 and S2 go to a fixed array inside the library (151,552 bytes of device memory, held by every
+ * GPU that has loaded liblsd_b200.so until the process exits).  Its size sets the limits: K <= LSD_NOALLOC_MAX_K and
+ * n_atoms <= LSD_NOALLOC_MAX_ATOMS; anything larger is refused with LSD_ERR_INVALID_ARG and a message, nothing is launched.
+ *
+ *   inputs  (DEVICE, caller-owned): mass_amu [n_atoms]; F_draft, F_target [K][3][n_atoms] fp64 (F~_j and F_j at q_half_j, eV/A).
+ *           seed and n0 key the noise exactly as in the context path: step j (1..K) uses xi = Philox(seed; n0 + j, atom) and
+ *           u_j = Philox(seed; n0 + j) (R5), n0 = committed step index of the window's start state.
+ *   outputs (DEVICE, caller-owned): stats [4][K] = S1 | S2 | ell | ln u;  reject [K] (1 = step rejected);
+ *           verdict [3] = {first_reject l (0: none), n_commit (l, or K), 1 if S1 or S2 of a committed step is not finite}.
+ *           The override of step l (a5) is not part of this call.
+ *   The arithmetic, reduction order and block decomposition are those of lsd_transport_accept, so with the same forces, seed
+ *   and n0 the numbers agree with lsd_get_window_debug(S1 / S2 / ELL / LNU / REJECT).
+ *
+ * Asynchronous on `stream`; nothing is synchronised.  The FIRST call on each device also looks up the device address of the
+ * array (once per device, with that device current): make that first call before you begin any stream capture.
+ * All calls on a device share the array, and it keeps what the last call wrote.  Nothing in it needs to start at zero (each
+ * call overwrites every slot it later reads), so calls that follow each other on one stream, or are otherwise ordered, are safe;
+ * two calls that may run on the GPU at the same time (different streams, different host threads, no ordering) race on it and
+ * give wrong sums.  Serialise them.
+ * Errors: INVALID_ARG (sizes beyond the limits, non-positive T / friction / dt, null or non-device pointers), CUDA (launch or
+ * address look-up failed).  The message is returned by lsd_noalloc_last_error() (per host thread). */
+#define LSD_NOALLOC_MAX_K      64
+#define LSD_NOALLOC_MAX_ATOMS  (1 << 28)
+lsd_status lsd_transport_window_noalloc(int32_t n_atoms, int32_t K, uint64_t seed, uint64_t n0, double temperature_K,
+                                        double friction_per_fs, double dt_fs, const double* mass_amu, const double* F_draft,
+                                        const double* F_target, double* stats, int32_t* reject, int32_t* verdict, void* stream);
+const char* lsd_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_roll
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
                     "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k",
                     "lsd_get_window_obabo", "lsd_get_edge_launch_info", "lsd_measure_fma_peak", "lsd_set_force_slack", "lsd_tiny_rollout_enabled", "lsd_set_window_slots",
-                    "lsd_measure_tmem_bandwidth", "lsd_measure_half_list_delivery"]
+                    "lsd_measure_tmem_bandwidth", "lsd_measure_half_list_delivery", "lsd_transport_window_noalloc", "lsd_noalloc_last_error"]
 
 
 class LsdError(RuntimeError):
@@ -79,6 +79,8 @@ def load_library():
         L.lsd_launch_count.argtypes = [C.c_void_p]
         L.lsd_destroy.restype = None
         L.lsd_destroy.argtypes = [C.c_void_p]
+        L.lsd_noalloc_last_error.restype = C.c_char_p
+        L.lsd_noalloc_last_error.argtypes = []
         _lib = L
     return _lib
 
@@ -310,6 +312,29 @@ def lsd_measure_half_list_delivery(n_atoms: int, n_states: int, rows_per_atom: i
     _check(None, load_library().lsd_measure_half_list_delivery(C.c_int32(n_atoms), C.c_int32(n_states), C.c_int32(rows_per_atom), _stream(stream),
                                                                C.byref(a), C.byref(b)))
     return float(a.value), float(b.value)
+
+
+LSD_NOALLOC_MAX_K, LSD_NOALLOC_MAX_ATOMS = 64, 1 << 28
+
+
+def lsd_transport_window_noalloc(n_atoms, K, seed, n0, temperature_K, friction_per_fs, dt_fs, mass_amu, F_draft, F_target,
+                                 stats, reject, verdict, stream=None):
+    """Accept / reject decisions of one drafted window from forces already on the device, for callers that must not allocate
+    GPU memory (a host program whose pool owns the device; a callback that may not trigger cudaMalloc's device-wide
+    synchronisation): see include/lsd.h.  Every array is a CUDA tensor the caller owns: mass_amu [n] f64, F_draft / F_target
+    [K][3][n] f64 in, stats [4][K] f64 (S1 | S2 | ell | ln u), reject [K] i32, verdict [3] i32 out.  Asynchronous on `stream`;
+    calls that may overlap on the GPU race on the library's fixed scratch array.  This wrapper allocates nothing either."""
+    ptrs = []
+    for a in (mass_amu, F_draft, F_target, stats, reject, verdict):
+        ptr, where = _ptr(a)
+        if where != LSD_DEVICE:
+            raise LsdError(-1, "lsd_transport_window_noalloc takes device (CUDA) tensors only")
+        ptrs.append(ptr)
+    L = load_library()
+    st = L.lsd_transport_window_noalloc(C.c_int32(n_atoms), C.c_int32(K), C.c_uint64(seed), C.c_uint64(n0), C.c_double(temperature_K),
+                                        C.c_double(friction_per_fs), C.c_double(dt_fs), *ptrs, _stream(stream))
+    if st != 0:
+        raise LsdError(st, L.lsd_noalloc_last_error().decode())
 
 
 def lsd_tc_enabled(h) -> bool:
