@@ -163,12 +163,17 @@ int32_t lsd_get_adaptive_k(const lsd_ctx* ctx);
 /* Plain Langevin dynamics (no speculation): n_steps ABOBA steps (Eq. 2) with the forces of potential `which`
  * (LSD_TARGET: the serial baseline in the paper's definition of speed-up; LSD_DRAFT: the draft alone) from
  * the base state, same kernels and same noise keying as the draft rollout (R5), committed in chunks of k_max steps that
- * share one neighbour list; synchronises once per chunk.  With `which` = LSD_TARGET the trajectory equals LSD with
+ * share one neighbour list; synchronises once per chunk and before it returns (`stream` may be destroyed afterwards).  With `which` = LSD_TARGET the trajectory equals LSD with
  * draft = target.  A skin violation or row overflow inside a chunk is answered like in lsd_run (lists rebuilt with a larger
  * skin, chunk repeated).  Errors: STATE (a drafted window is pending), NONFINITE (the base state is the last good one). */
 lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void* stream);
 
-/* Base state x_n: q, p [3][n_atoms] (either may be NULL), *step = n.  Synchronises. */
+/* Base state x_n: q, p [3][n_atoms] (either may be NULL), *step = n.
+ * where = LSD_DEVICE (caller-owned device buffers): both calls synchronise the WHOLE device first, so the copy is ordered after
+ * every kernel of the caller that produces (set) or still reads (get) the buffers, whatever stream it runs on, and is complete
+ * on return.  where = LSD_HOST: lsd_get_state waits for this context's own work and returns with q, p filled.  lsd_set_state
+ * copies the caller's arrays before it returns (they may be re-used at once); for small systems the upload itself is only
+ * enqueued, and every later call of this context that reads the state waits for it. */
 lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int32_t where);
 lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t step, int32_t where);
 lsd_status lsd_get_stats(const lsd_ctx* ctx, lsd_stats* out);
@@ -180,7 +185,9 @@ lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, i
  * staggering (App. F :632-753): q = q_half_j (:753), p = p_mid of Eq. 30 from the committed
  * momenta before and after the step, the target force F_j already evaluated by the verification (no force call) and one
  * extra normal per component drawn from Philox stream tag 3 at step index n0 + j (R18).  Valid until the next
- * lsd_verify_window (it overwrites F).  q, p: [3][n_atoms] or NULL; `where` = LSD_HOST | LSD_DEVICE.  Synchronises. */
+ * lsd_verify_window (it overwrites F).  q, p: [3][n_atoms] or NULL; `where` = LSD_HOST | LSD_DEVICE.  Synchronises.
+ * Errors: STATE (no window transported yet; or force slack is on: the committed kicks then used F_(eps), which is not kept,
+ * so Eq. 30 cannot be evaluated consistently -- switch slack off first), INVALID_ARG (j). */
 lsd_status lsd_get_window_obabo(lsd_ctx* ctx, int32_t j, double* q, double* p, int32_t where);
 
 /* Speculative error correction, EC (App. E :626-630; Alg. 3 :663-717), window form:
@@ -225,7 +232,9 @@ lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const 
 /* Effective directed edge set of state b of the last lsd_eval_forces / lsd_verify_window call
  * (T1): kind 0 = network list (r < r_c), 1 = pair-prior list (r < r_c(s_i, s_j)).
  * Host outputs: start[n_atoms + 1], idx[cap], shifts[cap][3]; *n_edges = total (may exceed cap, then
- * only cap entries are written).  Rows are sorted by (j, shift).  Synchronises. */
+ * only cap entries are written).  Rows are sorted by (j, shift).  Synchronises.  Errors: STATE (no evaluation yet; or
+ * which = LSD_DRAFT in a context with the one-kernel tiny rollout and no lsd_eval_forces(LSD_DRAFT) since the last rollout:
+ * that rollout keeps its neighbour rows on chip). */
 lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t b, int64_t cap,
                              int64_t* start, int32_t* idx, int8_t* shifts, int64_t* n_edges);
 
@@ -264,8 +273,9 @@ int64_t     lsd_launch_count(const lsd_ctx* ctx);
 const char* lsd_version(void);
 /* Which tcgen05 edge kernel the last MLIP edge launch of this process used, pass 0 = forward (M5), 1 = backward (M9); parity
  * tests use it to assert that the instantiation they compared with the oracle is the one the benchmark times.
- * out[5] = {kernel (1 k_edge_tc, 2 k_edge_tc128, 3 k_edge_er128_fwd, 4 k_edge_rows, 5 k_edge_pipe; 0: none yet),
- * atoms per chunk, threads per block, grid size, network width}.  Errors: INVALID_ARG. */
+ * out[5] = {kernel (0: none yet; 1 k_edge_tc, 2 k_edge_tc128, 3 k_edge_er128_fwd, 4 k_edge_rows [width 128, the default backward],
+ * 5 k_edge_pipe, 7 k_edge_rows of the narrow widths 32 / 64, 8 k_edge_fwd4 [width 128, the default forward], 9 k_edge_rows with
+ * TMA gathers [LSD_EDGE_TMA=1]), atoms per chunk, threads per block, grid size, network width}.  Errors: INVALID_ARG. */
 lsd_status lsd_get_edge_launch_info(int32_t pass, int32_t* out);
 /* 1 if the target network's filter contractions run on the bf16 tcgen05 path in this context, else 0. */
 int32_t     lsd_tc_enabled(const lsd_ctx* ctx);

@@ -45,6 +45,7 @@ struct lsd_ctx {
     std::vector<void*> list_allocs;                          // neighbour-list rows: freed and re-made by setup_lists (lsd_set_skin)
     bool alloc_lists = false;                                // dalloc files under list_allocs
     double slack = 0.0;                                      // force slack eps_F of App. H (0 = off: exact)
+    bool tiny_draft_lists_stale = true;                      // tiny contexts: no lsd_eval_forces(LSD_DRAFT) since the last one-kernel rollout (its rows stay on chip)
     double cap_growth = 1.0;                                 // extra head room of the rows after an overflow (x 1.5 per retry)
     double c1 = 0, b = 0, hdt = 0, kT = 0;
     double *q = nullptr, *p = nullptr;
@@ -737,6 +738,7 @@ lsd_status lsd_draft_rollout(lsd_ctx* ctx, int32_t K, void* stream)
     CK(cudaEventRecord(w.ev_drafted, st));
     w.K = K; w.drafted = 1; w.verified = 0;
     w.prior_valid = ctx->same_prior && !ctx->tiny;               // (the one-kernel rollout keeps its prior forces on chip)
+    if (ctx->tiny) ctx->tiny_draft_lists_stale = true;            // ... and its neighbour rows: the per-state draft lists no longer belong to the last evaluation
     ctx->pending++;
     CK(cudaGetLastError());
     return LSD_OK;
@@ -917,11 +919,13 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
     if (ctx->state_in_flight) CK(cudaStreamWaitEvent(st, ctx->ev_state, 0));
     const size_t n3 = (size_t)3 * ctx->sys.n;
     WindowSlot& w = ctx->slot[ctx->verify_idx];
+    // flushed speculative rollouts of ANY slot (after a rejection, or after an error return of lsd_run) may still run on another
+    // stream; they share the draft's work buffers, the per-state lists and the cell grid with this rollout (as in lsd_draft_rollout)
+    for (int s = 0; s < ctx->nslots; ++s) if (ctx->slot[s].ev_drafted) CK(cudaStreamWaitEvent(st, ctx->slot[s].ev_drafted, 0));
     int list_retries = 0;
     int64_t remaining = n_steps;
     while (remaining > 0) {
         const int K = (int)std::min<int64_t>(ctx->cfg.k_max, remaining);
-        if (w.ev_drafted) CK(cudaStreamWaitEvent(st, w.ev_drafted, 0));
         CK(cudaMemcpyAsync(w.qstart, ctx->q, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         CK(cudaMemcpyAsync(w.pstart, ctx->p, n3 * sizeof(double), cudaMemcpyDeviceToDevice, st));
         w.n0 = (uint64_t)ctx->step;
@@ -944,6 +948,9 @@ lsd_status lsd_plain_langevin(lsd_ctx* ctx, int32_t which, int64_t n_steps, void
         remaining -= K;
     }
     w.drafted = 0; w.verified = 0;
+    CK(cudaStreamSynchronize(st));            // the last chunk's copy into the base state
+    stream_idle(ctx, st);                     // the caller may destroy `stream` now: the context keeps no handle of it
+    if (ctx->tiny && which == LSD_DRAFT) ctx->tiny_draft_lists_stale = true;
     return LSD_OK;
 }
 
@@ -951,6 +958,9 @@ lsd_status lsd_get_state(lsd_ctx* ctx, double* q, double* p, int64_t* step, int3
 {
     if (!ctx) return LSD_ERR_INVALID_ARG;
     TRY(sync_pending(ctx));
+    // caller-owned DEVICE buffers: the copies below run on the internal non-blocking stream, which is not ordered against the
+    // caller's streams (nor torch's default stream), so kernels of the caller that still read q / p must have finished first
+    if (where == LSD_DEVICE) CK(cudaDeviceSynchronize());
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
     if (where == LSD_HOST && ctx->state_host && q && p) {     // small system: one device-to-host copy of (q, p) through the pinned staging
         CK(cudaMemcpyAsync(ctx->state_host, ctx->q, 2 * bytes, cudaMemcpyDeviceToHost, ctx->side));
@@ -972,6 +982,9 @@ lsd_status lsd_set_state(lsd_ctx* ctx, const double* q, const double* p, int64_t
 {
     if (!ctx || !q || !p) return LSD_ERR_INVALID_ARG;
     TRY(sync_pending(ctx));
+    // caller-owned DEVICE buffers: whatever kernel of the caller produces q / p (on any stream) must have finished before the
+    // internal non-blocking stream reads them
+    if (where == LSD_DEVICE) CK(cudaDeviceSynchronize());
     const size_t bytes = (size_t)3 * ctx->sys.n * sizeof(double);
     if (where == LSD_HOST && ctx->state_host) {
         // small system: the caller's buffers are copied into the pinned staging (they are free again on return), ONE upload is
@@ -1046,6 +1059,8 @@ lsd_status lsd_get_window_obabo(lsd_ctx* ctx, int32_t j, double* q, double* p, i
     if (!ctx) return LSD_ERR_INVALID_ARG;
     if (ctx->last_slot < 0) return fail(ctx, LSD_ERR_STATE, "no window has been transported yet");
     if (j < 1 || j > ctx->last_nc) return fail(ctx, LSD_ERR_INVALID_ARG, "j must be in 1..n_commit");
+    // Eq. 30 rebuilds p_mid from the kick the step was committed with; with force slack that kick used F_(eps), not the F kept in Fg
+    if (ctx->slack > 0.0) return fail(ctx, LSD_ERR_STATE, "OBABO outputs are not available while force slack is on (lsd_set_force_slack(0) first)");
     CK(cudaDeviceSynchronize());
     const WindowSlot& w = ctx->slot[ctx->last_slot];
     const int n = ctx->sys.n;
@@ -1067,6 +1082,8 @@ lsd_status lsd_get_window_state(lsd_ctx* ctx, int32_t j, double* q, double* p, i
     if (!ctx) return LSD_ERR_INVALID_ARG;
     if (ctx->last_slot < 0) return fail(ctx, LSD_ERR_STATE, "no window has been transported yet");
     if (j < 1 || j > ctx->last_nc) return fail(ctx, LSD_ERR_INVALID_ARG, "j must be in 1..n_commit");
+    // Eq. 30 rebuilds p_mid from the kick the step was committed with; with force slack that kick used F_(eps), not the F kept in Fg
+    if (ctx->slack > 0.0) return fail(ctx, LSD_ERR_STATE, "OBABO outputs are not available while force slack is on (lsd_set_force_slack(0) first)");
     CK(cudaDeviceSynchronize());
     const WindowSlot& w = ctx->slot[ctx->last_slot];
     const size_t n3 = (size_t)3 * ctx->sys.n;
@@ -1139,6 +1156,7 @@ lsd_status lsd_eval_forces(lsd_ctx* ctx, int32_t which, int32_t n_states, const 
     CK(cudaMemcpyAsync(&hf, ctx->flags_eval, sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
+    if (which == LSD_DRAFT) ctx->tiny_draft_lists_stale = false;             // the per-state draft lists are this evaluation's
     return flags_to_status(ctx, hf);
 }
 
@@ -1192,7 +1210,8 @@ lsd_status lsd_get_neighbors(lsd_ctx* ctx, int32_t which, int32_t kind, int32_t 
     if (!ctx || !start || !n_edges || (which != 0 && which != 1) || (kind != 0 && kind != 1)) return LSD_ERR_INVALID_ARG;
     const CompactList& cl = (kind == 0 || ctx->pair_is_mlip[which]) ? ctx->cl_mlip[which] : ctx->cl_pair[which];
     if (!cl.count || !ctx->cl_img[which]) return fail(ctx, LSD_ERR_STATE, "this potential has no such list (or no evaluation has run yet)");
-    if (ctx->tiny && which == LSD_DRAFT) return fail(ctx, LSD_ERR_STATE, "the one-kernel draft rollout of a tiny system keeps its neighbour rows on chip");
+    if (ctx->tiny && which == LSD_DRAFT && ctx->tiny_draft_lists_stale)
+        return fail(ctx, LSD_ERR_STATE, "the one-kernel draft rollout of a tiny system keeps its neighbour rows on chip (call lsd_eval_forces(LSD_DRAFT) for a list)");
     if (b < 0 || b >= cl.bmax) return fail(ctx, LSD_ERR_INVALID_ARG, "state index out of range");
     CK(cudaDeviceSynchronize());
     const int n = ctx->sys.n;

@@ -239,7 +239,9 @@ struct EdgeArgs {
     uint16_t* ybar16_out = nullptr;   // BWD, width 128: ybar as bf16 rows instead of ybar
     const float* mbar; float* ybar;   // BWD
     double* Fout;                     // BWD: [B][3][n], accumulated
-    unsigned long long* trace = nullptr;   // debug (LSD_EDGE_TRACE=1): clock64 stamps of one chunk of block 0
+#ifdef LSD_EDGE_TRACE_BUILD
+    unsigned long long* trace = nullptr;   // debug builds (LSD_NVCC_FLAGS=-DLSD_EDGE_TRACE_BUILD, then LSD_EDGE_TRACE=1): clock64 stamps of one chunk of block 0
+#endif
 };
 
 // per-device one-time state (function attributes, SM count): indexed by the current device, not per process
@@ -254,7 +256,7 @@ inline int lsd_sm_count()
 
 // which tcgen05 edge kernel the last forward / backward launch of this process used (parity tests assert that the timed
 // instantiation is the one they compared with the oracle): kernel 1 = k_edge_tc (mlip_tc.cu), 2 = k_edge_tc128, 3 = k_edge_er128_fwd,
-// 4 = k_edge_rows, 5 = k_edge_pipe, 7 = k_edge_rows (narrow widths)
+// 4 = k_edge_rows, 5 = k_edge_pipe, 7 = k_edge_rows (narrow widths), 8 = k_edge_fwd4, 9 = k_edge_rows with TMA gathers
 struct EdgeLaunchInfo { int kernel = 0, atoms_per_chunk = 0, threads = 0, grid = 0, width = 0; };
 inline EdgeLaunchInfo g_edge_last[2];
 inline void note_edge_launch(bool backward, int kernel, int atoms_per_chunk, int threads, int grid, int width)

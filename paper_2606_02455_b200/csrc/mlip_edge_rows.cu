@@ -254,7 +254,9 @@ k_edge_rows(EdgeArgs a, int chunks_per_state, int nchunks)
         for (int chunk = blockIdx.x * kTeams + team; chunk < nchunks; chunk += gridDim.x * kTeams) {
             const int b = chunk / chunks_per_state, ci = chunk - b * chunks_per_state;
             const int g0 = b * n + ci * kCH;                       // first feature row of the chunk
+#ifdef LSD_EDGE_TRACE_BUILD
             tr_on = a.trace != nullptr && blockIdx.x == 0 && tt == 0 && chunk == blockIdx.x * kTeams + team + 3 * (int)gridDim.x * kTeams;
+#endif
             const int natoms = min(kCH, n - ci * kCH);
             if (tt < 32) {                                         // groups per atom, exclusive scan over the 16 atoms
                 const int c = tt < natoms ? a.count[g0 + tt] : 0;
@@ -638,6 +640,7 @@ template <bool BWD, int SPLIT, bool TMA = false> void launch_rows(Launcher L, co
     const int cps = (a.n + kCH - 1) / kCH;
     const int nchunks = cps * (a.total / a.n);
     const int grid = std::max(1, std::min(device_sm_count(), (nchunks + kTeams - 1) / kTeams));
+#ifdef LSD_EDGE_TRACE_BUILD                                         // debug builds only: this block allocates and synchronises inside a launch
     static const bool trace_on = [] { const char* v = getenv("LSD_EDGE_TRACE"); return v && v[0] == '1'; }();
     static int trace_launch[2] = {0, 0};
     if (trace_on && ++trace_launch[BWD] == 8) {                    // debug: time stamps of one chunk, printed once per direction
@@ -661,6 +664,7 @@ template <bool BWD, int SPLIT, bool TMA = false> void launch_rows(Launcher L, co
         LSD_COUNT(L);
         return;
     }
+#endif
     k_edge_rows<BWD, SPLIT, TMA><<<grid, threads, Lay<BWD, TMA>::Smem, L.s>>>(a, cps, nchunks);
     note_edge_launch(BWD, TMA ? 9 : 4, kCH, threads, grid, kF);
     LSD_COUNT(L);
