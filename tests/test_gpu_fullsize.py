@@ -1,6 +1,7 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (cfg5: 65,536 atoms, K = 8, bf16 tcgen05
 path; cfg4: 4,096 atoms, K = 32; cfg3: 1,536 atoms, K = 16).  Forces are compared with the oracle element-wise per atom
-(test_full_size_forces_match_oracle: cfg3 / cfg4 two window states each in fp32 and bf16, cfg5 one state -- one oracle evaluation
+(test_full_size_forces_match_oracle: cfg3 / cfg4 two window states each in fp32 and bf16, cfg5 one state, plus the draft forces of
+one state each -- one oracle evaluation
 of the 6-block network on 65,536 atoms takes about a minute on the box's host cores); everything else the oracle can do at
 full size is compared directly too: neighbour lists (cell-list oracle, bit-exact), the transport map / decisions on the GPU's
 own forces, the noise; plus properties that hold at any size (sum of forces, batch invariance, reproducibility)."""
@@ -133,7 +134,7 @@ def test_full_size_forces_match_oracle(P, orc, name, prec, states):
     ctx.window(K, stream)                                       # first window: plain launches, captures the graphs
     P.lsd_draft_rollout(ctx.h, K, stream); P.lsd_verify_window(ctx.h, K, stream)
     l, nc = P.lsd_transport_accept(ctx.h, K, stream)
-    qh, Fg = ctx.debug("q_half", K), ctx.debug("F_target", K)
+    qh, Fg, Ft = ctx.debug("q_half", K), ctx.debug("F_target", K), ctx.debug("F_draft", K)
     if bf16:
         fwd, bwd = P.lsd_get_edge_launch_info(False), P.lsd_get_edge_launch_info(True)
         assert fwd["width"] == w.target.mlip.width and bwd["width"] == w.target.mlip.width     # the target's launches were the last ones
@@ -152,5 +153,11 @@ def test_full_size_forces_match_oracle(P, orc, name, prec, states):
         Eo, Fo = orc.energy_forces(w, w.target, np.ascontiguousarray(qh[j].T))
         err = _t2_error(Fg[j].T, Fo)
         assert err <= tol, (name, prec, j, err)
+    # the draft forces of the same rollout (cfg4 / cfg5: the width-32 one-block network, whose four-team tcgen05 kernels run here
+    # in the full-size launch configuration; cfg3: the classical prior alone), one state
+    j = states[-1]
+    Fo = orc.energy_forces(w, w.draft, np.ascontiguousarray(qh[j].T))[1]
+    err = _t2_error(Ft[j].T, Fo)
+    assert err <= tol, (name, prec, "draft", j, err)
     P.lsd_rollback(ctx.h, l)
     ctx.close()
