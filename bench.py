@@ -37,12 +37,26 @@ UNIT = "atom-steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from one ncu capture of this
 # command (per workload and arithmetic type; null where no capture is committed).  Not measured by this run: a run under a
-# profiler is never a bench run; `roofline.traffic_source` names the committed capture the figure comes from.
-NCU_TRAFFIC = {("cfg5", "bf16"): (1.6515e9 + 0.1405e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)"),
-               ("cfg4", "bf16"): (0.2073e9 + 0.0250e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)"),
-               ("cfg4", "f32"): (0.2750e9 + 0.0565e9, "profiles/r2_traffic.md (k_edge<128,bwd>)"),
-               ("cfg3", "bf16"): (0.0572e9 + 0.0004e9, "profiles/r2_traffic.md (k_edge_rows<64,1,2>)"),
-               ("cfg3", "f32"): (0.0635e9 + 0.0002e9, "profiles/r2_traffic.md (k_edge<64,bwd>)")}
+# profiler is never a bench run; `roofline.traffic_source` names the committed capture the figure comes from.  The third field is
+# the identity of the kernel the capture was taken on, as lsd_get_edge_launch_info reports it (kernel, network width, threads per
+# block; None for the fp32 kernels, which have one instantiation per width): when the kernel that runs differs, the figure is
+# stale and `traffic` is reported as null.
+NCU_TRAFFIC = {("cfg5", "bf16"): (1.6515e9 + 0.1405e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)", ("k_edge_rows", 128, 512)),
+               ("cfg4", "bf16"): (0.2073e9 + 0.0250e9, "profiles/r2_traffic.md (k_edge_rows<1,2>)", ("k_edge_rows", 128, 512)),
+               ("cfg4", "f32"): (0.2750e9 + 0.0565e9, "profiles/r2_traffic.md (k_edge<128,bwd>)", None),
+               ("cfg3", "bf16"): (0.05723e9 + 0.00023e9, "profiles/r3_traffic_cfg3_bf16.md (k_edge_rows<64,1,1>)", ("k_edge_rows_narrow", 64, 512)),
+               ("cfg3", "f32"): (0.0635e9 + 0.0002e9, "profiles/r2_traffic.md (k_edge<64,bwd>)", None)}
+
+
+def traffic_for(name, dtype, running):
+    """(traffic, source) for the roofline block; `running` = (kernel, width, threads) of the dominant kernel of this run or None."""
+    tr = NCU_TRAFFIC.get((name, dtype))
+    if tr is None:
+        return None, None
+    if tr[2] is not None and running is not None and tuple(tr[2]) != tuple(running):
+        return None, f"stale: {tr[1]} was captured on {tr[2]}, this run launched {tuple(running)}"
+    return tr[0], tr[1]
+
 
 # the workloads of BASELINE.json with the arithmetic types it lists for them (north_star: "report throughput on the five synthetic
 # workloads"): the default run times --workload in full and the others for a few windows each (`all_workloads`)
@@ -339,10 +353,12 @@ def build_roofline(env, w, name, precision, prec, ctx, prof, edges, steps, ms_pr
         info_b, info_f = P.lsd_get_edge_launch_info(True), P.lsd_get_edge_launch_info(False)
         kernel = f"{info_b['kernel']} (grid {info_b['grid']} x {info_b['threads']} threads, {info_b['atoms_per_chunk']} atoms per chunk)"
         fwd_kernel = info_f["kernel"]
+        running = (info_b["kernel"], info_b["width"], info_b["threads"])
     else:
         bound, dtype, peak = "alu", "f32", fp32_peak
         peak_note = "fp32 FMA peak measured by lsd_measure_fma_peak in this run"
         kernel, fwd_kernel = f"k_edge<{F},bwd>", f"k_edge<{F},fwd>"
+        running = None
     mlip_ms = prof["mlip_edge_bwd"]["ms"] + prof["mlip_edge_fwd"]["ms"] + prof["mlip_dense"]["ms"]
     a2_ms = mlip_ms / steps
     # three-term roofline of the batched target force evaluation (a2) per window: strict tensor / FMA flops, algorithmic
@@ -355,9 +371,9 @@ def build_roofline(env, w, name, precision, prec, ctx, prof, edges, steps, ms_pr
     t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
     t_sfu = mufu_ops / (16.0 * 148.0 * sm_hz) * 1e3
     terms = {"tensor" if use_tc else "fma": t_tensor, "hbm": t_hbm, "sfu": t_sfu}
-    tr = NCU_TRAFFIC.get((name, dtype))
+    traffic, traffic_source = traffic_for(name, dtype, running)
     roofline = dict(bound=bound, achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak,
-                    traffic=tr[0] if tr else None, traffic_source=tr[1] if tr else None,
+                    traffic=traffic, traffic_source=traffic_source,
                     kernel=kernel + " (MLIP edge backward: filter value + tangent, cfconv adjoints)", avg_launch_ms=avg_ms, launches=eb["launches"],
                     algorithmic_flops_per_launch=flops_per_launch, directed_edges_per_window=edges, peak_note=peak_note,
                     share_of_step=eb["ms"] / ms_prof if ms_prof > 0 else None, profiled_ms_per_step=ms_prof / steps,
@@ -565,7 +581,7 @@ def main():
 
     m = measure_workload(env, args.workload, args.precision, args.steps, args.warmup, full=True, ec=args.ec, overlap=args.overlap)
 
-    side, variant, ring, design = None, None, None, None
+    side, variant, ring = None, None, None
     if not args.no_side and world == 1 and not args.ec and not args.overlap:
         # the other BASELINE.json workloads, a few windows each, through the same measurement code (the headline is listed again in short form)
         side = {}
@@ -589,22 +605,6 @@ def main():
                 return dict(error=f"{type(exc).__name__}: {exc}")
         variant = guarded(acceptance_variant, env, args.workload, args.precision)
         ring = guarded(async_depth_block, env)
-        # two design measurements DESIGN.md cites (section 4.1, section 7): tensor-memory bandwidth of an SM, and the second delivery of a
-        # half-list schedule at the headline workload's sizes (rows = half of the mean directed neighbour count)
-        def design_block():
-            wl = L.make_workload(args.workload)
-            nb_half = max(1, int(round(0.5 * m["roofline"].get("directed_edges_per_window", 0) / max(wl.K * wl.n_atoms, 1)))) if m["roofline"] else 0
-            design = dict(tmem_bytes_per_clk_per_sm={"ld_x16_%dw" % nw: P.lsd_measure_tmem_bandwidth(nw, False, stream) for nw in (1, 4, 8, 16)})
-            design["tmem_bytes_per_clk_per_sm"].update({"st_x16_%dw" % nw: P.lsd_measure_tmem_bandwidth(nw, True, stream) for nw in (4, 8, 16)})
-            if nb_half > 0 and wl.target.mlip is not None and wl.target.mlip.width == 128:
-                sc, ga = P.lsd_measure_half_list_delivery(wl.n_atoms, wl.K, nb_half, stream)
-                rows_gb = wl.n_atoms * wl.K * nb_half * 256e-9
-                design["half_list_delivery"] = dict(rows_per_atom=nb_half, rows_GB=rows_gb, scatter_ms=sc, ordered_gather_sum_ms=ga, total_ms=sc + ga,
-                                                    edge_backward_launch_ms=m["roofline"].get("avg_launch_ms"),
-                                                    note="one 256-byte bf16 row per undirected pair written to the partner's slot, then summed per atom in slot order: what a "
-                                                         "deterministic half-list schedule adds per edge pass; it replaces at most half of the edge kernel's launch time")
-            return design
-        design = guarded(design_block)
 
     if rank == 0:
         N, K = m["n_atoms"], m["window_K"]
@@ -629,8 +629,6 @@ def main():
             line["acceptance_variant"] = variant
         if ring is not None:
             line["async_depth"] = ring
-        if design is not None:
-            line["design_measurements"] = design
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = {k: v for k, v in cpu_baseline(args.workload).items() if k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))

@@ -258,16 +258,6 @@ lsd_status lsd_get_profile(lsd_ctx* ctx, double* ms, int64_t* count);
  * grid of resident warps, CUDA events on `stream`, best of three): the roofline denominators of the fp32 MLIP path and of the
  * fp64 path ("measured fp32-FMA peak", "measured fp64 peak").  Synchronises.  Errors: INVALID_ARG, CUDA. */
 lsd_status lsd_measure_fma_peak(int32_t kind, void* stream, double* tflops);
-/* Two design measurements DESIGN.md cites (no part of the hot path).  lsd_measure_tmem_bandwidth: bytes per cycle and SM that
- * `warps` (1, 4, 8 or 16) warps of one CTA per SM move with tcgen05.ld.32x32b.x16 (+ wait) or, store != 0, tcgen05.st (the
- * accumulator reads of the edge kernels).  lsd_measure_half_list_delivery: the second delivery of a
- * half-list schedule (one filter evaluation per undirected pair, w_ij = w_ji) without float atomics, at the
- * given sizes: every pair writes one 128-channel bf16 row (256 B) to its partner's slot, then every atom sums its
- * rows_per_atom incoming rows in slot order; milliseconds of the two kernels (best of 2 after a warm-up; allocates
- * 256 B x n_atoms x n_states x rows_per_atom of scratch).  Synchronise.  Errors: INVALID_ARG, OOM, CUDA. */
-lsd_status lsd_measure_tmem_bandwidth(int32_t warps, int32_t store, void* stream, double* bytes_per_clk);
-lsd_status lsd_measure_half_list_delivery(int32_t n_atoms, int32_t n_states, int32_t rows_per_atom, void* stream,
-                                          double* scatter_ms, double* gather_ms);
 /* Number of kernels this library has launched on behalf of ctx (bench.py's gpu_launches). */
 int64_t     lsd_launch_count(const lsd_ctx* ctx);
 const char* lsd_version(void);

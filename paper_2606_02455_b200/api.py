@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = ["lsd_init", "lsd_destroy", "lsd_last_error", "lsd_draft_roll
                     "lsd_get_window_debug", "lsd_eval_forces", "lsd_get_neighbors", "lsd_set_skin", "lsd_launch_count", "lsd_version", "lsd_profile", "lsd_get_profile", "lsd_get_edge_count", "lsd_tc_enabled",
                     "lsd_set_error_correction", "lsd_get_ec_cache", "lsd_set_ec_cache", "lsd_plain_langevin", "lsd_get_adaptive_k",
                     "lsd_get_window_obabo", "lsd_get_edge_launch_info", "lsd_measure_fma_peak", "lsd_set_force_slack", "lsd_tiny_rollout_enabled", "lsd_set_window_slots",
-                    "lsd_measure_tmem_bandwidth", "lsd_measure_half_list_delivery", "lsd_transport_window_noalloc", "lsd_noalloc_last_error"]
+                    "lsd_transport_window_noalloc", "lsd_noalloc_last_error"]
 
 
 class LsdError(RuntimeError):
@@ -297,21 +297,6 @@ def lsd_measure_fma_peak(kind: int, stream=None) -> float:
     out = C.c_double()
     _check(None, load_library().lsd_measure_fma_peak(C.c_int32(kind), _stream(stream), C.byref(out)))
     return float(out.value)
-
-
-def lsd_measure_tmem_bandwidth(warps: int, store: bool = False, stream=None) -> float:
-    """Bytes per cycle and SM moved by tcgen05.ld (or tcgen05.st) with `warps` warps of one CTA per SM."""
-    out = C.c_double()
-    _check(None, load_library().lsd_measure_tmem_bandwidth(C.c_int32(warps), C.c_int32(int(store)), _stream(stream), C.byref(out)))
-    return float(out.value)
-
-
-def lsd_measure_half_list_delivery(n_atoms: int, n_states: int, rows_per_atom: int, stream=None):
-    """(scatter_ms, gather_ms) of the second delivery of a half-list schedule at the given sizes."""
-    a, b = C.c_double(), C.c_double()
-    _check(None, load_library().lsd_measure_half_list_delivery(C.c_int32(n_atoms), C.c_int32(n_states), C.c_int32(rows_per_atom), _stream(stream),
-                                                               C.byref(a), C.byref(b)))
-    return float(a.value), float(b.value)
 
 
 LSD_NOALLOC_MAX_K, LSD_NOALLOC_MAX_ATOMS = 64, 1 << 28
