@@ -263,9 +263,10 @@ int64_t     lsd_launch_count(const lsd_ctx* ctx);
 const char* lsd_version(void);
 /* Which tcgen05 edge kernel the last MLIP edge launch of this process used, pass 0 = forward (M5), 1 = backward (M9); parity
  * tests use it to assert that the instantiation they compared with the oracle is the one the benchmark times.
- * out[5] = {kernel (0: none yet; 1 k_edge_tc, 2 k_edge_tc128, 3 k_edge_er128_fwd, 4 k_edge_rows [width 128, the default backward],
- * 5 k_edge_pipe, 7 k_edge_rows of the narrow widths 32 / 64, 8 k_edge_fwd4 [width 128, the default forward], 9 k_edge_rows with
- * TMA gathers [LSD_EDGE_TMA=1]), atoms per chunk, threads per block, grid size, network width}.  Errors: INVALID_ARG. */
+ * out[5] = {kernel (0: none yet; 4 k_edge_rows [width 128: the default backward; the forward with LSD_EDGE_FWD4=0], 7 k_edge_rows of
+ * the narrow widths 32 / 64, 8 k_edge_fwd4 [width 128, the default forward], 9 k_edge_rows with TMA gathers [LSD_EDGE_TMA=1];
+ * ids 1, 2, 3, 5 belonged to kernels removed in round 3), atoms per chunk, threads per block, grid size, network width}.
+ * Errors: INVALID_ARG. */
 lsd_status lsd_get_edge_launch_info(int32_t pass, int32_t* out);
 /* 1 if the target network's filter contractions run on the bf16 tcgen05 path in this context, else 0. */
 int32_t     lsd_tc_enabled(const lsd_ctx* ctx);

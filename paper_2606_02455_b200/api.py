@@ -283,7 +283,7 @@ def lsd_get_profile(h) -> dict:
     return {name: dict(ms=ms[i], launches=cnt[i]) for i, name in enumerate(PROFILE_CLASSES)}
 
 
-EDGE_KERNELS = {0: None, 1: "k_edge_tc", 2: "k_edge_tc128", 3: "k_edge_er128_fwd", 4: "k_edge_rows", 5: "k_edge_pipe", 7: "k_edge_rows_narrow", 8: "k_edge_fwd4", 9: "k_edge_rows_tma"}
+EDGE_KERNELS = {0: None, 4: "k_edge_rows", 7: "k_edge_rows_narrow", 8: "k_edge_fwd4", 9: "k_edge_rows_tma"}
 
 
 def lsd_get_edge_launch_info(backward: bool) -> dict:

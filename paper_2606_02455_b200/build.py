@@ -14,7 +14,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "liblsd_b200.so")
-SOURCES = ["lsd_api.cu", "integrator.cu", "neighbor.cu", "prior.cu", "mlip_simt.cu", "mlip_tc.cu", "mlip_tc128.cu", "mlip_atom_tc128.cu", "mlip_er128.cu", "mlip_edge_rows.cu", "mlip_edge_rows_narrow.cu", "mlip_edge_fwd4.cu", "mlip_edge_pipe.cu", "tiny_rollout.cu", "peaks.cu", "transport_noalloc.cu"]
+SOURCES = ["lsd_api.cu", "integrator.cu", "neighbor.cu", "prior.cu", "mlip_simt.cu", "mlip_tc.cu", "mlip_atom_tc128.cu", "mlip_edge_rows.cu", "mlip_edge_rows_narrow.cu", "mlip_edge_fwd4.cu", "tiny_rollout.cu", "peaks.cu", "transport_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-I" + os.path.join(ROOT, "include"), "-I" + CSRC] + os.environ.get("LSD_NVCC_FLAGS", "").split()   # e.g. -DLSD_EDGE_TRACE_BUILD

@@ -255,8 +255,8 @@ inline int lsd_sm_count()
 }
 
 // which tcgen05 edge kernel the last forward / backward launch of this process used (parity tests assert that the timed
-// instantiation is the one they compared with the oracle): kernel 1 = k_edge_tc (mlip_tc.cu), 2 = k_edge_tc128, 3 = k_edge_er128_fwd,
-// 4 = k_edge_rows, 5 = k_edge_pipe, 7 = k_edge_rows (narrow widths), 8 = k_edge_fwd4, 9 = k_edge_rows with TMA gathers
+// instantiation is the one they compared with the oracle): kernel 4 = k_edge_rows (width 128), 7 = k_edge_rows (narrow widths),
+// 8 = k_edge_fwd4, 9 = k_edge_rows with TMA gathers (1, 2, 3, 5 were round-1 / opt-in kernels, removed in round 3)
 struct EdgeLaunchInfo { int kernel = 0, atoms_per_chunk = 0, threads = 0, grid = 0, width = 0; };
 inline EdgeLaunchInfo g_edge_last[2];
 inline void note_edge_launch(bool backward, int kernel, int atoms_per_chunk, int threads, int grid, int width)
@@ -269,12 +269,8 @@ void mlip_forward_backward_fp32(Launcher L, const SysDev& sys, const MlipDev& ne
                                 const int* img, const CompactList& cl, double* F /*accumulated*/, double* e_atom);
 size_t mlip_work_bytes(const MlipDev& net, int n, int bmax);
 
-// ---- mlip_tc.cu (bf16 tcgen05 filter path)
+// ---- bf16 tcgen05 filter path (mlip_tc.cu: host-side packing; the kernels are in mlip_edge_*.cu)
 bool mlip_tc_supported(const MlipDev& net);
-void launch_edge_tc(Launcher L, const EdgeArgs& a, int F, bool backward);
-void launch_edge_tc128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_tc128.cu: width 128
-void launch_edge_er128(Launcher L, const EdgeArgs& a, bool backward);      // mlip_er128.cu: width 128, edges-as-rows schedule
-void launch_edge_pipe(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_pipe.cu: width 128, warp-specialised pipeline of the same tile algebra
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward);       // mlip_edge_rows.cu: width 128, edges-as-rows, activations in TMEM
 bool lsd_encode_row_tmap(void* host_map_128B, const void* base, size_t rows, int row_bytes);   // mlip_edge_rows.cu: false if the driver lacks the entry point
 void launch_edge_fwd4(Launcher L, const EdgeArgs& a);                      // mlip_edge_fwd4.cu: width 128, forward, four tiles in flight per SM

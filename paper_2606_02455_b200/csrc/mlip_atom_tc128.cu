@@ -364,23 +364,16 @@ void tc_pack_rect128(const double* W, int rows, int cols, bool transpose, std::v
         }
 }
 
-// Width-128 bf16 tensor-core network: edge kernels of mlip_tc128.cu + the chain kernels above.  bf16 aliases of fp32 work
+// Width-128 bf16 tensor-core network: edge kernels of mlip_edge_fwd4.cu / mlip_edge_rows.cu + the chain kernels above.  bf16 aliases of fp32 work
 // buffers that this path does not need: m16 in w.m, ybar16 in w.ybar, xbar16 in w.mbar.
 void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, int B, const double* q,
                                  const int* img, const CompactList& cl, double* Fout, double* e_atom)
 {
     (void)q; (void)img;
     const int total = B * sys.n, T = net.T;
-    static const bool use_er = [] { const char* v = getenv("LSD_EDGE_ER"); return v == nullptr || v[0] != '0'; }();
-    // LSD_EDGE_ROWS: which passes use the second-generation edge kernel (mlip_edge_rows.cu) instead of mlip_er128.cu (forward) /
-    // mlip_tc128.cu (backward): 0 none, 1 forward, 2 backward (default: measured faster there), 3 both
-    static const int rows_sel = [] { const char* v = getenv("LSD_EDGE_ROWS"); return v ? atoi(v) : 2; }();   // bit 0: forward, bit 1: backward
-    const bool use_rows_f = (rows_sel & 1) != 0, use_rows = (rows_sel & 2) != 0;
-    // LSD_EDGE_PIPE: which passes use the warp-specialised pipeline (mlip_edge_pipe.cu); same bits; takes precedence
-    static const int pipe_sel = [] { const char* v = getenv("LSD_EDGE_PIPE"); return v ? atoi(v) : 0; }();
-    const bool use_pipe_f = (pipe_sel & 1) != 0, use_pipe_b = (pipe_sel & 2) != 0;
     // LSD_EDGE_FWD4: forward pass with four tiles in flight per SM (mlip_edge_fwd4.cu; default, measured 2.9 vs 3.9 ms per cfg5
-    // launch); 0 falls back to the selection above
+    // launch); 0 selects the forward instantiation of k_edge_rows (two tiles in flight), kept as the A/B partner and tested in
+    // tests/test_gpu_variants.py.  The backward is k_edge_rows (LSD_EDGE_TMA=1: its TMA-gather variant, same test file).
     static const bool use_fwd4 = [] { const char* v = getenv("LSD_EDGE_FWD4"); return v == nullptr || v[0] != '0'; }();
     uint16_t* const m16 = reinterpret_cast<uint16_t*>(w.m);
     uint16_t* const ybar16 = reinterpret_cast<uint16_t*>(w.ybar);
@@ -395,7 +388,7 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
     for (int t = 0; t < T; ++t) {
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.m16_out = m16;
         pid = prof_begin(L, PROF_EDGE_FWD);
-        if (use_fwd4) launch_edge_fwd4(L, ea); else if (use_pipe_f) launch_edge_pipe(L, ea, false); else if (use_rows_f) launch_edge_rows(L, ea, false); else if (use_er) launch_edge_er128(L, ea, false); else launch_edge_tc128(L, ea, false);
+        if (use_fwd4) launch_edge_fwd4(L, ea); else launch_edge_rows(L, ea, false);
         prof_end(L, pid);
         AtomArgs aa{};
         aa.total = total; aa.in16 = m16; aa.h = w.h[t]; aa.x = w.x;
@@ -414,18 +407,18 @@ void mlip_forward_backward_tc128(Launcher L, const SysDev& sys, const MlipDev& n
         if (t == T - 1) {
             AtomArgs aa{};
             aa.total = total; aa.in16 = xbar16; aa.h = w.h[t]; aa.y16 = w.y16[t]; aa.ym16 = w.ym16;
-            aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t]; aa.ym_pairs = use_rows || use_pipe_b;
+            aa.W[1] = net.Wo2T_tc[t]; aa.W[2] = net.Wo1T_tc[t]; aa.ym_pairs = 1;
             launch_atom<BWD2>(L, aa);
         }
         ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.ym16 = w.ym16; ea.ym_tmap = w.ym_tmap;
         ea.ybar16_out = t > 0 ? ybar16 : nullptr; ea.ybar = nullptr; ea.Fout = Fout;
         pid = prof_begin(L, PROF_EDGE_BWD);
-        if (use_pipe_b) launch_edge_pipe(L, ea, true); else if (use_rows) launch_edge_rows(L, ea, true); else launch_edge_tc128(L, ea, true);
+        launch_edge_rows(L, ea, true);
         prof_end(L, pid);
         if (t > 0) {
             AtomArgs aa{};
             aa.total = total; aa.in16 = ybar16; aa.x = w.xbar; aa.h = w.h[t - 1]; aa.y16 = w.y16[t - 1]; aa.ym16 = w.ym16;
-            aa.W[0] = net.WinT_tc[t]; aa.W[1] = net.Wo2T_tc[t - 1]; aa.W[2] = net.Wo1T_tc[t - 1]; aa.ym_pairs = use_rows || use_pipe_b;
+            aa.W[0] = net.WinT_tc[t]; aa.W[1] = net.Wo2T_tc[t - 1]; aa.W[2] = net.Wo1T_tc[t - 1]; aa.ym_pairs = 1;
             launch_atom<BWD3>(L, aa);
         }
     }

@@ -675,10 +675,8 @@ template <bool BWD, int SPLIT, bool TMA = false> void launch_rows(Launcher L, co
 // a.ym16 (backward) must be in the pair layout: per channel pair (f, f+1) the words (y_f | y_f+1 << 16), (mbar_f | mbar_f+1 << 16)
 void launch_edge_rows(Launcher L, const EdgeArgs& a, bool backward)
 {
-    static const int split = [] { const char* v = getenv("LSD_EDGE_SPLIT"); return (v && v[0] == '1') ? 1 : 2; }();
     // LSD_EDGE_TMA: the backward gathers its rows with TMA gather4 (needs the tensor map of alloc_work)
     static const bool tma = [] { const char* v = getenv("LSD_EDGE_TMA"); return v != nullptr && v[0] != '0'; }();
-    if (backward && split == 2 && tma && a.ym_tmap) { launch_rows<true, 2, true>(L, a); return; }
-    if (backward) { if (split == 2) launch_rows<true, 2>(L, a); else launch_rows<true, 1>(L, a); }
-    else { if (split == 2) launch_rows<false, 2>(L, a); else launch_rows<false, 1>(L, a); }
+    if (backward && tma && a.ym_tmap) { launch_rows<true, 2, true>(L, a); return; }
+    if (backward) launch_rows<true, 2>(L, a); else launch_rows<false, 2>(L, a);
 }

@@ -9,7 +9,7 @@
 // into allocated shared memory whose contents land in accumulator lanes >= F, which are ignored.
 // Replaces k_edge_tc (mlip_tc.cu: channels are rows, 64 edges per tile and three round trips) for these widths:
 // cfg3 bf16 window 2.45 -> 2.00 ms (1.43 ms with four teams), draft network at cfg5 7.5 -> 6.1 ms per window (4.35 ms with four
-// teams); LSD_EDGE_NARROW=0 selects k_edge_tc.
+// teams).
 // The width-128 instantiation lives in mlip_edge_rows.cu: generated from this generic source the dominant kernel came out
 // 2.3 % slower (44.6 vs 43.6 ms per cfg5 window, same instruction counts in the tile loop), so its tuned translation unit is kept.
 // Determinism / batch invariance: as in mlip_edge_rows.cu.

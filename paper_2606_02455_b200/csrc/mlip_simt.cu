@@ -442,9 +442,10 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         configured = true;
     }
     const int sms = num_sms();
-    // widths 32 / 64 on the tcgen05 path: the edges-as-rows kernel of mlip_edge_rows.cu (LSD_EDGE_NARROW=0: k_edge_tc of mlip_tc.cu)
-    static const bool narrow_env = [] { const char* v = getenv("LSD_EDGE_NARROW"); return !(v && v[0] == '0'); }();
-    const bool narrow_rows = use_tc && F < 128 && narrow_env;
+    // widths 32 / 64 on the tcgen05 path: the edges-as-rows kernels of mlip_edge_rows_narrow.cu (width 128 has its own driver,
+    // mlip_forward_backward_tc128)
+    static_assert(F == 32 || F == 64 || F == 128, "network widths");
+    if (use_tc && F == 128) return;                    // never reached: mlip_forward_backward_bf16tc routes width 128 elsewhere
     // 16 warps per CTA once every SM has at least 16 atoms to work on (occupancy: +8 % at cfg4 fp32); 8 for small batches,
     // whose kernels are latency-bound (a bigger CTA only adds to the weight-load and barrier time).  Same arithmetic either way.
     const int kWarps = total >= sms * kMaxWarps ? kMaxWarps : 8;
@@ -475,7 +476,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         pid = prof_begin(L, PROF_EDGE_FWD);
         if (use_tc) {
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t];
-            if (F == 128) launch_edge_tc128(L, ea, false); else if (narrow_rows) launch_edge_rows_narrow(L, ea, F, false); else launch_edge_tc(L, ea, F, false);
+            launch_edge_rows_narrow(L, ea, F, false);
         }
         else { k_edge<F, false><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);
@@ -484,7 +485,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         k_dense<F, DENSE_OUT><<<grid_tiles, kThreads, smem_dense<F>(true, kWarps), L.s>>>(total, w.m, net.Wo1T[t], net.Wo2T[t], w.h[t], w.x, nullptr); LSD_COUNT(L);
         prof_end(L, pid);
     }
-    const bool pairs = use_tc && narrow_rows;                   // (y, mbar) pair rows for k_edge_rows
+    const bool pairs = use_tc;                                  // (y, mbar) pair rows for k_edge_rows
     if (chain1) {
         const int pidc = prof_begin(L, PROF_DENSE);
         const int cw = 16, grid_c = std::max(1, std::min(sms * 2, (total + cw - 1) / cw));
@@ -508,7 +509,7 @@ void run_fp32(Launcher L, const SysDev& sys, const MlipDev& net, MlipWork& w, in
         pid = prof_begin(L, PROF_EDGE_BWD);
         if (use_tc) {
             ea.Wf1_tc = net.Wf1_bf16[t]; ea.Wf2_tc = net.Wf2_bf16[t]; ea.y16 = w.y16[t]; ea.mbar16 = w.mbar16; ea.ym16 = w.ym16;
-            if (F == 128) launch_edge_tc128(L, ea, true); else if (narrow_rows) launch_edge_rows_narrow(L, ea, F, true); else launch_edge_tc(L, ea, F, true);
+            launch_edge_rows_narrow(L, ea, F, true);
         }
         else { k_edge<F, true><<<grid_atoms, kThreads, smem_edge<F>(kWarps), L.s>>>(ea); LSD_COUNT(L); }
         prof_end(L, pid);

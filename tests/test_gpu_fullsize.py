@@ -140,14 +140,12 @@ def test_full_size_forces_match_oracle(P, orc, name, prec, states):
         assert fwd["width"] == w.target.mlip.width and bwd["width"] == w.target.mlip.width     # the target's launches were the last ones
         if w.target.mlip.width == 128:
             # the kernels the cfg5 / cfg4 bench lines time, with a grid that fills the device
-            if os.environ.get("LSD_EDGE_TMA", "0") not in ("", "0"):
-                assert bwd["kernel"] == "k_edge_rows_tma"      # tests/test_gpu_variants.py: the switch reached the kernel
-            if os.environ.get("LSD_EDGE_FWD4") == "0":
-                assert fwd["kernel"] == "k_edge_er128_fwd"
-            assert bwd["kernel"] in ("k_edge_rows", "k_edge_rows_tma", "k_edge_pipe", "k_edge_tc128") and fwd["kernel"] in ("k_edge_er128_fwd", "k_edge_rows", "k_edge_pipe", "k_edge_fwd4")
+            tma = os.environ.get("LSD_EDGE_TMA", "0") not in ("", "0")          # tests/test_gpu_variants.py: the switch reached the kernel
+            assert bwd["kernel"] == ("k_edge_rows_tma" if tma else "k_edge_rows")
+            assert fwd["kernel"] == ("k_edge_rows" if os.environ.get("LSD_EDGE_FWD4") == "0" else "k_edge_fwd4")
             assert bwd["grid"] >= 148 and fwd["grid"] >= 148
-            if bwd["kernel"] == "k_edge_tc128":
-                assert bwd["atoms_per_chunk"] == 64                # not the small-batch instantiation
+        else:
+            assert bwd["kernel"] == fwd["kernel"] == "k_edge_rows_narrow"
     tol = 2e-2 if bf16 else 1e-5
     for j in states:
         Eo, Fo = orc.energy_forces(w, w.target, np.ascontiguousarray(qh[j].T))

@@ -1,7 +1,8 @@
 """The opt-in / fallback edge kernels stay parity-green: the same full-size force parity case (cfg4, bf16, width 128, against the
 oracle) is run in a child process per environment switch (the switches are read once per process).
 DESIGN.md section 4.1: LSD_EDGE_TMA=1 gathers the backward's rows with TMA gather4 into 128-byte swizzled regions;
-LSD_EDGE_FWD4=0 is the round-1 forward (k_edge_er128_fwd); LSD_EDGE_ROWS=0 the round-1 backward (k_edge_tc128)."""
+LSD_EDGE_FWD4=0 runs the forward instantiation of k_edge_rows (two tiles in flight) instead of k_edge_fwd4.  These are the only
+two kernel switches the library still reads (the round-1 / opt-in kernel families behind the others were removed in round 3)."""
 import os
 import subprocess
 import sys
@@ -12,7 +13,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("env", [{"LSD_EDGE_TMA": "1"}, {"LSD_EDGE_FWD4": "0"}, {"LSD_EDGE_ROWS": "0"}])
+@pytest.mark.parametrize("env", [{"LSD_EDGE_TMA": "1"}, {"LSD_EDGE_FWD4": "0"}])
 def test_edge_kernel_variant_matches_oracle(env):
     e = dict(os.environ)
     e.update(env)
